@@ -1,0 +1,246 @@
+"""CAS hot-path ORACLE (integer bookkeeping) -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Pure-Python (arbitrary-precision ints, lists, sorts) restatement of the budget manager's integer
+state machine: slot tables (K1), swap round-trip accounting (K2), the rotation plan (K3) and the
+per-step protocol (K4) of DESIGN.md "Bookkeeping".  The CUDA library implements the same rules
+independently in C++ (``csrc/cas_host.cpp``); the two share no code and are compared bit-exactly.
+
+Passages followed:
+  * PAPER.md:73 (sec. 2.1 Budget Manager): "maintains a fixed GPU pool of B <= N cartridges, keeping
+    the remaining N-B cartridges offloaded to CPU memory"; samples only from active cartridges.
+  * PAPER.md:75 (Pool rotation): "a fraction phi of the pool is evicted and replaced with new
+    cartridges from persistent storage ... preferentially swaps in cartridges that have received
+    the fewest optimizer steps"; Table 5 "Prioritize least trained: Yes".
+  * BASELINE.json configs[2]: "swap in 16 priority-drawn cartridges and evict 16 LRU".
+  * per-sample cartridge subsets -> per-sequence slot lists.
+Tie-breaks the paper does not give are DESIGN.md readings R13-R16.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+from typing import List, Optional, Sequence, Tuple
+
+MASK64 = (1 << 64) - 1
+
+DIR_OUT = 0
+DIR_IN = 1
+
+
+def mix64(seed: int, step: int, cart: int) -> int:
+    """DESIGN.md R15: priority hash = SplitMix64 finaliser of
+    seed + 0x9E3779B97F4A7C15*(step+1) + 0xD1B54A32D192ED03*(cart+1)  (mod 2^64)."""
+    z = (seed + 0x9E3779B97F4A7C15 * (step + 1) + 0xD1B54A32D192ED03 * (cart + 1)) & MASK64
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & MASK64
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & MASK64
+    return z ^ (z >> 31)
+
+
+class BookError(Exception):
+    def __init__(self, code: str, msg: str = ""):
+        super().__init__(f"{code}: {msg}")
+        self.code = code
+
+
+@dataclass
+class ManifestEntry:
+    cart: int
+    slot: int
+    dir: int
+    host_off: int
+    nbytes: int
+
+    def as_tuple(self):
+        return (self.cart, self.slot, self.dir, self.host_off, self.nbytes)
+
+
+class PoolBook:
+    """Integer state of the cartridge pool."""
+
+    def __init__(self, cart_len: Sequence[int], n_slots: int, Hkv: int, D: int,
+                 tile_tokens: int = 128):
+        self.cart_len = [int(x) for x in cart_len]
+        self.n_carts = len(self.cart_len)
+        self.n_slots = int(n_slots)
+        self.row_elems = Hkv * D
+        self.tile = tile_tokens
+        up = lambda x: (x + tile_tokens - 1) // tile_tokens * tile_tokens
+        # slot capacities: everything resident -> slot s is sized for cartridge s;
+        # otherwise uniform slots sized for the longest cartridge.
+        if self.n_slots == self.n_carts:
+            self.slot_cap = [up(l) for l in self.cart_len]
+        else:
+            cap = up(max(self.cart_len))
+            self.slot_cap = [cap] * self.n_slots
+        self.slot_base = [0] * self.n_slots
+        for s in range(1, self.n_slots):
+            self.slot_base[s] = self.slot_base[s - 1] + self.slot_cap[s - 1]
+        self.pool_tokens = self.slot_base[-1] + self.slot_cap[-1] if self.n_slots else 0
+        # pinned homes: 6 fp32 tensors (pK,pV,mK,mV,vK,vV) of len*Hkv*D per cartridge, packed
+        self.home_off = [0] * self.n_carts
+        for c in range(1, self.n_carts):
+            self.home_off[c] = self.home_off[c - 1] + self.home_bytes(c - 1)
+        # state: the first n_slots cartridges start resident, slot s <- cartridge s
+        self.slot_of = [-1] * self.n_carts
+        self.cart_in = [-1] * self.n_slots
+        for s in range(min(self.n_slots, self.n_carts)):
+            self.slot_of[s] = s
+            self.cart_in[s] = s
+        self.opt_steps = [0] * self.n_carts
+        self.last_used = [-1] * self.n_carts
+        self.in_transit = [0] * self.n_carts        # 0 stable, 1 leaving, 2 arriving
+        self.grad_dirty = [0] * self.n_slots
+        self.pending: List[Tuple[ManifestEntry, int]] = []   # (entry, plan step)
+
+    def home_bytes(self, c: int) -> int:
+        return 6 * self.cart_len[c] * self.row_elems * 4
+
+    # ---- K1 ---------------------------------------------------------------------------------
+    def slot_table(self, seq_off: Sequence[int], sel_off: Sequence[int], sel_cart: Sequence[int],
+                   step: int):
+        B = len(seq_off) - 1
+        if B < 1 or len(sel_off) != B + 1 or seq_off[0] != 0 or sel_off[0] != 0:
+            raise BookError("INVALID_ARG", "offsets")
+        for b in range(B):
+            if seq_off[b + 1] <= seq_off[b]:
+                raise BookError("SHAPE", "Lq_b >= 1 required")
+            if sel_off[b + 1] < sel_off[b]:
+                raise BookError("INVALID_ARG", "sel_off not monotone")
+        if sel_off[B] != len(sel_cart):
+            raise BookError("INVALID_ARG", "sel_off[B] != nsel")
+        sel_slot = []
+        P = []
+        for b in range(B):
+            seen = set()
+            pb = 0
+            for k in range(sel_off[b], sel_off[b + 1]):
+                c = int(sel_cart[k])
+                if c < 0 or c >= self.n_carts:
+                    raise BookError("INVALID_ARG", "cartridge id")
+                if c in seen:
+                    raise BookError("INVALID_ARG", "duplicate cartridge in one sequence")
+                seen.add(c)
+                if self.slot_of[c] < 0:
+                    raise BookError("NOT_RESIDENT", str(c))
+                if self.in_transit[c]:
+                    raise BookError("BUSY", str(c))
+                sel_slot.append(self.slot_of[c])
+                pb += self.cart_len[c]
+            P.append(pb)
+        for c in set(int(x) for x in sel_cart):
+            self.last_used[c] = step
+        # inverted CSR: entries sorted by (slot asc, sequence asc)
+        pairs = sorted((sel_slot[k], b) for b in range(B) for k in range(sel_off[b], sel_off[b + 1]))
+        inv_off = [0] * (self.n_slots + 1)
+        for s, _ in pairs:
+            inv_off[s + 1] += 1
+        for s in range(self.n_slots):
+            inv_off[s + 1] += inv_off[s]
+        inv_seq = [b for _, b in pairs]
+        return sel_slot, inv_off, inv_seq, P
+
+    # ---- K3 ---------------------------------------------------------------------------------
+    def plan_rotation(self, step: int, n_in: int, n_out: int, protect: Sequence[int], seed: int
+                      ) -> List[ManifestEntry]:
+        prot = set(int(c) for c in protect)
+        evictable = [c for c in range(self.n_carts)
+                     if self.slot_of[c] >= 0 and not self.in_transit[c] and c not in prot]
+        evictable.sort(key=lambda c: (self.last_used[c], c))
+        evictees = evictable[:max(0, n_out)]
+        waiting = [c for c in range(self.n_carts) if self.slot_of[c] < 0 and not self.in_transit[c]]
+        waiting.sort(key=lambda c: (self.opt_steps[c], mix64(seed, step, c), c))
+        free = [s for s in range(self.n_slots) if self.cart_in[s] < 0]
+        free += [self.slot_of[c] for c in evictees]
+        free.sort()
+        arrivals = []
+        used = set()
+        for c in waiting:
+            if len(arrivals) >= max(0, n_in):
+                break
+            # first free slot (ascending) that is large enough and not yet paired
+            for s in free:
+                if s not in used and self.slot_cap[s] >= self.cart_len[c]:
+                    used.add(s)
+                    arrivals.append((c, s))
+                    break
+        outs = sorted(((self.slot_of[c], c) for c in evictees))
+        man = [ManifestEntry(c, s, DIR_OUT, self.home_off[c], self.home_bytes(c)) for s, c in outs]
+        man += [ManifestEntry(c, s, DIR_IN, self.home_off[c], self.home_bytes(c))
+                for c, s in arrivals]
+        return man
+
+    # ---- K4 (state transitions of swap_out / swap_in / commit / adam) -------------------------
+    def swap_out(self, man: Sequence[ManifestEntry], step: int):
+        for e in man:
+            if e.dir != DIR_OUT:
+                continue
+            if self.slot_of[e.cart] != e.slot or self.in_transit[e.cart]:
+                raise BookError("NOT_RESIDENT" if self.slot_of[e.cart] != e.slot else "BUSY")
+            if self.grad_dirty[e.slot]:
+                raise BookError("BUSY", "un-consumed grads")
+        for e in man:
+            if e.dir == DIR_OUT:
+                self.in_transit[e.cart] = 1
+                self.pending.append((e, step))
+
+    def swap_in(self, man: Sequence[ManifestEntry], step: int):
+        leaving = {e.slot for e, _ in self.pending if e.dir == DIR_OUT}
+        for e in man:
+            if e.dir != DIR_IN:
+                continue
+            if self.slot_of[e.cart] >= 0 or self.in_transit[e.cart]:
+                raise BookError("BUSY", "arrival already resident / in transit")
+            if not (self.cart_in[e.slot] < 0 or e.slot in leaving):
+                raise BookError("BUSY", "slot occupied")
+            if self.slot_cap[e.slot] < self.cart_len[e.cart]:
+                raise BookError("CAPACITY")
+        for e in man:
+            if e.dir == DIR_IN:
+                self.in_transit[e.cart] = 2
+                self.pending.append((e, step))
+
+    def commit(self):
+        for e, step in self.pending:
+            if e.dir == DIR_OUT:
+                self.slot_of[e.cart] = -1
+                self.in_transit[e.cart] = 0
+                if self.cart_in[e.slot] == e.cart:
+                    self.cart_in[e.slot] = -1
+        for e, step in self.pending:
+            if e.dir == DIR_IN:
+                self.slot_of[e.cart] = e.slot
+                self.cart_in[e.slot] = e.cart
+                self.in_transit[e.cart] = 0
+                self.last_used[e.cart] = step
+        self.pending = []
+
+    def mark_grads(self, sel_slot: Sequence[int]):
+        for s in set(sel_slot):
+            self.grad_dirty[s] = 1
+
+    def adam_slots(self, slots: Optional[Sequence[int]] = None) -> List[int]:
+        """Slots an adam_step covers: the given list, or every resident, not-in-transit slot
+        (ascending).  Increments opt_steps of their cartridges, clears grad_dirty."""
+        if slots is None:
+            slots = [s for s in range(self.n_slots)
+                     if self.cart_in[s] >= 0 and not self.in_transit[self.cart_in[s]]]
+        for s in slots:
+            c = self.cart_in[s]
+            if c < 0:
+                raise BookError("NOT_RESIDENT")
+            if self.in_transit[c]:
+                raise BookError("BUSY")
+        for s in slots:
+            self.opt_steps[self.cart_in[s]] += 1
+            self.grad_dirty[s] = 0
+        return list(slots)
+
+    def stable_resident(self) -> List[int]:
+        return [c for c in range(self.n_carts) if self.slot_of[c] >= 0 and not self.in_transit[c]]
+
+
+def position_offsets(book: PoolBook, P: Sequence[int]):
+    """query position ids are offset by the number of active cartridge KV tokens.
+    Returns (sum of resident cartridge lengths  [the packed layout of PAPER.md:71, every active
+    cartridge sits in the prompt], per-sequence visible prefix lengths P_b)  -- DESIGN.md R7."""
+    tot = sum(book.cart_len[c] for c in range(book.n_carts) if book.slot_of[c] >= 0)
+    return tot, list(P)
