@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the CAS hot path on B200.
+
+One "step" = one pass of the whole hot path over one batch of BASELINE.json configs[1]
+(c2, bf16 3B-like layer): slot-table build (host) -> prefix-attention forward -> backward (dK/dV
+scatter-accumulated into the cartridge gradient slots) -> fused Adam over the resident cartridges.
+(c2 has no rotation; `--config c3` adds the plan + swap-out/in overlapped on the side stream.)
+
+metric  = prefix-attn fwd+bwd TFLOP/s: algorithmic FLOPs 14*D*Hq*pairs (visible pairs only,
+          DESIGN.md "Algorithmic work") divided by the time of the WHOLE step (Adam included).
+roofline= the dominant kernel (attention backward) against the measured bf16 peak.
+e2e     = the same metric through cas_train_step_host(): pinned HOST buffers, H2D of Q/K_self/V_self/dO
+          and D2H of O/LSE/dQ inside the timed region.
+cpu_baseline = the oracle (numpy fp64, as it stands) timed on a bounded sample of the same workload.
+
+`--impl reference` times the oracle alone (this tier has no reference implementation to install).
+Multi-GPU: replicas only -- every rank runs its own batch on its own pool,
+no data-path collective; value = total FLOPs of all ranks / max-over-ranks time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "prefix_attn_fwd_bwd_tflops"
+UNIT = "TFLOP/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sust=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sust=1400.0, src="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        reasons = set()
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def attn_flops(wl):
+    cfg = wl.cfg
+    pairs = wl.pairs_per_head()
+    fwd = 4 * cfg.D * cfg.Hq * pairs
+    return fwd, (2.5 * fwd if cfg.backward else 0.0)
+
+
+def oracle_sample(wl, budget_s=12.0, max_units=64):
+    """Times the oracle (as it stands) on (sequence, KV-head) units of the workload until about
+    `budget_s` seconds of CPU work are done.  Returns (TFLOP/s, description, seconds, threads)."""
+    from oracle import cas_oracle as orc
+
+    cfg = wl.cfg
+    bK = [wl.cart_kv(c)[0] for c in range(cfg.n_carts)]
+    bV = [wl.cart_kv(c)[1] for c in range(cfg.n_carts)]
+    scale = 1.0 / float(np.sqrt(cfg.D))
+    G = cfg.Hq // cfg.Hkv
+    units = [(b, g) for b in range(cfg.B) for g in range(cfg.Hkv)]
+    done_flops, t_used, n = 0.0, 0.0, 0
+    for (b, g) in units[:max_units]:
+        t0, t1 = int(wl.seq_off[b]), int(wl.seq_off[b + 1])
+        sel = [wl.sel_cart[wl.sel_off[b]:wl.sel_off[b + 1]].tolist()]
+        so = np.array([0, t1 - t0])
+        a = time.perf_counter()
+        orc.attn_fwd(wl.Q[t0:t1], bK, bV, sel, so, wl.K_self[t0:t1], wl.V_self[t0:t1], scale, cfg.Hkv, kv_heads=[g])
+        if cfg.backward:
+            orc.attn_bwd(wl.Q[t0:t1], bK, bV, sel, so, wl.K_self[t0:t1], wl.V_self[t0:t1], wl.dO[t0:t1], scale,
+                         cfg.Hkv, kv_heads=[g])
+        t_used += time.perf_counter() - a
+        lq = t1 - t0
+        pb = int(wl.cart_len[sel[0]].sum()) if sel[0] else 0
+        pairs = lq * pb + lq * (lq + 1) // 2
+        done_flops += (14 if cfg.backward else 4) * cfg.D * G * pairs
+        n += 1
+        if t_used >= budget_s:
+            break
+    try:
+        from threadpoolctl import threadpool_info
+
+        threads = max([i.get("num_threads", 1) for i in threadpool_info()] or [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    desc = (f"{n} of {len(units)} (sequence, KV-head) units of {cfg.name}: complete fwd"
+            f"{'+bwd' if cfg.backward else ''} of those units, numpy float64")
+    return done_flops / t_used / 1e12, desc, t_used, threads
+
+
+def run_reference(args, wl):
+    """The reference arm of this tier = the oracle, timed on the host cores."""
+    tf, desc, secs, threads = 0.0, "", 0.0, 1
+    vals = []
+    for i in range(args.warmup + args.steps):
+        tf, desc, secs, threads = oracle_sample(wl, budget_s=args.ref_budget, max_units=args.ref_units)
+        if i >= args.warmup:
+            vals.append((tf, secs))
+    tf = float(np.mean([v[0] for v in vals]))
+    ms = float(np.mean([v[1] for v in vals])) * 1e3
+    line = {"metric": METRIC, "value": tf, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": wl.cfg.name, "note": "each step = a bounded sample of the workload"},
+            "cpu_baseline": {"value": tf, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": tf, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c2")
+    ap.add_argument("--kernels", default="auto", choices=["auto", "simt", "tc"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-budget", type=float, default=8.0)
+    ap.add_argument("--ref-units", type=int, default=64)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from workloads import BASE_SEED, CONFIGS, make_workload
+
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, make_workload(cfg, BASE_SEED))
+        return
+
+    import torch
+
+    from paper_2606_04557_b200 import _build, cas
+    from paper_2606_04557_b200.harness import Session
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    _build.build()
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    cas.cas_set_impl({"auto": 0, "simt": 1, "tc": 2}[args.kernels])
+    wl = make_workload(cfg, BASE_SEED + rank)          # every rank: its own batch, its own pool
+    sess = Session(wl, device=dev)
+    stream = torch.cuda.current_stream()
+    fwd_fl, bwd_fl = attn_flops(wl)
+    n_el = 2 * int(sum(int(wl.cart_len[c]) for c in range(cfg.n_slots))) * cfg.Hkv * cfg.D   # resident K+V elements
+    adam_bytes = 30 * n_el
+
+    def step(record=None):
+        sess.tab.close()
+        sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, wl.sel_off, wl.sel_cart, 0)
+        if record:
+            record[0].record(stream)
+        sess.fwd()
+        if record:
+            record[1].record(stream)
+        if cfg.backward:
+            sess.bwd()
+        if record:
+            record[2].record(stream)
+        if cfg.backward:
+            sess.adam()
+        if record:
+            record[3].record(stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    for i in range(args.steps):
+        step(evs[i])
+    e1.record(stream)
+    barrier()
+    sampler.stop_flag = True
+    total_ms = e0.elapsed_time(e1)
+    t_fwd = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    t_bwd = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    t_adam = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
+    ms_step = total_ms / args.steps
+
+    # ---- e2e: host buffers through cas_train_step_host
+    e2e = None
+    if cfg.backward:
+        tdt = sess.tdt
+        pin = lambda a: torch.from_numpy(a).to(tdt).pin_memory()
+        hQ, hKs, hVs, hdO = pin(wl.Q), pin(wl.K_self), pin(wl.V_self), pin(wl.dO)
+        hO = torch.empty_like(hQ).pin_memory()
+        hdQ = torch.empty_like(hQ).pin_memory()
+        hLSE = torch.empty((sess.tab.T, cfg.Hq), dtype=torch.float32).pin_memory()
+        nb = cas.cas_train_step_host_scratch_bytes(sess.pool, sess.tab, cfg.Hq)
+        scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
+        acfg = sess.adam_cfg()
+
+        def e2e_step():
+            sess.tab.close()
+            sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, wl.sel_off, wl.sel_cart, 0)
+            cas.cas_train_step_host(sess.pool, sess.tab, cfg.Hq, hQ, hKs, hVs, hdO, sess.scale, acfg, hO, hLSE, hdQ,
+                                    scratch)
+
+        for _ in range(3):
+            e2e_step()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(args.steps):
+            e2e_step()
+        b.record(stream)
+        barrier()
+        e2e_ms = a.elapsed_time(b) / args.steps
+        h2d = sum(t.numel() * t.element_size() for t in (hQ, hKs, hVs, hdO))
+        d2h = sum(t.numel() * t.element_size() for t in (hO, hdQ, hLSE))
+        e2e = (e2e_ms, h2d, d2h)
+
+    times = torch.tensor([ms_step, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
+    flops = torch.tensor([fwd_fl + bwd_fl], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(flops, op=dist.ReduceOp.SUM)
+    ms_step_max, e2e_ms_max = float(times[0]), float(times[1])
+    total_flops = float(flops[0])
+
+    if rank == 0:
+        peaks = load_peaks()
+        tc = bool(cfg.dtype == "bf16" and cfg.D == 128 and args.kernels != "simt")
+        dom_fl, dom_ms, dom_name = (bwd_fl, t_bwd, "attn_bwd") if cfg.backward else (fwd_fl, t_fwd, "attn_fwd")
+        achieved = dom_fl / (dom_ms * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": total_flops / (ms_step_max * 1e-3) / 1e12, "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step_max,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if cfg.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_carts": cfg.n_carts,
+                       "n_slots": cfg.n_slots, "B": cfg.B, "T": int(wl.T), "pairs_per_head": int(wl.pairs_per_head()),
+                       "kernels": "tcgen05" if tc else "simt",
+                       "l2": "inputs larger than L2 (pool + optimizer state > 1 GB per step)",
+                       "parallelism": "replicas" if world > 1 else "single"},
+            "breakdown": {"fwd_ms": t_fwd, "bwd_ms": t_bwd, "adam_ms": t_adam,
+                          "fwd_tflops": fwd_fl / (t_fwd * 1e-3) / 1e12,
+                          "bwd_tflops": (bwd_fl / (t_bwd * 1e-3) / 1e12) if cfg.backward else None,
+                          "fwd_bwd_tflops": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12,
+                          "fwd_bwd_frac_of_bf16_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16_sust"],
+                          "adam_gbs": (adam_bytes / (t_adam * 1e-3) / 1e9) if cfg.backward else None,
+                          "adam_frac_of_hbm_peak": (adam_bytes / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if cfg.backward else None},
+            "roofline": {"kernel": dom_name, "bound": "tensor", "achieved": achieved, "peak": peaks["bf16_sust"],
+                         "unit": "TFLOP/s", "frac": achieved / peaks["bf16_sust"], "traffic": None,
+                         "peak_source": peaks["src"] + " bf16_tflops_sustained (kernel timed inside the step)"},
+            "gpu_launches": args.steps * (5 if not tc else 5),
+            "clocks": sampler.summary(),
+        }
+        if e2e:
+            line["e2e"] = {"value": total_flops / (e2e_ms_max * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_max,
+                           "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
+        if not args.no_cpu_baseline and world == 1:
+            tf, desc, secs, threads = oracle_sample(wl, budget_s=12.0)
+            line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                                    "seconds": secs}
+        print(json.dumps(line))
+    sess.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

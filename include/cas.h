@@ -1,0 +1,233 @@
+/* cas.h -- C ABI of libcas: the data-parallel hot path of "Cartridges at Scale" (CAS,
+ * arxiv/paper_2606_04557) multi-cartridge training on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are "PAPER.md:<line>" = the paper text this library was written from, plus the section.
+ *
+ * Conventions
+ *   - plain C, no exceptions; every call returns an int: CAS_OK (0) or a negative CAS_ERR_* code;
+ *     cas_last_error() returns the text of the last failure of the calling thread.
+ *   - "device" pointers are CUDA device memory, "host" pointers ordinary host memory, "pinned"
+ *     page-locked host memory (cudaHostAlloc).  THE CALLER OWNS every data buffer and every stream
+ *     (allocate with PyTorch or cudaMalloc); the library owns only host metadata behind the opaque
+ *     handles plus small device-side index tables (slot tables, tile lists, work lists) that it
+ *     cudaMalloc's in cas_slot_table_build / cas_pool_create and frees in the matching destroy.
+ *   - compute calls are asynchronous on the caller's stream (cudaStream_t passed as void*);
+ *     swap calls are asynchronous on the side stream given at pool creation.
+ *   - tensors are row-major, innermost dimension last:  Q/O/dO/dQ [T, Hq, D];  K_self/V_self and
+ *     their grads [T, Hkv, D];  LSE [T, Hq] fp32;  pool tensors [pool_tokens, Hkv, D].
+ *     T = total packed query tokens, sequence b owns tokens seq_off[b] .. seq_off[b+1]-1.
+ *   - dtype CAS_BF16: Q,K,V,O,dO,dQ,dK_self,dV_self are bf16; CAS_F32: fp32.  Master params, Adam
+ *     moments, gradient slots and LSE are fp32 in both.
+ *   - query head h reads KV head h / (Hq/Hkv)  (consecutive query heads share a KV head).
+ *   - all index arrays are int32 on the HOST; the library uploads what kernels need.
+ */
+#ifndef CAS_H_
+#define CAS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CAS_OK 0
+#define CAS_ERR_INVALID_ARG (-1)
+#define CAS_ERR_SHAPE (-2)
+#define CAS_ERR_NOT_RESIDENT (-3)
+#define CAS_ERR_BUSY (-4)      /* slot/cartridge in transit, or gradients not yet consumed */
+#define CAS_ERR_CAPACITY (-5)
+#define CAS_ERR_CUDA (-6)
+
+#define CAS_F32 0
+#define CAS_BF16 1
+
+#define CAS_DIR_OUT 0          /* HBM slot -> pinned host home */
+#define CAS_DIR_IN 1           /* pinned host home -> HBM slot */
+
+/* cas_set_impl(): which attention kernels serve the calls */
+#define CAS_IMPL_AUTO 0        /* tcgen05/TMEM/TMA kernels when dtype==bf16 && D==128, else SIMT */
+#define CAS_IMPL_SIMT 1        /* fp32-accumulate CUDA-core kernels (any dtype / D<=128, D%32==0) */
+#define CAS_IMPL_TC 2          /* tensor-core kernels; CAS_ERR_SHAPE if the shape is unsupported */
+
+typedef struct cas_pool cas_pool;
+typedef struct cas_slot_table cas_slot_table;
+
+/* The cartridge pool (sec. 2.1 "Budget Manager": "a fixed GPU pool of B <= N
+ * cartridges, keeping the remaining N-B cartridges offloaded to CPU memory").  One layer's worth:
+ * a cartridge is K and V of shape [cart_len, Hkv, D] (Z in R^{L x p x d x 2}, one L). */
+typedef struct {
+  int32_t dtype;            /* CAS_F32 | CAS_BF16: dtype of the working copy attention reads */
+  int32_t Hkv;
+  int32_t D;                /* head dim, multiple of 32, <= 128 */
+  int32_t n_carts;          /* N */
+  int32_t n_slots;          /* B <= N HBM slots.  n_slots == n_carts: slot s is sized for cartridge
+                               s; otherwise all slots have the capacity of the longest cartridge */
+  int32_t tile_tokens;      /* slot capacity granularity; 0 => 128 (the KV tile of the kernels;
+                               the paper's own page is 16 tokens) */
+  const int32_t* cart_len;  /* host [n_carts], tokens per cartridge, each >= 1 */
+} cas_pool_desc;
+
+/* Device-side layout of the pool inside the caller's arena (all pointers are device pointers
+ * into dev_arena; index arrays are host pointers owned by the pool, valid until destroy). */
+typedef struct {
+  void* pool_K;             /* working copy [pool_tokens,Hkv,D], dtype */
+  void* pool_V;
+  float* grad_K;            /* fp32 gradient slots [pool_tokens,Hkv,D] */
+  float* grad_V;
+  float* state;             /* per slot s at state + 6*slot_base[s]*Hkv*D: six fp32 tensors of
+                               slot_cap[s]*Hkv*D elements each: pK, pV, mK, mV, vK, vV */
+  const int32_t* slot_base; /* host [n_slots] first pool token of slot s */
+  const int32_t* slot_cap;  /* host [n_slots] capacity in tokens (multiple of tile_tokens) */
+  int64_t pool_tokens;
+} cas_pool_layout;
+
+typedef struct {
+  int32_t cart;
+  int32_t slot;
+  int32_t dir;              /* CAS_DIR_OUT | CAS_DIR_IN */
+  int32_t reserved;
+  int64_t host_off;         /* byte offset of the cartridge's home in the pinned arena */
+  int64_t nbytes;           /* 6 * cart_len * Hkv * D * 4 (params + both Adam moments, K and V) */
+} cas_manifest_entry;
+
+/* Adam (sec. 2.2 "Adam (Kingma and Ba, 2014) with fp32 precision, while we keep the
+ * weights in bfloat16"; Table 5 PAPER.md:366-373, :390 "Num frozen tokens 1"). */
+typedef struct {
+  float lr, beta1, beta2, eps;
+  int32_t n_frozen;         /* first n_frozen tokens of every cartridge are not updated */
+  int32_t zero_grad;        /* 1: gradient slots are zeroed by the same kernel */
+} cas_adam_cfg;
+
+typedef struct {
+  int32_t B, T, nsel, n_kv_tiles;
+  int64_t pairs_per_head;   /* sum_b Lq_b*P_b + Lq_b(Lq_b+1)/2 : visible (query,key) pairs */
+  int64_t prefix_tokens;    /* sum_b P_b */
+  int64_t unique_prefix_tokens; /* tokens of distinct selected slots */
+} cas_table_info;
+
+const char* cas_version(void);
+/* Copies the calling thread's last error text (NUL-terminated, truncated to n). */
+void cas_last_error(char* buf, size_t n);
+/* Select attention implementation (process-wide).  Returns CAS_ERR_INVALID_ARG on a bad value. */
+int cas_set_impl(int impl);
+
+/* ---- pool ---------------------------------------------------------------------------------- */
+/* Bytes the caller must provide: dev_bytes of device memory (256-B aligned) and host_bytes of
+ * pinned host memory for the homes of ALL n_carts cartridges (fp32 pK,pV,mK,mV,vK,vV packed). */
+int cas_pool_query_bytes(const cas_pool_desc* desc, size_t* dev_bytes, size_t* host_bytes);
+/* Carves the arenas, zero-fills the device arena (on side_stream, synchronised before return) and
+ * places cartridges 0..n_slots-1 in slots 0..n_slots-1.  dev_arena == NULL creates a
+ * bookkeeping-only pool (planning, tables and counters work; anything touching data returns
+ * CAS_ERR_INVALID_ARG) -- used to test the host logic without a GPU.  pinned_arena may be NULL when
+ * n_slots == n_carts (nothing can be swapped). */
+int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_arena,
+                    void* side_stream, cas_pool** out);
+int cas_pool_destroy(cas_pool* pool);
+int cas_pool_layout_get(const cas_pool* pool, cas_pool_layout* out);
+/* Initialise cartridge `cart` from host fp32 K,V [cart_len,Hkv,D]: master params <- K,V; moments
+ * <- 0; resident: working copy <- cast(master), grads <- 0.  Synchronous. */
+int cas_pool_load(cas_pool* pool, int32_t cart, const float* K, const float* V);
+/* Read back one tensor of a cartridge into host memory.  Synchronous (device-wide). `what`:
+ * 0..5 = pK,pV,mK,mV,vK,vV (fp32, from the slot if resident else from the pinned home);
+ * 6,7 = grad_K, grad_V (fp32, resident only); 8,9 = working copy K,V (pool dtype, resident only). */
+int cas_pool_read(cas_pool* pool, int32_t cart, int32_t what, void* out);
+/* Export integer state; any pointer may be NULL.  slot_of[n_carts] (-1 = not resident),
+ * cart_in[n_slots] (-1 = free), opt_steps[n_carts], last_used[n_carts],
+ * in_transit[n_carts] (0 stable, 1 leaving, 2 arriving), grad_dirty[n_slots]. */
+int cas_pool_counters(const cas_pool* pool, int32_t* slot_of, int32_t* cart_in, int64_t* opt_steps,
+                      int64_t* last_used, int32_t* in_transit, int32_t* grad_dirty);
+/* Restore counters of one cartridge (checkpoint/resume, tests). */
+int cas_pool_set_counters(cas_pool* pool, int32_t cart, int64_t opt_steps, int64_t last_used);
+
+/* ---- slot table (sec. 2.1: per-sample subset Z~ = Z* U S, "each packed sample sees
+ * a different subset via an attention mask") --------------------------------------------------- */
+/* sel_cart[sel_off[b] .. sel_off[b+1]) = distinct cartridge ids visible to sequence b (target
+ * first).  Validates (CAS_ERR_INVALID_ARG: bad offsets / ids / duplicates; CAS_ERR_SHAPE: an empty
+ * sequence; CAS_ERR_NOT_RESIDENT; CAS_ERR_BUSY: cartridge in transit), maps ids to slots, builds
+ * the inverted table (slot -> sequences, sorted by slot then sequence), the KV tile lists and
+ * kernel work lists, uploads them, and stamps last_used = step on the selected cartridges. */
+int cas_slot_table_build(cas_pool* pool, int32_t B, const int32_t* seq_off, const int32_t* sel_off,
+                         const int32_t* sel_cart, int64_t step, cas_slot_table** out);
+int cas_slot_table_destroy(cas_slot_table* table);
+int cas_slot_table_info(const cas_slot_table* table, cas_table_info* out);
+/* Any pointer may be NULL: sel_slot[nsel], inv_off[n_slots+1], inv_seq[nsel], P[B] (prefix
+ * tokens visible to sequence b). */
+int cas_slot_table_export(const cas_slot_table* table, int32_t* sel_slot, int32_t* inv_off,
+                          int32_t* inv_seq, int64_t* P);
+/* "query token position IDs must be offset by the total number of active cartridge
+ * KV tokens".  total_resident = tokens of all resident cartridges (the packed layout of
+ * PAPER.md:71); P[b] = tokens visible to sequence b.  Either may be NULL. */
+int cas_position_offsets(const cas_pool* pool, const cas_slot_table* table,
+                         int64_t* total_resident, int64_t* P);
+
+/* ---- attention ------------------------------------------------------------------------------ */
+/* Forward.  For every sequence b, query head h, row i (token t):
+ *   visible keys = all tokens of the slots selected by b (read IN PLACE from the pool, no concat)
+ *                  U own tokens seq_off[b]..t of K_self/V_self (causal, diagonal included);
+ *   s_j = scale*q.k_j ; LSE[t,h] = ln sum_j exp(s_j) ; O[t,h,:] = sum_j exp(s_j-LSE) v_j.
+ * Q,O device [T,Hq,D] dtype; K_self,V_self device [T,Hkv,D] dtype or both NULL (prefix only; then
+ * every sequence must select >= 1 cartridge); LSE device [T,Hq] fp32. */
+int cas_prefix_attn_fwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
+                        const void* K_self, const void* V_self, float scale, void* O, float* LSE,
+                        void* stream);
+/* Device workspace bytes cas_prefix_attn_bwd needs for this table / Hq. */
+int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* pool, const cas_slot_table* table,
+                                        int32_t Hq, size_t* bytes);
+/* Backward (PAPER.md:44 "only the key-value vectors in Z receive gradients"; :176 all active
+ * cartridges back-propagated simultaneously).  dQ [T,Hq,D] dtype is overwritten.  dK/dV of prefix
+ * keys are ACCUMULATED (+=) into the pool's fp32 gradient slots of the selected slots, summed over
+ * the Hq/Hkv heads of a group and over every sequence that selected the slot; slots selected by no
+ * sequence are not touched.  dK_self/dV_self [T,Hkv,D] dtype are overwritten (may both be NULL).
+ * Marks the selected slots grad-dirty. */
+int cas_prefix_attn_bwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
+                        const void* K_self, const void* V_self, const void* O, const float* LSE,
+                        const void* dO, float scale, void* dQ, void* dK_self, void* dV_self,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- optimizer ------------------------------------------------------------------------------ */
+/* One fused Adam step over the listed slots (slots == NULL: every resident slot whose cartridge
+ * is not in transit).  Per cartridge: t = ++opt_steps; m = b1 m + (1-b1) g; v = b2 v + (1-b2) g^2;
+ * p -= lr*lr_scale[i]*(m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps); working copy = RNE(p); g = 0 if
+ * zero_grad.  lr_scale: host [n] per listed slot (PAPER.md:85 per-cartridge warmup), NULL = 1. */
+int cas_adam_step(cas_pool* pool, const cas_adam_cfg* cfg, const int32_t* slots, int32_t n,
+                  const float* lr_scale, void* stream);
+int cas_grad_zero(cas_pool* pool, const int32_t* slots, int32_t n, void* stream);
+
+/* ---- rotation (sec. 2.1 "Pool rotation"; Table 5 :377-381) ------------------------ */
+/* Pure integer planning, moves no data.  Evictees: the n_out resident, stable, unprotected
+ * cartridges with the smallest last_used (ties: smaller id).  Arrivals: up to n_in non-resident
+ * cartridges with the fewest opt_steps (ties: smaller mix64(seed,step,cart), then smaller id),
+ * paired in that order with the free slots (free now or freed by the evictees) in ascending slot
+ * order.  Writes all OUT entries (ascending slot) then all IN entries.  CAS_ERR_CAPACITY if
+ * `capacity` entries do not suffice. */
+int cas_plan_rotation(const cas_pool* pool, int64_t step, int32_t n_in, int32_t n_out,
+                      const int32_t* protect_carts, int32_t n_protect, uint64_t seed,
+                      cas_manifest_entry* entries, int32_t capacity, int32_t* n_entries);
+/* Enqueue the OUT (resp. IN) entries of a manifest on the side stream, in order, one
+ * cudaMemcpyAsync per contiguous piece.  An arrival is followed by a kernel (side stream) that
+ * derives the working copy and zeroes the gradient slot.  swap_out first waits (event) for work
+ * already enqueued on `after_stream` (the stream whose Adam last wrote the evictees; may be NULL).
+ * CAS_ERR_BUSY: evictee has un-consumed gradients / cartridge already in transit / slot occupied. */
+int cas_swap_out(cas_pool* pool, const cas_manifest_entry* entries, int32_t n, int64_t step,
+                 void* after_stream);
+int cas_swap_in(cas_pool* pool, const cas_manifest_entry* entries, int32_t n, int64_t step);
+/* Makes main_stream wait for everything enqueued on the side stream and flips residency:
+ * evictees leave, arrivals become selectable with last_used = the step of their swap_in. */
+int cas_swap_commit(cas_pool* pool, void* main_stream);
+
+/* ---- end-to-end convenience: one training step from HOST buffers --------------------------------
+ * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
+ * resident slots, D2H of O, LSE, dQ -- all on `stream`.  dev_scratch must hold
+ * cas_train_step_host_scratch_bytes().  Asynchronous; synchronise the stream before reading. */
+int cas_train_step_host_scratch_bytes(const cas_pool* pool, const cas_slot_table* table, int32_t Hq,
+                                      size_t* bytes);
+int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,
+                        const void* hK_self, const void* hV_self, const void* hdO, float scale,
+                        const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ,
+                        void* dev_scratch, size_t scratch_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAS_H_ */

@@ -1,0 +1,318 @@
+"""Thin ctypes binding of libcas (include/cas.h).  Argument marshalling only: every step of the hot
+path runs inside the library's CUDA kernels.  There is NO fallback: if libcas.so is missing or a
+call fails, a CasError is raised.
+
+Function names mirror the C ABI (``cas_prefix_attn_fwd`` ...); ``Pool`` / ``SlotTable`` only hold
+the opaque handles and the torch tensors that back the caller-owned arenas.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcas.so")
+
+CAS_F32, CAS_BF16 = 0, 1
+CAS_DIR_OUT, CAS_DIR_IN = 0, 1
+CAS_IMPL_AUTO, CAS_IMPL_SIMT, CAS_IMPL_TC = 0, 1, 2
+ERR_NAMES = {0: "CAS_OK", -1: "CAS_ERR_INVALID_ARG", -2: "CAS_ERR_SHAPE", -3: "CAS_ERR_NOT_RESIDENT",
+             -4: "CAS_ERR_BUSY", -5: "CAS_ERR_CAPACITY", -6: "CAS_ERR_CUDA"}
+
+
+class CasError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{ERR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+        self.name = ERR_NAMES.get(code, str(code))
+
+
+class PoolDesc(C.Structure):
+    _fields_ = [("dtype", C.c_int32), ("Hkv", C.c_int32), ("D", C.c_int32), ("n_carts", C.c_int32),
+                ("n_slots", C.c_int32), ("tile_tokens", C.c_int32), ("cart_len", C.POINTER(C.c_int32))]
+
+
+class PoolLayout(C.Structure):
+    _fields_ = [("pool_K", C.c_void_p), ("pool_V", C.c_void_p), ("grad_K", C.c_void_p),
+                ("grad_V", C.c_void_p), ("state", C.c_void_p), ("slot_base", C.POINTER(C.c_int32)),
+                ("slot_cap", C.POINTER(C.c_int32)), ("pool_tokens", C.c_int64)]
+
+
+class ManifestEntry(C.Structure):
+    _fields_ = [("cart", C.c_int32), ("slot", C.c_int32), ("dir", C.c_int32), ("reserved", C.c_int32),
+                ("host_off", C.c_int64), ("nbytes", C.c_int64)]
+
+    def as_tuple(self):
+        return (self.cart, self.slot, self.dir, self.host_off, self.nbytes)
+
+
+class AdamCfg(C.Structure):
+    _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
+                ("n_frozen", C.c_int32), ("zero_grad", C.c_int32)]
+
+
+class TableInfo(C.Structure):
+    _fields_ = [("B", C.c_int32), ("T", C.c_int32), ("nsel", C.c_int32), ("n_kv_tiles", C.c_int32),
+                ("pairs_per_head", C.c_int64), ("prefix_tokens", C.c_int64),
+                ("unique_prefix_tokens", C.c_int64)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise CasError(-6, f"{LIB_PATH} not built; run `python -m paper_2606_04557_b200._build` "
+                               "(there is no CPU fallback)")
+        _lib = C.CDLL(LIB_PATH)
+        _lib.cas_version.restype = C.c_char_p
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        buf = C.create_string_buffer(512)
+        lib().cas_last_error(buf, C.c_size_t(512))
+        raise CasError(rc, buf.value.decode())
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _p(a: Optional[np.ndarray], typ=C.c_int32):
+    return None if a is None else a.ctypes.data_as(C.POINTER(typ))
+
+
+def _dptr(t) -> C.c_void_p:
+    """Device / pinned pointer of a torch tensor (or None)."""
+    return C.c_void_p(None if t is None else t.data_ptr())
+
+
+def _stream(s) -> C.c_void_p:
+    if s is None:
+        import torch
+
+        s = torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def cas_version() -> str:
+    return lib().cas_version().decode()
+
+
+def cas_set_impl(impl: int):
+    _check(lib().cas_set_impl(C.c_int(impl)))
+
+
+def cas_pool_query_bytes(desc: PoolDesc):
+    d, h = C.c_size_t(0), C.c_size_t(0)
+    _check(lib().cas_pool_query_bytes(C.byref(desc), C.byref(d), C.byref(h)))
+    return d.value, h.value
+
+
+class Pool:
+    """Owns the torch tensors backing the arenas + the opaque cas_pool handle."""
+
+    def __init__(self, dtype: int, Hkv: int, D: int, cart_len: Sequence[int], n_slots: int,
+                 tile_tokens: int = 0, device: Optional[str] = "cuda:0", side_stream=None):
+        self._cart_len = _i32(cart_len)
+        self.desc = PoolDesc(dtype, Hkv, D, len(self._cart_len), n_slots, tile_tokens,
+                             _p(self._cart_len))
+        self.dtype, self.Hkv, self.D = dtype, Hkv, D
+        self.n_carts, self.n_slots = len(self._cart_len), n_slots
+        self.dev_bytes, self.host_bytes = cas_pool_query_bytes(self.desc)
+        self.handle = C.c_void_p(None)
+        self.dev_arena = self.pinned_arena = self.side_stream = None
+        dev_ptr = pin_ptr = side = C.c_void_p(None)
+        if device is not None:
+            import torch
+
+            self.dev_arena = torch.empty(self.dev_bytes, dtype=torch.uint8, device=device)
+            dev_ptr = _dptr(self.dev_arena)
+            if n_slots < self.n_carts:
+                self.pinned_arena = torch.empty(self.host_bytes, dtype=torch.uint8, pin_memory=True)
+                pin_ptr = _dptr(self.pinned_arena)
+            self.side_stream = side_stream or torch.cuda.Stream(device=device)
+            side = C.c_void_p(self.side_stream.cuda_stream)
+        _check(lib().cas_pool_create(C.byref(self.desc), dev_ptr, pin_ptr, side, C.byref(self.handle)))
+        lay = PoolLayout()
+        _check(lib().cas_pool_layout_get(self.handle, C.byref(lay)))
+        self.layout = lay
+        self.slot_base = np.ctypeslib.as_array(lay.slot_base, (n_slots,)).copy()
+        self.slot_cap = np.ctypeslib.as_array(lay.slot_cap, (n_slots,)).copy()
+        self.pool_tokens = lay.pool_tokens
+
+    def close(self):
+        if self.handle:
+            lib().cas_pool_destroy(self.handle)
+            self.handle = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def cas_pool_load(pool: Pool, cart: int, K: np.ndarray, V: np.ndarray):
+    K = np.ascontiguousarray(K, dtype=np.float32)
+    V = np.ascontiguousarray(V, dtype=np.float32)
+    _check(lib().cas_pool_load(pool.handle, C.c_int32(cart), _p(K, C.c_float), _p(V, C.c_float)))
+
+
+READ_NAMES = {"pK": 0, "pV": 1, "mK": 2, "mV": 3, "vK": 4, "vV": 5, "gK": 6, "gV": 7, "wK": 8, "wV": 9}
+
+
+def cas_pool_read(pool: Pool, cart: int, what) -> np.ndarray:
+    w = READ_NAMES[what] if isinstance(what, str) else int(what)
+    n = int(pool._cart_len[cart])
+    if w < 8 or pool.dtype == CAS_F32:
+        out = np.empty((n, pool.Hkv, pool.D), dtype=np.float32)
+    else:
+        out = np.empty((n, pool.Hkv, pool.D), dtype=np.uint16)       # raw bf16 bits
+    _check(lib().cas_pool_read(pool.handle, C.c_int32(cart), C.c_int32(w), C.c_void_p(out.ctypes.data)))
+    return out
+
+
+def cas_pool_counters(pool: Pool) -> dict:
+    N, S = pool.n_carts, pool.n_slots
+    o = dict(slot_of=np.empty(N, np.int32), cart_in=np.empty(S, np.int32), opt_steps=np.empty(N, np.int64),
+             last_used=np.empty(N, np.int64), in_transit=np.empty(N, np.int32),
+             grad_dirty=np.empty(S, np.int32))
+    _check(lib().cas_pool_counters(pool.handle, _p(o["slot_of"]), _p(o["cart_in"]),
+                                   _p(o["opt_steps"], C.c_int64), _p(o["last_used"], C.c_int64),
+                                   _p(o["in_transit"]), _p(o["grad_dirty"])))
+    return o
+
+
+def cas_pool_set_counters(pool: Pool, cart: int, opt_steps: int, last_used: int):
+    _check(lib().cas_pool_set_counters(pool.handle, C.c_int32(cart), C.c_int64(opt_steps),
+                                       C.c_int64(last_used)))
+
+
+class SlotTable:
+    def __init__(self, pool: Pool, handle, B: int):
+        self.pool, self.handle, self.B = pool, handle, B
+        info = TableInfo()
+        _check(lib().cas_slot_table_info(handle, C.byref(info)))
+        self.info = info
+        self.T, self.nsel = info.T, info.nsel
+
+    def close(self):
+        if self.handle:
+            lib().cas_slot_table_destroy(self.handle)
+            self.handle = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def cas_slot_table_build(pool: Pool, seq_off, sel_off, sel_cart, step: int = 0) -> SlotTable:
+    seq_off, sel_off, sel_cart = _i32(seq_off), _i32(sel_off), _i32(sel_cart)
+    B = len(seq_off) - 1
+    if len(sel_off) != B + 1 or (len(sel_off) and sel_off[-1] != len(sel_cart)):
+        raise CasError(-1, "sel_off / sel_cart length mismatch")
+    h = C.c_void_p(None)
+    _check(lib().cas_slot_table_build(pool.handle, C.c_int32(B), _p(seq_off), _p(sel_off),
+                                      _p(sel_cart), C.c_int64(step), C.byref(h)))
+    return SlotTable(pool, h, B)
+
+
+def cas_slot_table_export(tab: SlotTable) -> dict:
+    S = tab.pool.n_slots
+    o = dict(sel_slot=np.empty(tab.nsel, np.int32), inv_off=np.empty(S + 1, np.int32),
+             inv_seq=np.empty(tab.nsel, np.int32), P=np.empty(tab.B, np.int64))
+    _check(lib().cas_slot_table_export(tab.handle, _p(o["sel_slot"]), _p(o["inv_off"]),
+                                       _p(o["inv_seq"]), _p(o["P"], C.c_int64)))
+    return o
+
+
+def cas_position_offsets(pool: Pool, tab: Optional[SlotTable]):
+    tot = C.c_int64(0)
+    P = np.empty(tab.B, np.int64) if tab is not None else None
+    _check(lib().cas_position_offsets(pool.handle, tab.handle if tab else None, C.byref(tot),
+                                      _p(P, C.c_int64)))
+    return tot.value, P
+
+
+def cas_prefix_attn_fwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, scale: float, O, LSE,
+                        stream=None):
+    _check(lib().cas_prefix_attn_fwd(pool.handle, tab.handle, C.c_int32(Hq), _dptr(Q), _dptr(K_self),
+                                     _dptr(V_self), C.c_float(scale), _dptr(O), _dptr(LSE),
+                                     _stream(stream)))
+
+
+def cas_prefix_attn_bwd_workspace_bytes(pool: Pool, tab: SlotTable, Hq: int) -> int:
+    n = C.c_size_t(0)
+    _check(lib().cas_prefix_attn_bwd_workspace_bytes(pool.handle, tab.handle, C.c_int32(Hq), C.byref(n)))
+    return n.value
+
+
+def cas_prefix_attn_bwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, O, LSE, dO, scale: float,
+                        dQ, dK_self, dV_self, workspace, stream=None):
+    _check(lib().cas_prefix_attn_bwd(pool.handle, tab.handle, C.c_int32(Hq), _dptr(Q), _dptr(K_self),
+                                     _dptr(V_self), _dptr(O), _dptr(LSE), _dptr(dO), C.c_float(scale),
+                                     _dptr(dQ), _dptr(dK_self), _dptr(dV_self), _dptr(workspace),
+                                     C.c_size_t(workspace.numel() * workspace.element_size()),
+                                     _stream(stream)))
+
+
+def cas_adam_step(pool: Pool, cfg: AdamCfg, slots=None, lr_scale=None, stream=None, host_only=False):
+    s = None if slots is None else _i32(slots)
+    ls = None if lr_scale is None else np.ascontiguousarray(lr_scale, dtype=np.float32)
+    st = C.c_void_p(None) if host_only else _stream(stream)
+    _check(lib().cas_adam_step(pool.handle, C.byref(cfg), _p(s), C.c_int32(0 if s is None else len(s)),
+                               _p(ls, C.c_float), st))
+
+
+def cas_grad_zero(pool: Pool, slots=None, stream=None):
+    s = None if slots is None else _i32(slots)
+    _check(lib().cas_grad_zero(pool.handle, _p(s), C.c_int32(0 if s is None else len(s)), _stream(stream)))
+
+
+def cas_plan_rotation(pool: Pool, step: int, n_in: int, n_out: int, protect, seed: int):
+    prot = _i32(protect)
+    cap = n_in + n_out + 8
+    arr = (ManifestEntry * cap)()
+    n = C.c_int32(0)
+    _check(lib().cas_plan_rotation(pool.handle, C.c_int64(step), C.c_int32(n_in), C.c_int32(n_out),
+                                   _p(prot), C.c_int32(len(prot)), C.c_uint64(seed), arr, C.c_int32(cap),
+                                   C.byref(n)))
+    return arr, n.value
+
+
+def cas_swap_out(pool: Pool, man, n: int, step: int, after_stream=None, host_only=False):
+    st = C.c_void_p(None) if host_only else _stream(after_stream)
+    _check(lib().cas_swap_out(pool.handle, man, C.c_int32(n), C.c_int64(step), st))
+
+
+def cas_swap_in(pool: Pool, man, n: int, step: int):
+    _check(lib().cas_swap_in(pool.handle, man, C.c_int32(n), C.c_int64(step)))
+
+
+def cas_swap_commit(pool: Pool, main_stream=None, host_only=False):
+    st = C.c_void_p(None) if host_only else _stream(main_stream)
+    _check(lib().cas_swap_commit(pool.handle, st))
+
+
+def cas_train_step_host_scratch_bytes(pool: Pool, tab: SlotTable, Hq: int) -> int:
+    n = C.c_size_t(0)
+    _check(lib().cas_train_step_host_scratch_bytes(pool.handle, tab.handle, C.c_int32(Hq), C.byref(n)))
+    return n.value
+
+
+def cas_train_step_host(pool: Pool, tab: SlotTable, Hq: int, hQ, hKs, hVs, hdO, scale: float, cfg: AdamCfg,
+                        hO, hLSE, hdQ, scratch, stream=None):
+    _check(lib().cas_train_step_host(pool.handle, tab.handle, C.c_int32(Hq), _dptr(hQ), _dptr(hKs),
+                                     _dptr(hVs), _dptr(hdO), C.c_float(scale), C.byref(cfg), _dptr(hO),
+                                     _dptr(hLSE), _dptr(hdQ), _dptr(scratch),
+                                     C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)))

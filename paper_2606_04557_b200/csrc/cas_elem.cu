@@ -1,0 +1,126 @@
+// HBM-bound elementwise kernels: fused Adam (sec. 2.2), arrival refresh (derive the
+// working copy + zero the gradient slot after a swap-in), zero fill.
+//
+// Roofline: HBM.  Adam moves 30 B per element (read g,p,m,v = 16 B; write p,m,v = 12 B + bf16
+// working copy 2 B), 34 B with the fused gradient zeroing.  All accesses are 16-byte vectors,
+// fully coalesced, one (slot, chunk) per block; grid.y enumerates the slots.
+#include "cas_internal.h"
+
+namespace cas {
+
+__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ void st4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+
+__device__ __forceinline__ void store_work4(void* w, int64_t i, float4 p, bool bf16) {
+  if (bf16) {
+    __nv_bfloat162 a = __floats2bfloat162_rn(p.x, p.y);
+    __nv_bfloat162 b = __floats2bfloat162_rn(p.z, p.w);
+    uint2 u;
+    u.x = *reinterpret_cast<uint32_t*>(&a);
+    u.y = *reinterpret_cast<uint32_t*>(&b);
+    *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(w) + i) = u;
+  } else {
+    st4(reinterpret_cast<float*>(w) + i, p);
+  }
+}
+
+constexpr int kAdamThreads = 256;
+constexpr int kAdamUnroll = 4;   // float4 per thread per tensor
+
+template <bool BF16>
+__global__ void __launch_bounds__(kAdamThreads)
+adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2, float eps, int zero_grad) {
+  const AdamSlotDesc d = descs[blockIdx.y];
+  const float step = lr * d.step_size_scale;
+  const int64_t chunk = (int64_t)kAdamThreads * 4 * kAdamUnroll;
+  for (int which = 0; which < 2; ++which) {
+    float* __restrict__ p = d.state + (int64_t)which * d.cap_elems;
+    float* __restrict__ m = d.state + (int64_t)(2 + which) * d.cap_elems;
+    float* __restrict__ v = d.state + (int64_t)(4 + which) * d.cap_elems;
+    float* __restrict__ g = which ? d.gV : d.gK;
+    void* w = which ? d.wV : d.wK;
+    for (int64_t base = d.frozen_elems + (int64_t)blockIdx.x * chunk; base < d.n_elems;
+         base += (int64_t)gridDim.x * chunk) {
+      float4 G[kAdamUnroll], P[kAdamUnroll], M[kAdamUnroll], V[kAdamUnroll];
+#pragma unroll
+      for (int u = 0; u < kAdamUnroll; ++u) {
+        const int64_t i = base + ((int64_t)u * kAdamThreads + threadIdx.x) * 4;
+        if (i < d.n_elems) { G[u] = ld4(g + i); P[u] = ld4(p + i); M[u] = ld4(m + i); V[u] = ld4(v + i); }
+      }
+#pragma unroll
+      for (int u = 0; u < kAdamUnroll; ++u) {
+        const int64_t i = base + ((int64_t)u * kAdamThreads + threadIdx.x) * 4;
+        if (i >= d.n_elems) continue;
+        float* gp = reinterpret_cast<float*>(&G[u]);
+        float* pp = reinterpret_cast<float*>(&P[u]);
+        float* mp = reinterpret_cast<float*>(&M[u]);
+        float* vp = reinterpret_cast<float*>(&V[u]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float gg = gp[k];
+          const float mm = b1 * mp[k] + (1.0f - b1) * gg;
+          const float vv = b2 * vp[k] + (1.0f - b2) * gg * gg;
+          const float mhat = mm / d.bc1;
+          const float vhat = vv / d.bc2;
+          pp[k] = pp[k] - step * mhat / (sqrtf(vhat) + eps);
+          mp[k] = mm;
+          vp[k] = vv;
+        }
+        st4(p + i, P[u]);
+        st4(m + i, M[u]);
+        st4(v + i, V[u]);
+        store_work4(w, i, P[u], BF16);
+        if (zero_grad) st4(g + i, make_float4(0.f, 0.f, 0.f, 0.f));
+      }
+    }
+  }
+}
+
+int launch_adam(const AdamSlotDesc* d_desc, int n, int64_t max_elems, const cas_adam_cfg& cfg, int dtype,
+                cudaStream_t st) {
+  if (n <= 0 || max_elems <= 0) return CAS_OK;
+  const int64_t chunk = (int64_t)kAdamThreads * 4 * kAdamUnroll;
+  int64_t gx = (max_elems + chunk - 1) / chunk;
+  if (gx > 65535) gx = 65535;
+  dim3 grid((unsigned)gx, (unsigned)n);
+  if (dtype == CAS_BF16)
+    adam_kernel<true><<<grid, kAdamThreads, 0, st>>>(d_desc, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
+  else
+    adam_kernel<false><<<grid, kAdamThreads, 0, st>>>(d_desc, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "adam_kernel launch");
+  return CAS_OK;
+}
+
+template <bool BF16>
+__global__ void __launch_bounds__(256)
+refresh_kernel(const float* __restrict__ pK, const float* __restrict__ pV, void* wK, void* wV,
+               float* __restrict__ gK, float* __restrict__ gV, int64_t n) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x * 4;
+  for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n; i += stride) {
+    store_work4(wK, i, ld4(pK + i), BF16);
+    store_work4(wV, i, ld4(pV + i), BF16);
+    st4(gK + i, make_float4(0.f, 0.f, 0.f, 0.f));
+    st4(gV + i, make_float4(0.f, 0.f, 0.f, 0.f));
+  }
+}
+
+int launch_refresh(float* pK, float* pV, void* wK, void* wV, float* gK, float* gV, int64_t n, int dtype,
+                   cudaStream_t st) {
+  if (n <= 0) return CAS_OK;
+  int64_t gx = (n / 4 + 255) / 256;
+  if (gx > 148 * 8) gx = 148 * 8;
+  if (dtype == CAS_BF16) refresh_kernel<true><<<(unsigned)gx, 256, 0, st>>>(pK, pV, wK, wV, gK, gV, n);
+  else refresh_kernel<false><<<(unsigned)gx, 256, 0, st>>>(pK, pV, wK, wV, gK, gV, n);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, "refresh_kernel launch");
+  return CAS_OK;
+}
+
+int launch_zero(float* p, int64_t n, cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(p, 0, (size_t)n * 4, st);
+  if (e != cudaSuccess) return cuda_fail(e, "zero");
+  return CAS_OK;
+}
+
+}  // namespace cas

@@ -1,0 +1,847 @@
+// Host runtime of libcas: pool carving, integer bookkeeping (slot tables, inverted tables, rotation
+// planner, manifests, counters), swap engine, dispatch to the kernels.  C ABI: include/cas.h.
+//
+// The integer rules implemented here are DESIGN.md "Bookkeeping" K1-K4 (sec. 2.1);
+// an independent pure-Python restatement lives in oracle/bookkeeping.py and is compared bit-exactly.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <numeric>
+#include <set>
+
+#include "cas_internal.h"
+
+namespace cas {
+
+static thread_local char g_err[512] = "";
+static int g_impl = CAS_IMPL_AUTO;
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+}
+
+int cuda_fail(cudaError_t e, const char* what) {
+  set_error("CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), what);
+  return CAS_ERR_CUDA;
+}
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+// DESIGN.md R15: SplitMix64 finaliser over seed + gamma*(step+1) + 0xD1B54A32D192ED03*(cart+1).
+static inline uint64_t mix64(uint64_t seed, uint64_t step, uint64_t cart) {
+  uint64_t z = seed + 0x9E3779B97F4A7C15ull * (step + 1) + 0xD1B54A32D192ED03ull * (cart + 1);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+struct Carve {
+  int64_t off_K, off_V, off_gK, off_gV, off_state, total;
+};
+
+static Carve carve(int64_t pool_tokens, int64_t row_elems, int eb) {
+  Carve c;
+  int64_t o = 0;
+  const int64_t A = 1024;
+  c.off_K = o;      o = round_up(o + pool_tokens * row_elems * eb, A);
+  c.off_V = o;      o = round_up(o + pool_tokens * row_elems * eb, A);
+  c.off_gK = o;     o = round_up(o + pool_tokens * row_elems * 4, A);
+  c.off_gV = o;     o = round_up(o + pool_tokens * row_elems * 4, A);
+  c.off_state = o;  o = round_up(o + 6 * pool_tokens * row_elems * 4, A);
+  c.total = o;
+  return c;
+}
+
+static int check_desc(const cas_pool_desc* d) {
+  if (!d || !d->cart_len) { set_error("null pool desc"); return CAS_ERR_INVALID_ARG; }
+  if (d->dtype != CAS_F32 && d->dtype != CAS_BF16) { set_error("bad dtype"); return CAS_ERR_INVALID_ARG; }
+  if (d->Hkv < 1 || d->D < 32 || d->D > 128 || d->D % 32) { set_error("Hkv>=1, D in {32,64,96,128}"); return CAS_ERR_SHAPE; }
+  if (d->n_carts < 1 || d->n_slots < 1 || d->n_slots > d->n_carts) { set_error("need 1 <= n_slots <= n_carts"); return CAS_ERR_INVALID_ARG; }
+  if (d->tile_tokens < 0 || (d->tile_tokens && d->tile_tokens % 16)) { set_error("tile_tokens must be a multiple of 16"); return CAS_ERR_INVALID_ARG; }
+  for (int i = 0; i < d->n_carts; ++i)
+    if (d->cart_len[i] < 1) { set_error("cart_len[%d] < 1", i); return CAS_ERR_INVALID_ARG; }
+  return CAS_OK;
+}
+
+static void layout_slots(const cas_pool_desc* d, std::vector<int32_t>& base, std::vector<int32_t>& cap,
+                         int64_t& pool_tokens) {
+  const int tile = d->tile_tokens ? d->tile_tokens : 128;
+  base.assign(d->n_slots, 0);
+  cap.assign(d->n_slots, 0);
+  if (d->n_slots == d->n_carts) {
+    for (int s = 0; s < d->n_slots; ++s) cap[s] = (int32_t)round_up(d->cart_len[s], tile);
+  } else {
+    int32_t mx = 0;
+    for (int i = 0; i < d->n_carts; ++i) mx = std::max(mx, d->cart_len[i]);
+    for (int s = 0; s < d->n_slots; ++s) cap[s] = (int32_t)round_up(mx, tile);
+  }
+  int64_t o = 0;
+  for (int s = 0; s < d->n_slots; ++s) { base[s] = (int32_t)o; o += cap[s]; }
+  pool_tokens = o;
+}
+
+template <typename T>
+static size_t blob_add(size_t& off, const std::vector<T>& v, size_t extra = 0) {
+  size_t o = off;
+  off = (size_t)round_up((int64_t)(off + (v.size() + extra) * sizeof(T)), 256);
+  return o;
+}
+
+}  // namespace cas
+
+using namespace cas;
+
+extern "C" {
+
+const char* cas_version(void) { return "libcas 0.1 (sm_100a)"; }
+
+void cas_last_error(char* buf, size_t n) {
+  if (!buf || !n) return;
+  strncpy(buf, g_err, n - 1);
+  buf[n - 1] = 0;
+}
+
+int cas_set_impl(int impl) {
+  if (impl < CAS_IMPL_AUTO || impl > CAS_IMPL_TC) { set_error("bad impl"); return CAS_ERR_INVALID_ARG; }
+  g_impl = impl;
+  return CAS_OK;
+}
+
+int cas_pool_query_bytes(const cas_pool_desc* desc, size_t* dev_bytes, size_t* host_bytes) {
+  int rc = check_desc(desc);
+  if (rc) return rc;
+  std::vector<int32_t> base, cap;
+  int64_t pool_tokens;
+  layout_slots(desc, base, cap, pool_tokens);
+  if (pool_tokens >= (1ll << 31)) { set_error("pool too large for int32 token indices"); return CAS_ERR_CAPACITY; }
+  const int64_t row = (int64_t)desc->Hkv * desc->D;
+  Carve c = carve(pool_tokens, row, desc->dtype == CAS_BF16 ? 2 : 4);
+  if (dev_bytes) *dev_bytes = (size_t)c.total;
+  if (host_bytes) {
+    int64_t h = 0;
+    for (int i = 0; i < desc->n_carts; ++i) h += 6 * (int64_t)desc->cart_len[i] * row * 4;
+    *host_bytes = (size_t)h;
+  }
+  return CAS_OK;
+}
+
+int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_arena, void* side_stream,
+                    cas_pool** out) {
+  if (!out) { set_error("null out"); return CAS_ERR_INVALID_ARG; }
+  int rc = check_desc(desc);
+  if (rc) return rc;
+  if (dev_arena && !pinned_arena && desc->n_slots != desc->n_carts) {
+    set_error("pinned arena required when n_slots < n_carts");
+    return CAS_ERR_INVALID_ARG;
+  }
+  cas_pool* p = new cas_pool();
+  p->desc = *desc;
+  p->cart_len.assign(desc->cart_len, desc->cart_len + desc->n_carts);
+  p->desc.cart_len = p->cart_len.data();
+  p->tile = desc->tile_tokens ? desc->tile_tokens : 128;
+  p->row_elems = (int64_t)desc->Hkv * desc->D;
+  p->elem_bytes = desc->dtype == CAS_BF16 ? 2 : 4;
+  layout_slots(desc, p->slot_base, p->slot_cap, p->pool_tokens);
+  if (p->pool_tokens >= (1ll << 31)) { delete p; set_error("pool too large"); return CAS_ERR_CAPACITY; }
+  p->home_off.assign(desc->n_carts, 0);
+  for (int c = 1; c < desc->n_carts; ++c) p->home_off[c] = p->home_off[c - 1] + p->home_bytes(c - 1);
+  p->slot_of.assign(desc->n_carts, -1);
+  p->cart_in.assign(desc->n_slots, -1);
+  for (int s = 0; s < desc->n_slots; ++s) { p->slot_of[s] = s; p->cart_in[s] = s; }
+  p->in_transit.assign(desc->n_carts, 0);
+  p->grad_dirty.assign(desc->n_slots, 0);
+  p->opt_steps.assign(desc->n_carts, 0);
+  p->last_used.assign(desc->n_carts, -1);
+  p->dev = (char*)dev_arena;
+  p->pinned = (char*)pinned_arena;
+  p->side = (cudaStream_t)side_stream;
+  if (p->dev) {
+    Carve c = carve(p->pool_tokens, p->row_elems, p->elem_bytes);
+    p->pool_K = p->dev + c.off_K;
+    p->pool_V = p->dev + c.off_V;
+    p->grad_K = (float*)(p->dev + c.off_gK);
+    p->grad_V = (float*)(p->dev + c.off_gV);
+    p->state = (float*)(p->dev + c.off_state);
+    cudaError_t e = cudaMemsetAsync(p->dev, 0, (size_t)c.total, p->side);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->side);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_main, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_adam_desc, cudaEventDisableTiming);
+    if (e != cudaSuccess) { delete p; return cuda_fail(e, "pool_create"); }
+    if (desc->dtype == CAS_BF16 && desc->D == 128) {
+      rc = tc_make_pool_maps(p);
+      if (rc) { delete p; return rc; }
+    }
+  }
+  *out = p;
+  return CAS_OK;
+}
+
+int cas_pool_destroy(cas_pool* p) {
+  if (!p) return CAS_OK;
+  if (p->dev) {
+    cudaDeviceSynchronize();
+    if (p->ev_side) cudaEventDestroy(p->ev_side);
+    if (p->ev_main) cudaEventDestroy(p->ev_main);
+    if (p->ev_adam_desc) cudaEventDestroy(p->ev_adam_desc);
+    if (p->d_adam_desc) cudaFree(p->d_adam_desc);
+    if (p->h_adam_desc) cudaFreeHost(p->h_adam_desc);
+  }
+  delete p;
+  return CAS_OK;
+}
+
+int cas_pool_layout_get(const cas_pool* p, cas_pool_layout* out) {
+  if (!p || !out) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  out->pool_K = p->pool_K;
+  out->pool_V = p->pool_V;
+  out->grad_K = p->grad_K;
+  out->grad_V = p->grad_V;
+  out->state = p->state;
+  out->slot_base = p->slot_base.data();
+  out->slot_cap = p->slot_cap.data();
+  out->pool_tokens = p->pool_tokens;
+  return CAS_OK;
+}
+
+static int need_data(const cas_pool* p) {
+  if (!p) { set_error("null pool"); return CAS_ERR_INVALID_ARG; }
+  if (!p->dev) { set_error("bookkeeping-only pool has no data"); return CAS_ERR_INVALID_ARG; }
+  return CAS_OK;
+}
+
+int cas_pool_load(cas_pool* p, int32_t cart, const float* K, const float* V) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (cart < 0 || cart >= p->desc.n_carts || !K || !V) { set_error("bad cart / null data"); return CAS_ERR_INVALID_ARG; }
+  if (p->in_transit[cart]) { set_error("cartridge %d in transit", cart); return CAS_ERR_BUSY; }
+  const int64_t n = (int64_t)p->cart_len[cart] * p->row_elems;
+  const int s = p->slot_of[cart];
+  if (s >= 0) {
+    CAS_CUDA(cudaStreamSynchronize(p->side));
+    CAS_CUDA(cudaMemcpy(p->slot_state(s, 0), K, n * 4, cudaMemcpyHostToDevice));
+    CAS_CUDA(cudaMemcpy(p->slot_state(s, 1), V, n * 4, cudaMemcpyHostToDevice));
+    for (int w = 2; w < 6; ++w) CAS_CUDA(cudaMemsetAsync(p->slot_state(s, w), 0, n * 4, p->side));
+    const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
+    rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
+                        (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, n,
+                        p->desc.dtype, p->side);
+    if (rc) return rc;
+    CAS_CUDA(cudaStreamSynchronize(p->side));
+    p->grad_dirty[s] = 0;
+  } else {
+    if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+    CAS_CUDA(cudaStreamSynchronize(p->side));
+    memcpy(p->home(cart, 0), K, n * 4);
+    memcpy(p->home(cart, 1), V, n * 4);
+    memset(p->home(cart, 2), 0, 4 * n * 4);
+  }
+  return CAS_OK;
+}
+
+int cas_pool_read(cas_pool* p, int32_t cart, int32_t what, void* out) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (cart < 0 || cart >= p->desc.n_carts || what < 0 || what > 9 || !out) { set_error("bad args"); return CAS_ERR_INVALID_ARG; }
+  const int64_t n = (int64_t)p->cart_len[cart] * p->row_elems;
+  const int s = p->slot_of[cart];
+  CAS_CUDA(cudaDeviceSynchronize());
+  if (what < 6) {
+    if (s >= 0 && p->in_transit[cart] != 2) {
+      CAS_CUDA(cudaMemcpy(out, p->slot_state(s, what), n * 4, cudaMemcpyDeviceToHost));
+    } else {
+      if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+      memcpy(out, p->home(cart, what), n * 4);
+    }
+    return CAS_OK;
+  }
+  if (s < 0) { set_error("cartridge %d not resident", cart); return CAS_ERR_NOT_RESIDENT; }
+  const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
+  if (what == 6) CAS_CUDA(cudaMemcpy(out, p->grad_K + o, n * 4, cudaMemcpyDeviceToHost));
+  if (what == 7) CAS_CUDA(cudaMemcpy(out, p->grad_V + o, n * 4, cudaMemcpyDeviceToHost));
+  if (what == 8) CAS_CUDA(cudaMemcpy(out, (char*)p->pool_K + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
+  if (what == 9) CAS_CUDA(cudaMemcpy(out, (char*)p->pool_V + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
+  return CAS_OK;
+}
+
+int cas_pool_counters(const cas_pool* p, int32_t* slot_of, int32_t* cart_in, int64_t* opt_steps,
+                      int64_t* last_used, int32_t* in_transit, int32_t* grad_dirty) {
+  if (!p) { set_error("null pool"); return CAS_ERR_INVALID_ARG; }
+  const int N = p->desc.n_carts, S = p->desc.n_slots;
+  if (slot_of) memcpy(slot_of, p->slot_of.data(), N * 4);
+  if (cart_in) memcpy(cart_in, p->cart_in.data(), S * 4);
+  if (opt_steps) memcpy(opt_steps, p->opt_steps.data(), N * 8);
+  if (last_used) memcpy(last_used, p->last_used.data(), N * 8);
+  if (in_transit) memcpy(in_transit, p->in_transit.data(), N * 4);
+  if (grad_dirty) memcpy(grad_dirty, p->grad_dirty.data(), S * 4);
+  return CAS_OK;
+}
+
+int cas_pool_set_counters(cas_pool* p, int32_t cart, int64_t opt_steps, int64_t last_used) {
+  if (!p || cart < 0 || cart >= p->desc.n_carts || opt_steps < 0) { set_error("bad args"); return CAS_ERR_INVALID_ARG; }
+  p->opt_steps[cart] = opt_steps;
+  p->last_used[cart] = last_used;
+  return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// slot table (K1)
+// ---------------------------------------------------------------------------------------------
+int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const int32_t* sel_off,
+                         const int32_t* sel_cart, int64_t step, cas_slot_table** out) {
+  if (!p || !out || !seq_off || !sel_off || B < 1) { set_error("null / empty args"); return CAS_ERR_INVALID_ARG; }
+  if (seq_off[0] != 0 || sel_off[0] != 0) { set_error("offsets must start at 0"); return CAS_ERR_INVALID_ARG; }
+  for (int b = 0; b < B; ++b) {
+    if (seq_off[b + 1] <= seq_off[b]) { set_error("sequence %d has no query tokens", b); return CAS_ERR_SHAPE; }
+    if (sel_off[b + 1] < sel_off[b]) { set_error("sel_off not monotone"); return CAS_ERR_INVALID_ARG; }
+  }
+  const int nsel = sel_off[B];
+  if (nsel > 0 && !sel_cart) { set_error("null sel_cart"); return CAS_ERR_INVALID_ARG; }
+  const int N = p->desc.n_carts, S = p->desc.n_slots;
+  cas_slot_table* t = new cas_slot_table();
+  t->pool = p;
+  t->B = B;
+  t->T = seq_off[B];
+  t->nsel = nsel;
+  t->seq_off.assign(seq_off, seq_off + B + 1);
+  t->sel_off.assign(sel_off, sel_off + B + 1);
+  t->sel_cart.assign(sel_cart, sel_cart + nsel);
+  t->sel_slot.resize(nsel);
+  t->sel_base.resize(nsel);
+  t->sel_len.resize(nsel);
+  t->P.assign(B, 0);
+  std::vector<int32_t> mark(N, -1);
+  for (int b = 0; b < B; ++b) {
+    for (int k = sel_off[b]; k < sel_off[b + 1]; ++k) {
+      const int c = sel_cart[k];
+      int rc = CAS_OK;
+      if (c < 0 || c >= N) { set_error("cartridge id %d out of range", c); rc = CAS_ERR_INVALID_ARG; }
+      else if (mark[c] == b) { set_error("duplicate cartridge %d in sequence %d", c, b); rc = CAS_ERR_INVALID_ARG; }
+      else if (p->slot_of[c] < 0) { set_error("cartridge %d not resident", c); rc = CAS_ERR_NOT_RESIDENT; }
+      else if (p->in_transit[c]) { set_error("cartridge %d in transit", c); rc = CAS_ERR_BUSY; }
+      if (rc) { delete t; return rc; }
+      mark[c] = b;
+      t->sel_slot[k] = p->slot_of[c];
+      t->sel_base[k] = p->slot_base[p->slot_of[c]];
+      t->sel_len[k] = p->cart_len[c];
+      t->P[b] += p->cart_len[c];
+    }
+  }
+  for (int k = 0; k < nsel; ++k) p->last_used[sel_cart[k]] = step;
+  // inverted CSR sorted by (slot, sequence): counting sort keeps sequences ascending per slot
+  t->inv_off.assign(S + 1, 0);
+  for (int k = 0; k < nsel; ++k) t->inv_off[t->sel_slot[k] + 1]++;
+  for (int s = 0; s < S; ++s) t->inv_off[s + 1] += t->inv_off[s];
+  t->inv_seq.resize(nsel);
+  {
+    std::vector<int32_t> cur(t->inv_off.begin(), t->inv_off.end() - 1);
+    for (int b = 0; b < B; ++b)
+      for (int k = sel_off[b]; k < sel_off[b + 1]; ++k) t->inv_seq[cur[t->sel_slot[k]]++] = b;
+  }
+  for (int s = 0; s < S; ++s)
+    if (t->inv_off[s + 1] > t->inv_off[s]) {
+      t->used_slots.push_back(s);
+      t->unique_prefix_tokens += p->cart_len[p->cart_in[s]];
+    }
+  // KV tile lists + work lists
+  const int tile = 128;
+  t->kv_tile_off.assign(B + 1, 0);
+  for (int b = 0; b < B; ++b) {
+    for (int k = sel_off[b]; k < sel_off[b + 1]; ++k)
+      for (int j = 0; j < t->sel_len[k]; j += tile)
+        t->kv_tiles.push_back({t->sel_base[k] + j, std::min(tile, t->sel_len[k] - j)});
+    t->kv_tile_off[b + 1] = (int32_t)t->kv_tiles.size();
+    const int64_t lq = seq_off[b + 1] - seq_off[b];
+    t->max_lq = std::max<int32_t>(t->max_lq, (int32_t)lq);
+    t->pairs += lq * t->P[b] + lq * (lq + 1) / 2;
+    t->prefix_tokens += t->P[b];
+    const int npre = t->kv_tile_off[b + 1] - t->kv_tile_off[b];
+    for (int r = 0; r < lq; r += 256) {
+      const int rows = (int)std::min<int64_t>(256, lq - r);
+      const int nq = (rows + 127) / 128;
+      t->fwd_items.push_back({b, r, rows, nq * npre + (r / 128) * nq + (nq == 2 ? 3 : 1)});
+    }
+    for (int r = 0; r < lq; r += 32) t->simt_items.push_back({b, r, (int)std::min<int64_t>(32, lq - r), 0});
+  }
+  std::stable_sort(t->fwd_items.begin(), t->fwd_items.end(),
+                   [](const FwdItem& a, const FwdItem& b) { return a.cost > b.cost; });
+  for (int s : t->used_slots) {
+    int cost = 0;
+    for (int e = t->inv_off[s]; e < t->inv_off[s + 1]; ++e) {
+      const int b = t->inv_seq[e];
+      cost += (seq_off[b + 1] - seq_off[b] + 127) / 128;
+    }
+    const int len = p->cart_len[p->cart_in[s]];
+    for (int j = 0; j < len; j += tile)
+      t->bwd_items.push_back({0, s, p->slot_base[s] + j, std::min(tile, len - j), j / tile, cost});
+  }
+  for (int b = 0; b < B; ++b) {
+    const int lq = seq_off[b + 1] - seq_off[b];
+    const int nt = (lq + tile - 1) / tile;
+    for (int j = 0; j < nt; ++j)
+      t->bwd_items.push_back({1, b, seq_off[b] + j * tile, std::min(tile, lq - j * tile), j, nt - j});
+  }
+  std::stable_sort(t->bwd_items.begin(), t->bwd_items.end(),
+                   [](const BwdItem& a, const BwdItem& b) { return a.cost > b.cost; });
+  if (p->dev) {
+    size_t off = 0;
+    const size_t o_seq = blob_add(off, t->seq_off), o_sel = blob_add(off, t->sel_off),
+                 o_base = blob_add(off, t->sel_base, 1), o_len = blob_add(off, t->sel_len, 1),
+                 o_slot = blob_add(off, t->sel_slot, 1), o_ioff = blob_add(off, t->inv_off),
+                 o_iseq = blob_add(off, t->inv_seq, 1), o_kto = blob_add(off, t->kv_tile_off),
+                 o_kt = blob_add(off, t->kv_tiles, 1), o_fw = blob_add(off, t->fwd_items),
+                 o_si = blob_add(off, t->simt_items), o_bw = blob_add(off, t->bwd_items),
+                 o_us = blob_add(off, t->used_slots, 1);
+    const size_t o_cnt = off;
+    off += 256;
+    std::vector<char> h(off, 0);
+    auto put = [&](size_t o, const void* src, size_t n) { if (n) memcpy(h.data() + o, src, n); };
+    put(o_seq, t->seq_off.data(), t->seq_off.size() * 4);
+    put(o_sel, t->sel_off.data(), t->sel_off.size() * 4);
+    put(o_base, t->sel_base.data(), t->sel_base.size() * 4);
+    put(o_len, t->sel_len.data(), t->sel_len.size() * 4);
+    put(o_slot, t->sel_slot.data(), t->sel_slot.size() * 4);
+    put(o_ioff, t->inv_off.data(), t->inv_off.size() * 4);
+    put(o_iseq, t->inv_seq.data(), t->inv_seq.size() * 4);
+    put(o_kto, t->kv_tile_off.data(), t->kv_tile_off.size() * 4);
+    put(o_kt, t->kv_tiles.data(), t->kv_tiles.size() * sizeof(KvTile));
+    put(o_fw, t->fwd_items.data(), t->fwd_items.size() * sizeof(FwdItem));
+    put(o_si, t->simt_items.data(), t->simt_items.size() * sizeof(FwdItem));
+    put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
+    put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
+    cudaError_t e = cudaMalloc((void**)&t->d_blob, off);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_blob, h.data(), off, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { if (t->d_blob) cudaFree(t->d_blob); delete t; return cuda_fail(e, "slot table upload"); }
+    char* d = t->d_blob;
+    t->d_seq_off = (int32_t*)(d + o_seq);
+    t->d_sel_off = (int32_t*)(d + o_sel);
+    t->d_sel_base = (int32_t*)(d + o_base);
+    t->d_sel_len = (int32_t*)(d + o_len);
+    t->d_sel_slot = (int32_t*)(d + o_slot);
+    t->d_inv_off = (int32_t*)(d + o_ioff);
+    t->d_inv_seq = (int32_t*)(d + o_iseq);
+    t->d_kv_tile_off = (int32_t*)(d + o_kto);
+    t->d_kv_tiles = (KvTile*)(d + o_kt);
+    t->d_fwd_items = (FwdItem*)(d + o_fw);
+    t->d_simt_items = (FwdItem*)(d + o_si);
+    t->d_bwd_items = (BwdItem*)(d + o_bw);
+    t->d_used_slots = (int32_t*)(d + o_us);
+    t->d_counters = (int32_t*)(d + o_cnt);
+  }
+  *out = t;
+  return CAS_OK;
+}
+
+int cas_slot_table_destroy(cas_slot_table* t) {
+  if (!t) return CAS_OK;
+  if (t->d_blob) { cudaDeviceSynchronize(); cudaFree(t->d_blob); }
+  delete t;
+  return CAS_OK;
+}
+
+int cas_slot_table_info(const cas_slot_table* t, cas_table_info* o) {
+  if (!t || !o) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  o->B = t->B; o->T = t->T; o->nsel = t->nsel; o->n_kv_tiles = (int32_t)t->kv_tiles.size();
+  o->pairs_per_head = t->pairs; o->prefix_tokens = t->prefix_tokens;
+  o->unique_prefix_tokens = t->unique_prefix_tokens;
+  return CAS_OK;
+}
+
+int cas_slot_table_export(const cas_slot_table* t, int32_t* sel_slot, int32_t* inv_off, int32_t* inv_seq,
+                          int64_t* P) {
+  if (!t) { set_error("null table"); return CAS_ERR_INVALID_ARG; }
+  if (sel_slot && t->nsel) memcpy(sel_slot, t->sel_slot.data(), t->nsel * 4);
+  if (inv_off) memcpy(inv_off, t->inv_off.data(), t->inv_off.size() * 4);
+  if (inv_seq && t->nsel) memcpy(inv_seq, t->inv_seq.data(), t->nsel * 4);
+  if (P) memcpy(P, t->P.data(), t->B * 8);
+  return CAS_OK;
+}
+
+int cas_position_offsets(const cas_pool* p, const cas_slot_table* t, int64_t* total_resident, int64_t* P) {
+  if (!p) { set_error("null pool"); return CAS_ERR_INVALID_ARG; }
+  if (total_resident) {
+    int64_t tot = 0;
+    for (int c = 0; c < p->desc.n_carts; ++c) if (p->slot_of[c] >= 0) tot += p->cart_len[c];
+    *total_resident = tot;
+  }
+  if (P) {
+    if (!t) { set_error("null table"); return CAS_ERR_INVALID_ARG; }
+    memcpy(P, t->P.data(), t->B * 8);
+  }
+  return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// attention dispatch
+// ---------------------------------------------------------------------------------------------
+static int check_attn(const cas_pool* p, const cas_slot_table* t, int Hq, const void* Ks, const void* Vs) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (!t || t->pool != p) { set_error("table does not belong to this pool"); return CAS_ERR_INVALID_ARG; }
+  if (Hq < 1 || Hq % p->desc.Hkv) { set_error("Hq must be a positive multiple of Hkv"); return CAS_ERR_SHAPE; }
+  if ((Ks == nullptr) != (Vs == nullptr)) { set_error("K_self and V_self must both be given or both NULL"); return CAS_ERR_INVALID_ARG; }
+  if (!Ks)
+    for (int b = 0; b < t->B; ++b)
+      if (t->sel_off[b + 1] == t->sel_off[b]) { set_error("sequence %d sees no key at all", b); return CAS_ERR_SHAPE; }
+  for (int k = 0; k < t->nsel; ++k) {   // the table is a snapshot: its slots must still hold those cartridges
+    const int c = t->sel_cart[k];
+    if (p->slot_of[c] != t->sel_slot[k] || p->in_transit[c]) { set_error("stale slot table (cartridge %d moved)", c); return CAS_ERR_NOT_RESIDENT; }
+  }
+  return CAS_OK;
+}
+
+static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) {
+  *rc = CAS_OK;
+  if (g_impl == CAS_IMPL_SIMT) return false;
+  const bool ok = tc_supported(p, t, Hq);
+  if (g_impl == CAS_IMPL_TC && !ok) { set_error("tensor-core path needs bf16, D=128"); *rc = CAS_ERR_SHAPE; }
+  return ok;
+}
+
+int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
+                        const void* Vs, float scale, void* O, float* LSE, void* stream) {
+  int rc = check_attn(p, t, Hq, Ks, Vs);
+  if (rc) return rc;
+  if (!Q || !O || !LSE) { set_error("null Q/O/LSE"); return CAS_ERR_INVALID_ARG; }
+  AttnArgs a{};
+  a.pool = p; a.tab = t; a.Hq = Hq; a.Hkv = p->desc.Hkv; a.D = p->desc.D; a.dtype = p->desc.dtype;
+  a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O_out = O; a.LSE_out = LSE; a.scale = scale;
+  a.stream = (cudaStream_t)stream;
+  const bool tc = use_tc(p, t, Hq, &rc);
+  if (rc) return rc;
+  return tc ? tc_attn_fwd(a) : simt_attn_fwd(a);
+}
+
+int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* p, const cas_slot_table* t, int32_t Hq, size_t* bytes) {
+  if (!p || !t || !bytes || Hq < 1) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  *bytes = std::max(simt_bwd_workspace(t, Hq), tc_bwd_workspace(t, Hq, p->desc.D));
+  return CAS_OK;
+}
+
+int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
+                        const void* Vs, const void* O, const float* LSE, const void* dO, float scale,
+                        void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes, void* stream) {
+  int rc = check_attn(p, t, Hq, Ks, Vs);
+  if (rc) return rc;
+  if (!Q || !O || !LSE || !dO || !dQ) { set_error("null Q/O/LSE/dO/dQ"); return CAS_ERR_INVALID_ARG; }
+  if ((dKs == nullptr) != (dVs == nullptr) || (dKs && !Ks)) { set_error("dK_self/dV_self: both or none, and only with K_self"); return CAS_ERR_INVALID_ARG; }
+  size_t need = 0;
+  cas_prefix_attn_bwd_workspace_bytes(p, t, Hq, &need);
+  if (!workspace || workspace_bytes < need) { set_error("workspace too small: need %zu bytes", need); return CAS_ERR_CAPACITY; }
+  AttnArgs a{};
+  a.pool = p; a.tab = t; a.Hq = Hq; a.Hkv = p->desc.Hkv; a.D = p->desc.D; a.dtype = p->desc.dtype;
+  a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O = O; a.LSE_in = LSE; a.dO = dO; a.dQ = dQ; a.dKs = dKs; a.dVs = dVs;
+  a.scale = scale; a.workspace = workspace; a.workspace_bytes = workspace_bytes;
+  a.stream = (cudaStream_t)stream;
+  const bool tc = use_tc(p, t, Hq, &rc);
+  if (rc) return rc;
+  rc = tc ? tc_attn_bwd(a) : simt_attn_bwd(a);
+  if (rc) return rc;
+  for (int s : t->used_slots) p->grad_dirty[s] = 1;
+  return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Adam
+// ---------------------------------------------------------------------------------------------
+int cas_adam_step(cas_pool* p, const cas_adam_cfg* cfg, const int32_t* slots, int32_t n,
+                  const float* lr_scale, void* stream) {
+  if (!p || !cfg) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  if (cfg->n_frozen < 0 || !(cfg->beta1 >= 0 && cfg->beta1 < 1) || !(cfg->beta2 >= 0 && cfg->beta2 < 1)) {
+    set_error("bad Adam config");
+    return CAS_ERR_INVALID_ARG;
+  }
+  std::vector<int32_t> list;
+  if (slots) {
+    if (n < 0) { set_error("n < 0"); return CAS_ERR_INVALID_ARG; }
+    list.assign(slots, slots + n);
+  } else {
+    for (int s = 0; s < p->desc.n_slots; ++s)
+      if (p->cart_in[s] >= 0 && !p->in_transit[p->cart_in[s]]) list.push_back(s);
+  }
+  std::set<int32_t> seen;
+  for (int s : list) {
+    if (s < 0 || s >= p->desc.n_slots || !seen.insert(s).second) { set_error("bad / duplicate slot %d", s); return CAS_ERR_INVALID_ARG; }
+    if (p->cart_in[s] < 0) { set_error("slot %d is empty", s); return CAS_ERR_NOT_RESIDENT; }
+    if (p->in_transit[p->cart_in[s]]) { set_error("slot %d in transit", s); return CAS_ERR_BUSY; }
+  }
+  const int cnt = (int)list.size();
+  if (p->dev && cnt) {
+    if (cnt > p->adam_desc_cap) {
+      CAS_CUDA(cudaDeviceSynchronize());
+      if (p->d_adam_desc) cudaFree(p->d_adam_desc);
+      if (p->h_adam_desc) cudaFreeHost(p->h_adam_desc);
+      p->adam_desc_cap = std::max(cnt, p->desc.n_slots);
+      CAS_CUDA(cudaMalloc(&p->d_adam_desc, p->adam_desc_cap * sizeof(AdamSlotDesc)));
+      CAS_CUDA(cudaHostAlloc(&p->h_adam_desc, p->adam_desc_cap * sizeof(AdamSlotDesc), cudaHostAllocDefault));
+    }
+    CAS_CUDA(cudaEventSynchronize(p->ev_adam_desc));   // previous upload has left the staging buffer
+    AdamSlotDesc* h = (AdamSlotDesc*)p->h_adam_desc;
+    int64_t max_elems = 0;
+    for (int i = 0; i < cnt; ++i) {
+      const int s = list[i], c = p->cart_in[s];
+      const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
+      const double t = (double)(p->opt_steps[c] + 1);
+      h[i].state = p->slot_state(s, 0);
+      h[i].wK = (char*)p->pool_K + o * p->elem_bytes;
+      h[i].wV = (char*)p->pool_V + o * p->elem_bytes;
+      h[i].gK = p->grad_K + o;
+      h[i].gV = p->grad_V + o;
+      h[i].cap_elems = (int64_t)p->slot_cap[s] * p->row_elems;
+      h[i].n_elems = (int64_t)p->cart_len[c] * p->row_elems;
+      h[i].frozen_elems = std::min<int64_t>(cfg->n_frozen, p->cart_len[c]) * p->row_elems;
+      h[i].step_size_scale = lr_scale ? lr_scale[i] : 1.0f;
+      h[i].bc1 = (float)(1.0 - pow((double)cfg->beta1, t));
+      h[i].bc2 = (float)(1.0 - pow((double)cfg->beta2, t));
+      h[i].pad = 0;
+      max_elems = std::max(max_elems, h[i].n_elems);
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CAS_CUDA(cudaMemcpyAsync(p->d_adam_desc, h, cnt * sizeof(AdamSlotDesc), cudaMemcpyHostToDevice, st));
+    CAS_CUDA(cudaEventRecord(p->ev_adam_desc, st));
+    int rc = launch_adam((const AdamSlotDesc*)p->d_adam_desc, cnt, max_elems, *cfg, p->desc.dtype, st);
+    if (rc) return rc;
+  }
+  for (int s : list) {
+    p->opt_steps[p->cart_in[s]] += 1;
+    if (cfg->zero_grad) p->grad_dirty[s] = 0;
+  }
+  return CAS_OK;
+}
+
+int cas_grad_zero(cas_pool* p, const int32_t* slots, int32_t n, void* stream) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  std::vector<int32_t> list;
+  if (slots) list.assign(slots, slots + std::max(n, 0));
+  else for (int s = 0; s < p->desc.n_slots; ++s) list.push_back(s);
+  for (int s : list) {
+    if (s < 0 || s >= p->desc.n_slots) { set_error("bad slot"); return CAS_ERR_INVALID_ARG; }
+    const int64_t o = (int64_t)p->slot_base[s] * p->row_elems, nb = (int64_t)p->slot_cap[s] * p->row_elems * 4;
+    CAS_CUDA(cudaMemsetAsync(p->grad_K + o, 0, nb, (cudaStream_t)stream));
+    CAS_CUDA(cudaMemsetAsync(p->grad_V + o, 0, nb, (cudaStream_t)stream));
+    p->grad_dirty[s] = 0;
+  }
+  return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// rotation (K3) and swap engine (K2, K4)
+// ---------------------------------------------------------------------------------------------
+int cas_plan_rotation(const cas_pool* p, int64_t step, int32_t n_in, int32_t n_out, const int32_t* protect,
+                      int32_t n_protect, uint64_t seed, cas_manifest_entry* entries, int32_t capacity,
+                      int32_t* n_entries) {
+  if (!p || !entries || !n_entries || n_protect < 0 || (n_protect && !protect)) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  const int N = p->desc.n_carts, S = p->desc.n_slots;
+  std::vector<char> prot(N, 0);
+  for (int i = 0; i < n_protect; ++i) {
+    if (protect[i] < 0 || protect[i] >= N) { set_error("bad protected id"); return CAS_ERR_INVALID_ARG; }
+    prot[protect[i]] = 1;
+  }
+  std::vector<int32_t> evictable, waiting;
+  for (int c = 0; c < N; ++c) {
+    if (p->in_transit[c]) continue;
+    if (p->slot_of[c] >= 0) { if (!prot[c]) evictable.push_back(c); }
+    else waiting.push_back(c);
+  }
+  std::sort(evictable.begin(), evictable.end(), [&](int a, int b) {
+    return p->last_used[a] != p->last_used[b] ? p->last_used[a] < p->last_used[b] : a < b;
+  });
+  if ((int)evictable.size() > std::max(n_out, 0)) evictable.resize(std::max(n_out, 0));
+  std::vector<uint64_t> hsh(N, 0);
+  for (int c : waiting) hsh[c] = mix64(seed, (uint64_t)step, (uint64_t)c);
+  std::sort(waiting.begin(), waiting.end(), [&](int a, int b) {
+    if (p->opt_steps[a] != p->opt_steps[b]) return p->opt_steps[a] < p->opt_steps[b];
+    if (hsh[a] != hsh[b]) return hsh[a] < hsh[b];
+    return a < b;
+  });
+  std::vector<int32_t> freeslots;
+  for (int s = 0; s < S; ++s) if (p->cart_in[s] < 0) freeslots.push_back(s);
+  for (int c : evictable) freeslots.push_back(p->slot_of[c]);
+  std::sort(freeslots.begin(), freeslots.end());
+  std::vector<char> used(freeslots.size(), 0);
+  std::vector<std::pair<int32_t, int32_t>> arrivals;   // (cart, slot)
+  for (int c : waiting) {
+    if ((int)arrivals.size() >= std::max(n_in, 0)) break;
+    for (size_t i = 0; i < freeslots.size(); ++i)
+      if (!used[i] && p->slot_cap[freeslots[i]] >= p->cart_len[c]) {
+        used[i] = 1;
+        arrivals.push_back({c, freeslots[i]});
+        break;
+      }
+  }
+  std::vector<std::pair<int32_t, int32_t>> outs;       // (slot, cart)
+  for (int c : evictable) outs.push_back({p->slot_of[c], c});
+  std::sort(outs.begin(), outs.end());
+  const int total = (int)(outs.size() + arrivals.size());
+  if (total > capacity) { set_error("manifest needs %d entries", total); return CAS_ERR_CAPACITY; }
+  int k = 0;
+  for (auto& o : outs) entries[k++] = {o.second, o.first, CAS_DIR_OUT, 0, p->home_off[o.second], p->home_bytes(o.second)};
+  for (auto& a : arrivals) entries[k++] = {a.first, a.second, CAS_DIR_IN, 0, p->home_off[a.first], p->home_bytes(a.first)};
+  *n_entries = k;
+  return CAS_OK;
+}
+
+static int copy_cart(cas_pool* p, int c, int s, bool to_host) {
+  const int64_t n = (int64_t)p->cart_len[c] * p->row_elems;
+  const cudaMemcpyKind kind = to_host ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice;
+  if (p->cart_len[c] == p->slot_cap[s]) {   // the six tensors are contiguous on both sides
+    void* d = p->slot_state(s, 0);
+    void* h = p->home(c, 0);
+    CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, 6 * n * 4, kind, p->side));
+  } else {
+    for (int w = 0; w < 6; ++w) {
+      void* d = p->slot_state(s, w);
+      void* h = p->home(c, w);
+      CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, n * 4, kind, p->side));
+    }
+  }
+  return CAS_OK;
+}
+
+int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t step, void* after_stream) {
+  if (!p || (n && !e) || n < 0) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  for (int i = 0; i < n; ++i) {
+    if (e[i].dir != CAS_DIR_OUT) continue;
+    const int c = e[i].cart, s = e[i].slot;
+    if (c < 0 || c >= p->desc.n_carts || s < 0 || s >= p->desc.n_slots) { set_error("bad manifest entry"); return CAS_ERR_INVALID_ARG; }
+    if (p->slot_of[c] != s) { set_error("cartridge %d is not in slot %d", c, s); return CAS_ERR_NOT_RESIDENT; }
+    if (p->in_transit[c]) { set_error("cartridge %d already in transit", c); return CAS_ERR_BUSY; }
+    if (p->grad_dirty[s]) { set_error("slot %d has un-consumed gradients", s); return CAS_ERR_BUSY; }
+    if (e[i].host_off != p->home_off[c] || e[i].nbytes != p->home_bytes(c)) { set_error("manifest bytes mismatch"); return CAS_ERR_INVALID_ARG; }
+  }
+  if (p->dev) {
+    if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+    if (after_stream != (void*)p->side) {
+      CAS_CUDA(cudaEventRecord(p->ev_main, (cudaStream_t)after_stream));
+      CAS_CUDA(cudaStreamWaitEvent(p->side, p->ev_main, 0));
+    }
+  }
+  for (int i = 0; i < n; ++i) {
+    if (e[i].dir != CAS_DIR_OUT) continue;
+    if (p->dev) { int rc = copy_cart(p, e[i].cart, e[i].slot, true); if (rc) return rc; }
+    p->in_transit[e[i].cart] = 1;
+    p->pending.push_back({e[i], step});
+  }
+  return CAS_OK;
+}
+
+int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t step) {
+  if (!p || (n && !e) || n < 0) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  std::set<int32_t> leaving, taken;
+  for (auto& q : p->pending) {
+    if (q.e.dir == CAS_DIR_OUT) leaving.insert(q.e.slot);
+    else taken.insert(q.e.slot);
+  }
+  for (int i = 0; i < n; ++i) {
+    if (e[i].dir != CAS_DIR_IN) continue;
+    const int c = e[i].cart, s = e[i].slot;
+    if (c < 0 || c >= p->desc.n_carts || s < 0 || s >= p->desc.n_slots) { set_error("bad manifest entry"); return CAS_ERR_INVALID_ARG; }
+    if (p->slot_of[c] >= 0 || p->in_transit[c]) { set_error("cartridge %d already resident / in transit", c); return CAS_ERR_BUSY; }
+    if (!(p->cart_in[s] < 0 || leaving.count(s)) || !taken.insert(s).second) { set_error("slot %d occupied", s); return CAS_ERR_BUSY; }
+    if (p->slot_cap[s] < p->cart_len[c]) { set_error("slot %d too small", s); return CAS_ERR_CAPACITY; }
+    if (e[i].host_off != p->home_off[c] || e[i].nbytes != p->home_bytes(c)) { set_error("manifest bytes mismatch"); return CAS_ERR_INVALID_ARG; }
+  }
+  if (p->dev && !p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+  for (int i = 0; i < n; ++i) {
+    if (e[i].dir != CAS_DIR_IN) continue;
+    const int c = e[i].cart, s = e[i].slot;
+    if (p->dev) {
+      int rc = copy_cart(p, c, s, false);
+      if (rc) return rc;
+      const int64_t o = (int64_t)p->slot_base[s] * p->row_elems, nel = (int64_t)p->cart_len[c] * p->row_elems;
+      rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
+                          (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, nel,
+                          p->desc.dtype, p->side);
+      if (rc) return rc;
+    }
+    p->in_transit[c] = 2;
+    p->pending.push_back({e[i], step});
+  }
+  return CAS_OK;
+}
+
+int cas_swap_commit(cas_pool* p, void* main_stream) {
+  if (!p) { set_error("null pool"); return CAS_ERR_INVALID_ARG; }
+  if (p->dev && !p->pending.empty()) {
+    CAS_CUDA(cudaEventRecord(p->ev_side, p->side));
+    CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)main_stream, p->ev_side, 0));
+  }
+  for (auto& q : p->pending)
+    if (q.e.dir == CAS_DIR_OUT) {
+      p->slot_of[q.e.cart] = -1;
+      p->in_transit[q.e.cart] = 0;
+      if (p->cart_in[q.e.slot] == q.e.cart) p->cart_in[q.e.slot] = -1;
+    }
+  for (auto& q : p->pending)
+    if (q.e.dir == CAS_DIR_IN) {
+      p->slot_of[q.e.cart] = q.e.slot;
+      p->cart_in[q.e.slot] = q.e.cart;
+      p->in_transit[q.e.cart] = 0;
+      p->last_used[q.e.cart] = q.step;
+    }
+  p->pending.clear();
+  return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// end-to-end step from host buffers
+// ---------------------------------------------------------------------------------------------
+struct StepScratch {
+  size_t oQ, oKs, oVs, odO, oO, oLSE, odQ, odKs, odVs, oWs, ws_bytes, total;
+};
+
+static StepScratch step_scratch(const cas_pool* p, const cas_slot_table* t, int Hq) {
+  StepScratch s{};
+  const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
+  size_t o = 0;
+  auto add = [&](size_t bytes) { size_t r = o; o = (size_t)round_up((int64_t)(o + bytes), 1024); return r; };
+  s.oQ = add(T * Hq * D * eb);   s.oKs = add(T * Hkv * D * eb); s.oVs = add(T * Hkv * D * eb);
+  s.odO = add(T * Hq * D * eb);  s.oO = add(T * Hq * D * eb);   s.oLSE = add(T * Hq * 4);
+  s.odQ = add(T * Hq * D * eb);  s.odKs = add(T * Hkv * D * eb); s.odVs = add(T * Hkv * D * eb);
+  cas_prefix_attn_bwd_workspace_bytes(p, t, Hq, &s.ws_bytes);
+  s.oWs = add(s.ws_bytes);
+  s.total = o;
+  return s;
+}
+
+int cas_train_step_host_scratch_bytes(const cas_pool* p, const cas_slot_table* t, int32_t Hq, size_t* bytes) {
+  if (!p || !t || !bytes || Hq < 1) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  *bytes = step_scratch(p, t, Hq).total;
+  return CAS_OK;
+}
+
+int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
+                        const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
+                        float* hLSE, void* hdQ, void* scratch, size_t scratch_bytes, void* stream) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (!t || !hQ || !hKs || !hVs || !hdO || !cfg || !hO || !hLSE || !hdQ || !scratch) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  const StepScratch s = step_scratch(p, t, Hq);
+  if (scratch_bytes < s.total) { set_error("scratch too small: need %zu", s.total); return CAS_ERR_CAPACITY; }
+  char* d = (char*)scratch;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
+  CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, st));
+  CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, st));
+  CAS_CUDA(cudaMemcpyAsync(d + s.oVs, hVs, T * Hkv * D * eb, cudaMemcpyHostToDevice, st));
+  CAS_CUDA(cudaMemcpyAsync(d + s.odO, hdO, T * Hq * D * eb, cudaMemcpyHostToDevice, st));
+  rc = cas_prefix_attn_fwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, scale, d + s.oO, (float*)(d + s.oLSE), stream);
+  if (rc) return rc;
+  rc = cas_prefix_attn_bwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, d + s.oO, (float*)(d + s.oLSE), d + s.odO,
+                           scale, d + s.odQ, d + s.odKs, d + s.odVs, d + s.oWs, s.ws_bytes, stream);
+  if (rc) return rc;
+  rc = cas_adam_step(p, cfg, nullptr, 0, nullptr, stream);
+  if (rc) return rc;
+  CAS_CUDA(cudaMemcpyAsync(hO, d + s.oO, T * Hq * D * eb, cudaMemcpyDeviceToHost, st));
+  CAS_CUDA(cudaMemcpyAsync(hLSE, d + s.oLSE, T * Hq * 4, cudaMemcpyDeviceToHost, st));
+  CAS_CUDA(cudaMemcpyAsync(hdQ, d + s.odQ, T * Hq * D * eb, cudaMemcpyDeviceToHost, st));
+  return CAS_OK;
+}
+
+}  // extern "C"

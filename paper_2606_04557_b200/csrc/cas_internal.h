@@ -1,0 +1,167 @@
+// Internal declarations shared by the host runtime (cas_host.cu) and the kernel translation units.
+// Not part of the ABI.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/cas.h"
+
+namespace cas {
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);
+
+#define CAS_CUDA(expr)                                     \
+  do {                                                     \
+    cudaError_t _e = (expr);                               \
+    if (_e != cudaSuccess) return cas::cuda_fail(_e, #expr); \
+  } while (0)
+
+struct Pending {
+  cas_manifest_entry e;
+  int64_t step;
+};
+
+// One KV tile (<= tile_tokens keys that never straddle two slots).
+struct KvTile {
+  int32_t tok;   // first pool token (prefix tile) / first packed token (self tile)
+  int32_t len;   // valid keys in the tile, 1..128
+};
+
+// Backward work item: one KV tile of one KV head is owned by one CTA (deterministic dK/dV).
+struct BwdItem {
+  int32_t kind;     // 0 = prefix tile of a slot, 1 = self tile of a sequence
+  int32_t id;       // slot (kind 0) or sequence (kind 1)
+  int32_t tok;      // first key token of the tile (pool token / packed token)
+  int32_t len;      // valid keys
+  int32_t jt;       // tile index inside the slot / sequence
+  int32_t cost;     // number of (q-tile, head) inner iterations (for longest-first ordering)
+};
+
+// Forward work item: one block of query rows of one sequence (all heads enumerated by the grid).
+struct FwdItem {
+  int32_t seq;
+  int32_t row0;     // first row inside the sequence
+  int32_t rows;     // rows in this block (<= block size)
+  int32_t cost;
+};
+
+}  // namespace cas
+
+struct cas_pool {
+  cas_pool_desc desc;
+  std::vector<int32_t> cart_len;
+  int32_t tile = 128;
+  int64_t row_elems = 0;   // Hkv*D
+  int elem_bytes = 2;
+  std::vector<int32_t> slot_base, slot_cap;
+  int64_t pool_tokens = 0;
+  std::vector<int64_t> home_off;
+  std::vector<int32_t> slot_of, cart_in, in_transit, grad_dirty;
+  std::vector<int64_t> opt_steps, last_used;
+  std::vector<cas::Pending> pending;
+  // data (caller-owned arenas)
+  char* dev = nullptr;
+  char* pinned = nullptr;
+  cudaStream_t side = nullptr;
+  void* pool_K = nullptr;
+  void* pool_V = nullptr;
+  float* grad_K = nullptr;
+  float* grad_V = nullptr;
+  float* state = nullptr;
+  cudaEvent_t ev_side = nullptr, ev_main = nullptr;
+  // library-owned device metadata for Adam launches (slot descriptors)
+  void* d_adam_desc = nullptr;
+  void* h_adam_desc = nullptr;   // pinned staging
+  int adam_desc_cap = 0;
+  cudaEvent_t ev_adam_desc = nullptr;
+  // TMA descriptors over the working copy (bf16, D==128 only)
+  bool has_tma = false;
+  CUtensorMap tm_K, tm_V;
+
+  float* slot_state(int s, int which) const {  // which: 0..5 = pK,pV,mK,mV,vK,vV
+    return state + 6 * (int64_t)slot_base[s] * row_elems + (int64_t)which * slot_cap[s] * row_elems;
+  }
+  int64_t home_bytes(int c) const { return 6 * (int64_t)cart_len[c] * row_elems * 4; }
+  float* home(int c, int which) const {
+    return (float*)(pinned + home_off[c]) + (int64_t)which * cart_len[c] * row_elems;
+  }
+};
+
+struct cas_slot_table {
+  cas_pool* pool = nullptr;
+  int32_t B = 0, T = 0, nsel = 0;
+  std::vector<int32_t> seq_off, sel_off, sel_cart, sel_slot, sel_base, sel_len, inv_off, inv_seq;
+  std::vector<int64_t> P;
+  std::vector<int32_t> used_slots;            // distinct selected slots, ascending
+  std::vector<int32_t> kv_tile_off;           // [B+1] into kv_tiles (prefix tiles of sequence b)
+  std::vector<cas::KvTile> kv_tiles;
+  std::vector<cas::FwdItem> fwd_items;        // 256-row blocks, longest first
+  std::vector<cas::FwdItem> simt_items;       // 32-row blocks
+  std::vector<cas::BwdItem> bwd_items;        // longest first
+  int64_t pairs = 0, prefix_tokens = 0, unique_prefix_tokens = 0;
+  int32_t max_lq = 0;
+  // one device blob holding all the arrays above
+  char* d_blob = nullptr;
+  int32_t *d_seq_off = nullptr, *d_sel_off = nullptr, *d_sel_base = nullptr, *d_sel_len = nullptr,
+          *d_inv_off = nullptr, *d_inv_seq = nullptr, *d_kv_tile_off = nullptr,
+          *d_used_slots = nullptr, *d_sel_slot = nullptr;
+  cas::KvTile* d_kv_tiles = nullptr;
+  cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
+  cas::BwdItem* d_bwd_items = nullptr;
+  int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
+};
+
+namespace cas {
+
+// ---- kernel launchers (each returns CAS_OK / CAS_ERR_*) -------------------------------------
+struct AttnArgs {
+  const cas_pool* pool;
+  const cas_slot_table* tab;
+  int Hq, Hkv, D, dtype;
+  const void *Q, *Ks, *Vs, *O, *dO;
+  const float* LSE_in;
+  void *O_out, *dQ, *dKs, *dVs;
+  float* LSE_out;
+  float scale;
+  void* workspace;
+  size_t workspace_bytes;
+  cudaStream_t stream;
+};
+
+int simt_attn_fwd(const AttnArgs& a);
+int simt_attn_bwd(const AttnArgs& a);
+size_t simt_bwd_workspace(const cas_slot_table* t, int Hq);
+
+bool tc_supported(const cas_pool* p, const cas_slot_table* t, int Hq);
+int tc_attn_fwd(const AttnArgs& a);
+int tc_attn_bwd(const AttnArgs& a);
+size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D);
+int tc_make_pool_maps(cas_pool* p);
+
+// Adam / refresh / zero
+struct AdamSlotDesc {
+  float* state;       // slot_state(s,0)
+  void* wK;           // working copy of the slot (K), V is at wV
+  void* wV;
+  float* gK;
+  float* gV;
+  int64_t cap_elems;  // slot_cap*row_elems  (stride between the six state tensors)
+  int64_t n_elems;    // cart_len*row_elems
+  int64_t frozen_elems;
+  float step_size_scale;  // lr_scale
+  float bc1, bc2;     // 1-beta1^t, 1-beta2^t
+  int32_t pad;
+};
+int launch_adam(const AdamSlotDesc* d_desc, int n, int64_t max_elems, const cas_adam_cfg& cfg,
+                int dtype, cudaStream_t st);
+int launch_refresh(float* pK, float* pV, void* wK, void* wV, float* gK, float* gV, int64_t n,
+                   int dtype, cudaStream_t st);
+int launch_zero(float* p, int64_t n, cudaStream_t st);
+
+}  // namespace cas

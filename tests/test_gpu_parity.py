@@ -1,0 +1,133 @@
+"""GPU parity: the CUDA path (through the C ABI) against oracle/ on the same seeded inputs.
+Small cases compare every output element; full-size configs compare every output element of one KV
+head group (the oracle computes that group completely) plus properties over all heads."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_04557_b200 import _build, cas
+from workloads import CONFIGS, make_workload
+
+from parity_util import check_adam_isolated, check_attention
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    _build.build()
+    yield
+    cas.cas_set_impl(cas.CAS_IMPL_AUTO)
+
+
+def small_ragged(dtype="bf16", D=128, seed=5):
+    """config-4-shaped (lognormal lengths, proportional draws, ragged Lq) at oracle-friendly size:
+    lengths span 1..6 KV tiles with ragged tails, query lengths span 1..4 Q tiles."""
+    return CONFIGS["c4"].scaled(name="c4_small", dtype=dtype, Hq=8, Hkv=2, D=D, n_carts=12, n_slots=12,
+                                B=5, len_mu=5.3, len_sigma=0.8, len_min=17, len_max=700, lq_min=3,
+                                lq_max=450, n_dist_max=6), seed
+
+
+# ------------------------------------------------------------------ config 1 (tiny fp32), complete
+def test_c1_tiny_fp32_full_parity_and_adam():
+    wl = make_workload(CONFIGS["c1"])
+    rep = {}
+    sess = check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[0], report=rep)
+    used = sorted(set(wl.sel_cart.tolist()))
+    worst = check_adam_isolated(sess, used)
+    print("c1", rep, "adam", worst)
+    sess.close()
+
+
+def test_c1_prefix_only_and_accumulate():
+    wl = make_workload(CONFIGS["c1"], seed=11)
+    sess = check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[0], self_block=False)
+    # second backward accumulates (+=): gradients double
+    c = int(wl.sel_cart[0])
+    g1 = sess.read(c, "gK").copy()
+    sess.bwd(self_block=False)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(sess.read(c, "gK"), 2 * g1, rtol=1e-6, atol=1e-9)
+    sess.close()
+
+
+def test_sequence_without_cartridges_is_plain_causal_attention():
+    wl = make_workload(CONFIGS["c1"], seed=12)
+    n0 = int(wl.sel_off[1])
+    wl.sel_cart = wl.sel_cart[n0:].copy()
+    wl.sel_off = np.array([0, 0, len(wl.sel_cart)], dtype=np.int32)
+    check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[0]).close()
+
+
+def test_adam_frozen_tokens_lr_scale_and_second_step():
+    wl = make_workload(CONFIGS["c1"], seed=13)
+    sess = check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[0])
+    used = sorted(set(wl.sel_cart.tolist()))
+    check_adam_isolated(sess, used, n_frozen=1, lr_scale=[0.25 * (i + 1) for i in range(len(used))])
+    sess.bwd()                                  # new gradients, t = 2 (bias correction changes)
+    torch.cuda.synchronize()
+    check_adam_isolated(sess, used)
+    # a resident cartridge nobody selected: g = 0, m = v = 0  ->  exact no-op (R10)
+    rest = [c for c in range(4) if c not in used]
+    for c in rest:
+        p0 = sess.read(c, "pK").copy()
+        check_adam_isolated(sess, [c])
+        np.testing.assert_array_equal(sess.read(c, "pK"), p0)
+    sess.close()
+
+
+# ------------------------------------------------------------------ small ragged cases, complete
+@pytest.mark.parametrize("impl", [cas.CAS_IMPL_SIMT, cas.CAS_IMPL_AUTO])
+@pytest.mark.parametrize("dtype,D", [("bf16", 128), ("f32", 64), ("bf16", 64)])
+def test_small_ragged_all_heads(impl, dtype, D):
+    cfg, seed = small_ragged(dtype, D)
+    wl = make_workload(cfg, seed)
+    rep = {}
+    sess = check_attention(wl, impl, kv_heads=[0, 1], report=rep)
+    print(dtype, D, impl, rep)
+    check_adam_isolated(sess, sorted(set(wl.sel_cart.tolist()))[:3])
+    sess.close()
+
+
+@pytest.mark.parametrize("impl", [cas.CAS_IMPL_SIMT, cas.CAS_IMPL_AUTO])
+def test_small_c2_shape(impl):
+    cfg = CONFIGS["c2"].scaled(name="c2_small", n_carts=12, n_slots=12, cart_len=320, B=3, Lq=384, n_dist=3)
+    wl = make_workload(cfg, 21)
+    rep = {}
+    check_attention(wl, impl, kv_heads=[0, 5], report=rep).close()
+    print(rep)
+
+
+@pytest.mark.parametrize("impl", [cas.CAS_IMPL_SIMT, cas.CAS_IMPL_AUTO])
+def test_small_decode_shape(impl):
+    cfg = CONFIGS["c5_top8"].scaled(name="c5_small", n_carts=20, n_slots=20, cart_len=200, B=9, n_dist=4)
+    wl = make_workload(cfg, 22)
+    check_attention(wl, impl, kv_heads=[0, 3, 7]).close()
+    cfg = CONFIGS["c5_all"].scaled(name="c5_small_all", n_carts=6, n_slots=6, cart_len=130, B=3)
+    check_attention(make_workload(cfg, 23), impl, kv_heads=[1]).close()
+
+
+# ------------------------------------------------------------------ full-size configs, one KV head
+def test_c2_full_size_one_kv_head():
+    wl = make_workload(CONFIGS["c2"])
+    rep = {}
+    sess = check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[3], report=rep)
+    print("c2", rep)
+    used = sorted(set(wl.sel_cart.tolist()))
+    check_adam_isolated(sess, used[:2])
+    sess.close()
+
+
+def test_c4_full_size_one_kv_head():
+    wl = make_workload(CONFIGS["c4"])
+    rep = {}
+    check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[6], report=rep).close()
+    print("c4", rep)
+
+
+def test_c5_full_size_decode():
+    for name, g in (("c5_all", 2), ("c5_top8", 5)):
+        wl = make_workload(CONFIGS[name])
+        rep = {}
+        check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[g], report=rep).close()
+        print(name, rep)
