@@ -39,6 +39,10 @@ adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2
     float* __restrict__ v = d.state + (int64_t)(4 + which) * d.cap_elems;
     float* __restrict__ g = which ? d.gV : d.gK;
     void* w = which ? d.wV : d.wK;
+    if (zero_grad)   // frozen tokens are not updated, but their gradients are consumed
+      for (int64_t i = ((int64_t)blockIdx.x * kAdamThreads + threadIdx.x) * 4; i < d.frozen_elems;
+           i += (int64_t)gridDim.x * kAdamThreads * 4)
+        st4(g + i, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int64_t base = d.frozen_elems + (int64_t)blockIdx.x * chunk; base < d.n_elems;
          base += (int64_t)gridDim.x * chunk) {
       float4 G[kAdamUnroll], P[kAdamUnroll], M[kAdamUnroll], V[kAdamUnroll];

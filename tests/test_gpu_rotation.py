@@ -34,6 +34,7 @@ def run_rotation(cfg, steps, seed, check_attn_every=1):
     wl = make_workload(cfg, seed)
     sess = Session(wl)
     bk = PoolBook(wl.cart_len.tolist(), cfg.n_slots, cfg.Hkv, cfg.D)
+    bk.slot_table(wl.seq_off.tolist(), wl.sel_off.tolist(), wl.sel_cart.tolist(), 0)   # Session's own table
     rng = np.random.Generator(np.random.PCG64(seed + 1))
     main = torch.cuda.current_stream()
     G = cfg.Hq // cfg.Hkv
