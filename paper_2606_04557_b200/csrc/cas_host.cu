@@ -351,12 +351,14 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
   // KV tile lists + work lists
   const int tile = 128;
   t->kv_tile_off.assign(B + 1, 0);
+  t->qtile_off.assign(B + 1, 0);
   for (int b = 0; b < B; ++b) {
     for (int k = sel_off[b]; k < sel_off[b + 1]; ++k)
       for (int j = 0; j < t->sel_len[k]; j += tile)
         t->kv_tiles.push_back({t->sel_base[k] + j, std::min(tile, t->sel_len[k] - j)});
     t->kv_tile_off[b + 1] = (int32_t)t->kv_tiles.size();
     const int64_t lq = seq_off[b + 1] - seq_off[b];
+    t->qtile_off[b + 1] = t->qtile_off[b] + (int32_t)((lq + 127) / 128);
     t->max_lq = std::max<int32_t>(t->max_lq, (int32_t)lq);
     t->pairs += lq * t->P[b] + lq * (lq + 1) / 2;
     t->prefix_tokens += t->P[b];
@@ -396,7 +398,7 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
                  o_iseq = blob_add(off, t->inv_seq, 1), o_kto = blob_add(off, t->kv_tile_off),
                  o_kt = blob_add(off, t->kv_tiles, 1), o_fw = blob_add(off, t->fwd_items),
                  o_si = blob_add(off, t->simt_items), o_bw = blob_add(off, t->bwd_items),
-                 o_us = blob_add(off, t->used_slots, 1);
+                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off);
     const size_t o_cnt = off;
     off += 256;
     std::vector<char> h(off, 0);
@@ -414,6 +416,7 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     put(o_si, t->simt_items.data(), t->simt_items.size() * sizeof(FwdItem));
     put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
     put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
+    put(o_qt, t->qtile_off.data(), t->qtile_off.size() * 4);
     cudaError_t e = cudaMalloc((void**)&t->d_blob, off);
     if (e == cudaSuccess) e = cudaMemcpy(t->d_blob, h.data(), off, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { if (t->d_blob) cudaFree(t->d_blob); delete t; return cuda_fail(e, "slot table upload"); }
@@ -431,6 +434,7 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     t->d_simt_items = (FwdItem*)(d + o_si);
     t->d_bwd_items = (BwdItem*)(d + o_bw);
     t->d_used_slots = (int32_t*)(d + o_us);
+    t->d_qtile_off = (int32_t*)(d + o_qt);
     t->d_counters = (int32_t*)(d + o_cnt);
   }
   *out = t;

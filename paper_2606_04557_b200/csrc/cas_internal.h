@@ -100,6 +100,7 @@ struct cas_slot_table {
   std::vector<int64_t> P;
   std::vector<int32_t> used_slots;            // distinct selected slots, ascending
   std::vector<int32_t> kv_tile_off;           // [B+1] into kv_tiles (prefix tiles of sequence b)
+  std::vector<int32_t> qtile_off;             // [B+1] 128-row query tiles before sequence b
   std::vector<cas::KvTile> kv_tiles;
   std::vector<cas::FwdItem> fwd_items;        // 256-row blocks, longest first
   std::vector<cas::FwdItem> simt_items;       // 32-row blocks
@@ -110,7 +111,7 @@ struct cas_slot_table {
   char* d_blob = nullptr;
   int32_t *d_seq_off = nullptr, *d_sel_off = nullptr, *d_sel_base = nullptr, *d_sel_len = nullptr,
           *d_inv_off = nullptr, *d_inv_seq = nullptr, *d_kv_tile_off = nullptr,
-          *d_used_slots = nullptr, *d_sel_slot = nullptr;
+          *d_used_slots = nullptr, *d_sel_slot = nullptr, *d_qtile_off = nullptr;
   cas::KvTile* d_kv_tiles = nullptr;
   cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
   cas::BwdItem* d_bwd_items = nullptr;
