@@ -155,6 +155,7 @@ def main():
     ap.add_argument("--config", default="c2")
     ap.add_argument("--kernels", default="auto", choices=["auto", "simt", "tc"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--ref-budget", type=float, default=8.0)
     ap.add_argument("--ref-units", type=int, default=64)
     args = ap.parse_args()
@@ -237,7 +238,7 @@ def main():
 
     # ---- e2e: host buffers through cas_train_step_host
     e2e = None
-    if cfg.backward:
+    if cfg.backward and not args.no_e2e:
         tdt = sess.tdt
         pin = lambda a: torch.from_numpy(a).to(tdt).pin_memory()
         hQ, hKs, hVs, hdO = pin(wl.Q), pin(wl.K_self), pin(wl.V_self), pin(wl.dO)
