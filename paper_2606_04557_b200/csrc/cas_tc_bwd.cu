@@ -6,17 +6,24 @@
 // (read in place from the pool) or of a sequence's own keys -- and walks, through the INVERTED slot
 // table, every (sequence that selected the slot) x (query head of the group) x (128-row Q tile).
 // dK/dV of the tile accumulate in TMEM over that whole loop and are written ONCE ("+=" into the
-// slot's fp32 gradient buffer, no atomics, deterministic).  dQ tiles are reduced into an fp32
-// scratch with vector red.global.add and converted to bf16 (x scale) by a small epilogue kernel.
+// slot's fp32 gradient buffer, no atomics, deterministic).  dQ tiles are staged through shared
+// memory and added to an fp32 scratch with bulk reductions (cp.reduce.async.bulk ... add.f32: one
+// 16 KB contiguous L2 reduction per quarter tile), then converted to bf16 (x scale) by an epilogue
+// kernel.
 //
 // Per inner iteration i (Q tile, dO tile, LSE, delta of 128 query rows), five MMAs, keys on lanes:
 //   S^T  = K  Q^T        (SS)            dP^T = V  dO^T      (SS)
 //   dV  += P^T dO        (P^T from TMEM) dK  += dS^T Q       (dS^T from SMEM, K-major)
 //   dQ   = dS  K         (the same dS^T bytes in SMEM read as an MN-major A operand)
-// TMEM (512 cols): [S^T / P^T] [dP^T / dQ] [dV] [dK].   SMEM (224 KB): K,V | 2 x (Q,dO) | dS^T.
-// Warps: 0-3 softmax-backward (thread = key), 4-7 dQ reducers (thread = query), 8 TMA, 9 MMA.
-// Issue order:  dV(i)  S(i+1)  dK(i) dQ(i)  [dQ drained]  dP(i+1)   -- exp of tile i+1 overlaps
-// dK/dQ of tile i; the dQ drain overlaps the exp as well.
+// TMEM (512 cols): [S^T / P^T] [dP^T / dQ] [dV] [dK].   SMEM (226 KB): K,V | 2 x Q | 2 x dO | dS^T.
+// Warps: 0-3 / 4-7 two compute warpgroups (thread = key; group w owns query columns [64w, 64w+64)):
+// exp -> P^T, then dS^T; 8-11 dQ reducers (thread = query); 12 TMA producer; 13 MMA issuer.
+// Issue order:  dV(i)  S(i+1)  dQ(i) dK(i)  [dQ drained]  dP(i+1)   -- the exp of tile i+1 overlaps
+// dQ/dK of tile i, the dQ drain overlaps dK.  The dQ staging buffer of iteration i is the dO stage of
+// iteration i (dead once dV(i) has been issued); that stage is handed back to the producer when the
+// bulk reductions have finished reading it.
+#include <cstdlib>
+
 #include "cas_sm100.cuh"
 #include "cas_tc_common.cuh"
 
@@ -57,27 +64,41 @@ bwd_prep_kernel(const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __rest
   }
 }
 
-// dQ = bf16(scale * dQ_acc)
+// dQ scratch layout (written by the bulk reductions of tc_bwd_kernel): per (head h, global Q tile u)
+// four quarter tiles of 32 columns, each [128 rows][32 fp32] = 16 KB contiguous; inside a 128-byte
+// row the 16-byte chunk j sits at position j ^ (row & 7) (bank-conflict-free staging stores).
+// dQ[t,h,:] = bf16(scale * scratch);  one warp per (t, h) row, lane = 4 columns.
 __global__ void __launch_bounds__(256)
-dq_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dQ, float scale, int64_t n4) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
-    const float4 v = reinterpret_cast<const float4*>(acc)[i];
-    uint2 u;
-    u.x = pack_bf16(v.x * scale, v.y * scale);
-    u.y = pack_bf16(v.z * scale, v.w * scale);
-    reinterpret_cast<uint2*>(dQ)[i] = u;
+dq_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dQ, const int32_t* __restrict__ seq_off,
+                  const int32_t* __restrict__ qtile_off, int B, int Hq, int64_t nqt, float scale, int64_t n_rows) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (w >= n_rows) return;
+  const int t = (int)(w / Hq), h = (int)(w % Hq);
+  int lo = 0, hi = B - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (seq_off[mid] <= t) lo = mid; else hi = mid - 1;
   }
+  const int row = t - seq_off[lo];
+  const int64_t u = qtile_off[lo] + (row >> 7);
+  const int r = row & 127, c = lane >> 3, j = lane & 7;
+  const float4 v = *reinterpret_cast<const float4*>(acc + (((int64_t)h * nqt + u) * 4 + c) * 4096 + r * 32 +
+                                                    ((j ^ (r & 7)) << 2));
+  uint2 o;
+  o.x = pack_bf16(v.x * scale, v.y * scale);
+  o.y = pack_bf16(v.z * scale, v.w * scale);
+  *reinterpret_cast<uint2*>(dQ + w * 128 + lane * 4) = o;
 }
 
 // ------------------------------------------------------------------------------- main kernel
-constexpr int kBwdThreads = 384;   // warps 10,11 idle: whole warpgroups for setmaxnreg
+constexpr int kBwdThreads = 512;   // 4 warpgroups (setmaxnreg works on whole warpgroups); warps 14,15 idle
 constexpr uint32_t kT = 32768, kH = 16384;
 constexpr uint32_t oK = 0, oV = kT, oQ = 2 * kT, oDO = 4 * kT, oDS = 6 * kT, oAuxL = 7 * kT, oAuxD = 7 * kT + 1024,
                    oBar = 7 * kT + 2048;
 constexpr uint32_t kBwdSmem = oBar + 256;
-enum { C_KV = 0, C_QF = 1, C_DOF = 3, C_STE = 5, C_SF = 7, C_DPF = 8, C_PF = 9, C_DSF = 10, C_DQF = 11, C_DQD = 12,
-       C_DONE = 13, C_N = 14 };
+enum { C_KV = 0, C_QF = 1, C_DOF = 3, C_QE = 5, C_DOE = 7, C_SF = 9, C_DPF = 10, C_PF = 11, C_DSF = 12, C_DQF = 13,
+       C_DQD = 14, C_DONE = 15, C_N = 16 };
 
 struct BwdParams {
   const int32_t *seq_off, *inv_off, *inv_seq, *qtile_off;
@@ -86,7 +107,7 @@ struct BwdParams {
   float* dQacc;
   float *gradK, *gradV;
   __nv_bfloat16 *dKs, *dVs;
-  int64_t aux_stride;
+  int64_t aux_stride;     // nqt * 128
   int Hq, Hkv, has_self;
   float scale, scale_log2;
 };
@@ -127,7 +148,8 @@ struct Walk {
   }
   __device__ int tok() const { return t0 + 128 * qt; }                       // first packed token
   __device__ int rows() const { return min(128, lq - 128 * qt); }            // valid query rows
-  __device__ int64_t aux() const { return (int64_t)h * p.aux_stride + (int64_t)(p.qtile_off[b] + qt) * 128; }
+  __device__ int64_t utile() const { return p.qtile_off[b] + qt; }           // global Q tile index
+  __device__ int64_t aux() const { return (int64_t)h * p.aux_stride + utile() * 128; }
 };
 
 template <int N>
@@ -151,10 +173,11 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();
-    for (int i = 0; i < C_N; ++i) mbar_init(bar(i), (i == C_PF || i == C_DSF || i == C_DQD) ? 128 : 1);
+    for (int i = 0; i < C_N; ++i)
+      mbar_init(bar(i), (i == C_PF || i == C_DSF) ? 256 : (i == C_DQD ? 128 : 1));
     fence_mbar_init();
   }
-  if (warp == 8) {
+  if (warp == 12) {
     tmem_alloc(smem_u32(tmem_slot), 512);
     tmem_relinquish();
   }
@@ -164,9 +187,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   const uint32_t tbase = *tmem_slot;
   const uint32_t tS = tbase, tdP = tbase + 128, tdV = tbase + 256, tdK = tbase + 384;
 
-  if (warp >= 8) {
-    setmaxnreg_dec<64>();
-    if (warp == 8 && lane == 0) {
+  if (warp >= 12) {
+    setmaxnreg_dec<56>();
+    if (warp == 12 && lane == 0) {
       // ================================================================= TMA producer
       const CUtensorMap* mk = it.kind == 0 ? &tmKp : &tmKs;
       const CUtensorMap* mv = it.kind == 0 ? &tmVp : &tmVs;
@@ -179,18 +202,20 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const int n = w.total();
       for (int i = 0; i < n; ++i) {
         const int st = i & 1;
-        mbar_wait(bar(C_STE + st), ((i >> 1) & 1) ^ 1);
+        const uint32_t eph = ((i >> 1) & 1) ^ 1;
+        mbar_wait(bar(C_QE + st), eph);
         mbar_expect_tx(bar(C_QF + st), kT + 512);
         tma_load_3d(sbase + oQ + st * kT, &tmQ, bar(C_QF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oQ + st * kT + kH, &tmQ, bar(C_QF + st), 64, w.h, w.tok());
         bulk_load(sbase + oAuxL + st * 512, prm.auxL + w.aux(), 512, bar(C_QF + st));
+        mbar_wait(bar(C_DOE + st), eph);
         mbar_expect_tx(bar(C_DOF + st), kT + 512);
         tma_load_3d(sbase + oDO + st * kT, &tmdO, bar(C_DOF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oDO + st * kT + kH, &tmdO, bar(C_DOF + st), 64, w.h, w.tok());
         bulk_load(sbase + oAuxD + st * 512, prm.auxD + w.aux(), 512, bar(C_DOF + st));
         w.next();
       }
-    } else if (warp == 9 && lane == 0) {
+    } else if (warp == 13 && lane == 0) {
       // ================================================================= MMA issuer
       constexpr uint32_t id_kk = make_idesc(128, 128, 0, 0), id_kmn = make_idesc(128, 128, 0, 1),
                          id_mnmn = make_idesc(128, 128, 1, 1);
@@ -220,9 +245,11 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const uint32_t ph1 = ((i + 1) >> 1) & 1;
         mbar_wait(bar(C_PF), i & 1);
         tc_fence_after();
+        // dV += P^T dO ; P^T (bf16) of query columns [0,64) sits at tS+[0,32), of [64,128) at tS+64+[0,32)
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)     // dV += P^T dO
-          mma_ts(tdV, tS + kk * 8, mnmaj(sbase + oDO + st * kT, kk), id_kmn, (i > 0 || kk > 0) ? 1u : 0u);
+        for (int kk = 0; kk < 8; ++kk)
+          mma_ts(tdV, tS + (kk >> 2) * 64 + (kk & 3) * 8, mnmaj(sbase + oDO + st * kT, kk), id_kmn,
+                 (i > 0 || kk > 0) ? 1u : 0u);
         if (i + 1 < n) {
           mbar_wait(bar(C_QF + st1), ph1);
           tc_fence_after();
@@ -232,13 +259,13 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         mbar_wait(bar(C_DSF), i & 1);
         tc_fence_after();
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)     // dK += dS^T Q
-          mma_ss(tdK, kmaj(sbase + oDS, kk), mnmaj(sbase + oQ + st * kT, kk), id_kmn, (i > 0 || kk > 0) ? 1u : 0u);
-#pragma unroll
         for (int kk = 0; kk < 8; ++kk)     // dQ = dS K
           mma_ss(tdP, mnmaj(sbase + oDS, kk), mnmaj(sbase + oK, kk), id_mnmn, kk > 0);
         mma_commit(bar(C_DQF));
-        mma_commit(bar(C_STE + st));
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk)     // dK += dS^T Q
+          mma_ss(tdK, kmaj(sbase + oDS, kk), mnmaj(sbase + oQ + st * kT, kk), id_kmn, (i > 0 || kk > 0) ? 1u : 0u);
+        mma_commit(bar(C_QE + st));
         if (i + 1 < n) {
           mbar_wait(bar(C_DOF + st1), ph1);
           mbar_wait(bar(C_DQD), i & 1);
@@ -249,45 +276,58 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       }
       mma_commit(bar(C_DONE));
     }
-  } else if (warp < 4) {
-    // =================================================================== softmax backward
-    setmaxnreg_inc<232>();
-    const int k = threadIdx.x;                       // key lane
-    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  } else if (warp < 8) {
+    // =================================================================== compute: P^T, dS^T
+    setmaxnreg_inc<168>();
+    const int wg = warp >> 2;                        // query-column half owned by this warpgroup
+    const int k = threadIdx.x & 127;                 // key lane
+    const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t tSw = tS + lane_base + wg * 64, tdPw = tdP + lane_base + wg * 64;
     const bool key_ok = k < it.len;
+    const uint32_t ds_row = sbase + oDS + wg * kH + k * 128;
     Walk w(prm, it, g);
     const int n = w.total();
     for (int i = 0; i < n; ++i) {
       const int st = i & 1;
       const uint32_t ph = (i >> 1) & 1;
       const int rows = w.rows();
-      // valid query columns: qlo <= q < qhi
-      const int qlo = (it.kind == 1 && w.qt == it.jt) ? k : 0;
+      const bool diag = it.kind == 1 && w.qt == it.jt;
+      const bool masked = diag || rows < 128 || it.len < 128;          // block-uniform
+      // valid query columns of this key: qlo <= q < qhi
+      const int qlo = diag ? k : 0;
       const int qhi = key_ok ? rows : 0;
-      const float* aL = reinterpret_cast<const float*>(smem + oAuxL + st * 512);
-      const float* aD = reinterpret_cast<const float*>(smem + oAuxD + st * 512);
+      const float4* aL = reinterpret_cast<const float4*>(smem + oAuxL + st * 512 + wg * 256);
+      const float4* aD = reinterpret_cast<const float4*>(smem + oAuxD + st * 512 + wg * 256);
       mbar_wait(bar(C_QF + st), ph);
       mbar_wait(bar(C_SF), i & 1);
       tc_fence_after();
-      float p[128];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        uint32_t s[32];
-        tmem_ld32(tS + lane_base + c * 32, s);
+      float p[64];
+      {
+        uint32_t s[64];
+        tmem_ld32(tSw, s);
+        tmem_ld32(tSw + 32, s + 32);
         tc_wait_ld();
 #pragma unroll
-        for (int q = 0; q < 32; ++q) {
-          const int qq = c * 32 + q;
-          const float e = ex2_approx(__uint_as_float(s[q]) * prm.scale_log2 - aL[qq]);
-          p[qq] = (qq >= qlo && qq < qhi) ? e : 0.f;
+        for (int q4 = 0; q4 < 16; ++q4) {
+          const float4 L = aL[q4];
+          p[4 * q4 + 0] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 0]), prm.scale_log2, -L.x));
+          p[4 * q4 + 1] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 1]), prm.scale_log2, -L.y));
+          p[4 * q4 + 2] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 2]), prm.scale_log2, -L.z));
+          p[4 * q4 + 3] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 3]), prm.scale_log2, -L.w));
         }
       }
+      if (masked) {
 #pragma unroll
-      for (int c = 0; c < 2; ++c) {
+        for (int q = 0; q < 64; ++q) {
+          const int qq = wg * 64 + q;
+          p[q] = (qq >= qlo && qq < qhi) ? p[q] : 0.f;
+        }
+      }
+      {
         uint32_t pk[32];
 #pragma unroll
-        for (int q = 0; q < 32; ++q) pk[q] = pack_bf16(p[c * 64 + 2 * q], p[c * 64 + 2 * q + 1]);
-        tmem_st32(tS + lane_base + c * 32, pk);
+        for (int q = 0; q < 32; ++q) pk[q] = pack_bf16(p[2 * q], p[2 * q + 1]);
+        tmem_st32(tSw, pk);
       }
       tc_wait_st();
       tc_fence_before();
@@ -296,22 +336,24 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       mbar_wait(bar(C_DPF), i & 1);
       tc_fence_after();
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
+      for (int c = 0; c < 2; ++c) {
         uint32_t d[32];
-        tmem_ld32(tdP + lane_base + c * 32, d);
+        tmem_ld32(tdPw + c * 32, d);
         tc_wait_ld();
 #pragma unroll
         for (int q8 = 0; q8 < 4; ++q8) {
+          const float4 D0 = aD[c * 8 + q8 * 2], D1 = aD[c * 8 + q8 * 2 + 1];
+          const int q = c * 32 + q8 * 8;
           uint32_t pk[4];
-#pragma unroll
-          for (int x = 0; x < 4; ++x) {
-            const int q = q8 * 8 + 2 * x, qq = c * 32 + q;
-            const float d0 = p[qq] * (__uint_as_float(d[q]) - aD[qq]);
-            const float d1 = p[qq + 1] * (__uint_as_float(d[q + 1]) - aD[qq + 1]);
-            pk[x] = pack_bf16(d0, d1);
-          }
-          const int q0 = c * 32 + q8 * 8;
-          const uint32_t addr = sbase + oDS + (q0 >> 6) * kH + k * 128 + ((((q0 >> 3) & 7) ^ (k & 7)) << 4);
+          pk[0] = pack_bf16(p[q + 0] * (__uint_as_float(d[q8 * 8 + 0]) - D0.x),
+                            p[q + 1] * (__uint_as_float(d[q8 * 8 + 1]) - D0.y));
+          pk[1] = pack_bf16(p[q + 2] * (__uint_as_float(d[q8 * 8 + 2]) - D0.z),
+                            p[q + 3] * (__uint_as_float(d[q8 * 8 + 3]) - D0.w));
+          pk[2] = pack_bf16(p[q + 4] * (__uint_as_float(d[q8 * 8 + 4]) - D1.x),
+                            p[q + 5] * (__uint_as_float(d[q8 * 8 + 5]) - D1.y));
+          pk[3] = pack_bf16(p[q + 6] * (__uint_as_float(d[q8 * 8 + 6]) - D1.z),
+                            p[q + 7] * (__uint_as_float(d[q8 * 8 + 7]) - D1.w));
+          const uint32_t addr = ds_row + ((uint32_t)((c * 4 + q8) ^ (k & 7)) << 4);
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
         }
       }
@@ -321,15 +363,16 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       w.next();
     }
   } else {
-    // =================================================================== dQ reducers
+    // =================================================================== dQ reducers (warps 8-11)
     setmaxnreg_dec<96>();
-    const int q = threadIdx.x - 128;                 // query lane
+    const int q = threadIdx.x - 256;                 // query lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     Walk w(prm, it, g);
     const int n = w.total();
     for (int i = 0; i < n; ++i) {
-      const bool ok = q < w.rows();
-      float* dst = prm.dQacc + ((int64_t)(w.tok() + q) * prm.Hq + w.h) * 128;
+      const int st = i & 1;
+      const uint32_t stage = sbase + oDO + st * kT;  // dO(i) is dead: its 32 KB stage two 16 KB quarter tiles
+      float* dst = prm.dQacc + ((int64_t)w.h * (prm.aux_stride >> 7) + w.utile()) * 16384;
       mbar_wait(bar(C_DQF), i & 1);
       tc_fence_after();
 #pragma unroll
@@ -341,15 +384,32 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           tc_fence_before();
           mbar_arrive(bar(C_DQD));
         }
-        if (ok) {
-#pragma unroll
-          for (int x = 0; x < 8; ++x)
-            red_add_v4(dst + c * 32 + x * 4, __uint_as_float(d[4 * x]), __uint_as_float(d[4 * x + 1]),
-                       __uint_as_float(d[4 * x + 2]), __uint_as_float(d[4 * x + 3]));
+        const uint32_t buf = stage + (c & 1) * kH;
+        if (c >= 2) {                                // quarter c-2 must have left this buffer
+          if (q == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+          asm volatile("bar.sync 1, 128;" ::: "memory");
         }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const uint32_t addr = buf + q * 128 + ((uint32_t)(j ^ (q & 7)) << 4);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(d[4 * j]), "r"(d[4 * j + 1]),
+                       "r"(d[4 * j + 2]), "r"(d[4 * j + 3]) : "memory");
+        }
+        fence_proxy_async();
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (q == 0) {
+          asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+                       ::"l"(dst + c * 4096), "r"(buf), "r"(16384u) : "memory");
+          asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+      }
+      if (q == 0) {
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        mbar_arrive(bar(C_DOE + st));
       }
       w.next();
     }
+    if (q == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   }
   // ===================================================================== dK / dV write-out
   if (warp < 8) {
@@ -395,7 +455,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 8) tmem_dealloc(tbase, 512);
+  if (warp == 12) tmem_dealloc(tbase, 512);
 }
 
 static inline size_t up1k(size_t x) { return (x + 1023) / 1024 * 1024; }
@@ -403,7 +463,7 @@ static inline size_t up1k(size_t x) { return (x + 1023) / 1024 * 1024; }
 size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D) {
   if (D != 128) return 0;
   const size_t nqt = (size_t)t->qtile_off[t->B];
-  return up1k((size_t)t->T * Hq * 128 * 4) + 2 * up1k((size_t)Hq * nqt * 128 * 4) + 1024;
+  return up1k((size_t)Hq * nqt * 65536) + 2 * up1k((size_t)Hq * nqt * 128 * 4) + 1024;
 }
 
 int tc_attn_bwd(const AttnArgs& a) {
@@ -414,7 +474,7 @@ int tc_attn_bwd(const AttnArgs& a) {
     attr_set = true;
   }
   const size_t nqt = (size_t)t->qtile_off[t->B];
-  const size_t b_acc = up1k((size_t)t->T * a.Hq * 128 * 4), b_aux = up1k((size_t)a.Hq * nqt * 128 * 4);
+  const size_t b_acc = up1k((size_t)a.Hq * nqt * 65536), b_aux = up1k((size_t)a.Hq * nqt * 128 * 4);
   char* ws = (char*)(((uintptr_t)a.workspace + 1023) & ~(uintptr_t)1023);
   float* dQacc = (float*)ws;
   float* auxL = (float*)(ws + b_acc);
@@ -443,9 +503,8 @@ int tc_attn_bwd(const AttnArgs& a) {
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale, a.scale * kLog2e};
   const unsigned grid = (unsigned)(t->bwd_items.size() * a.Hkv);
   tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm);
-  const int64_t n4 = n_rows * 32;
-  dq_convert_kernel<<<(unsigned)std::min<int64_t>((n4 + 255) / 256, 148 * 16), 256, 0, a.stream>>>(
-      dQacc, (__nv_bfloat16*)a.dQ, a.scale, n4);
+  dq_convert_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
+      dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc bwd launch");
 }
