@@ -32,6 +32,21 @@ using namespace sm100;
 
 constexpr float kLog2e = 1.4426950408889634f;
 
+#ifdef CAS_TRACE
+// developer timeline: clock64 at the hand-offs of one CTA (role, iteration, event)
+__device__ long long cas_trace_buf[4 * 32 * 8];
+__device__ long long cas_cta_trace[8192 * 6];   // smid, t_start, t_loop0, t_loop1, t_end, n (globaltimer ns)
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define CTA_TRACE(slot, val) do { if (blockIdx.x < 8192) cas_cta_trace[blockIdx.x * 6 + (slot)] = (val); } while (0)
+#define TRACE(role, i, ev)                                                                   \
+  do {                                                                                       \
+    if (blockIdx.x == 777 && (i) < 32) cas_trace_buf[((role) * 32 + (i)) * 8 + (ev)] = clock64(); \
+  } while (0)
+#else
+#define TRACE(role, i, ev) do {} while (0)
+#define CTA_TRACE(slot, val) do {} while (0)
+#endif
+
 // delta[t,h] = sum_d dO*O (B1), stored head-major and padded per sequence to whole 128-row tiles
 // (so each (head, Q tile) is one aligned 512-byte run): auxD[h][tile*128 + r]; auxL = LSE*log2(e).
 __global__ void __launch_bounds__(256)
@@ -172,6 +187,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   if (it.kind == 1 && !prm.has_self) return;     // prefix-only call: no self tiles (block-uniform)
 
   if (threadIdx.x == 0) {
+#ifdef CAS_TRACE
+    { unsigned sm; asm volatile("mov.u32 %0, %smid;" : "=r"(sm)); CTA_TRACE(0, sm); CTA_TRACE(1, gtime()); }
+#endif
     if (sbase & 1023u) __trap();
     for (int i = 0; i < C_N; ++i)
       mbar_init(bar(i), (i == C_PF || i == C_DSF) ? 256 : (i == C_DQD ? 128 : 1));
@@ -204,11 +222,13 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int st = i & 1;
         const uint32_t eph = ((i >> 1) & 1) ^ 1;
         mbar_wait(bar(C_QE + st), eph);
+        TRACE(3, i, 0);
         mbar_expect_tx(bar(C_QF + st), kT + 512);
         tma_load_3d(sbase + oQ + st * kT, &tmQ, bar(C_QF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oQ + st * kT + kH, &tmQ, bar(C_QF + st), 64, w.h, w.tok());
         bulk_load(sbase + oAuxL + st * 512, prm.auxL + w.aux(), 512, bar(C_QF + st));
         mbar_wait(bar(C_DOE + st), eph);
+        TRACE(3, i, 1);
         mbar_expect_tx(bar(C_DOF + st), kT + 512);
         tma_load_3d(sbase + oDO + st * kT, &tmdO, bar(C_DOF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oDO + st * kT + kH, &tmdO, bar(C_DOF + st), 64, w.h, w.tok());
@@ -240,10 +260,14 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_fence_after();
       mma_dP(0);
       mma_commit(bar(C_DPF));
+#ifdef CAS_TRACE
+      CTA_TRACE(2, gtime()); CTA_TRACE(5, n);
+#endif
       for (int i = 0; i < n; ++i) {
         const int st = i & 1, st1 = st ^ 1;
         const uint32_t ph1 = ((i + 1) >> 1) & 1;
         mbar_wait(bar(C_PF), i & 1);
+        TRACE(0, i, 0);
         tc_fence_after();
         // dV += P^T dO ; P^T (bf16) of query columns [0,64) sits at tS+[0,32), of [64,128) at tS+64+[0,32)
 #pragma unroll
@@ -256,7 +280,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           mma_S(st1);
           mma_commit(bar(C_SF));
         }
+        TRACE(0, i, 1);
         mbar_wait(bar(C_DSF), i & 1);
+        TRACE(0, i, 2);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)     // dQ = dS K
@@ -266,19 +292,25 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         for (int kk = 0; kk < 8; ++kk)     // dK += dS^T Q
           mma_ss(tdK, kmaj(sbase + oDS, kk), mnmaj(sbase + oQ + st * kT, kk), id_kmn, (i > 0 || kk > 0) ? 1u : 0u);
         mma_commit(bar(C_QE + st));
+        TRACE(0, i, 3);
         if (i + 1 < n) {
           mbar_wait(bar(C_DOF + st1), ph1);
+          TRACE(0, i, 4);
           mbar_wait(bar(C_DQD), i & 1);
+          TRACE(0, i, 5);
           tc_fence_after();
           mma_dP(st1);
           mma_commit(bar(C_DPF));
         }
       }
       mma_commit(bar(C_DONE));
+#ifdef CAS_TRACE
+      CTA_TRACE(3, gtime());
+#endif
     }
   } else if (warp < 8) {
     // =================================================================== compute: P^T, dS^T
-    setmaxnreg_inc<168>();
+    setmaxnreg_inc<144>();
     const int wg = warp >> 2;                        // query-column half owned by this warpgroup
     const int k = threadIdx.x & 127;                 // key lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
@@ -299,21 +331,23 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const float4* aL = reinterpret_cast<const float4*>(smem + oAuxL + st * 512 + wg * 256);
       const float4* aD = reinterpret_cast<const float4*>(smem + oAuxD + st * 512 + wg * 256);
       mbar_wait(bar(C_QF + st), ph);
+      if (threadIdx.x == 0) TRACE(1, i, 0);
       mbar_wait(bar(C_SF), i & 1);
+      if (threadIdx.x == 0) TRACE(1, i, 1);
       tc_fence_after();
       float p[64];
-      {
-        uint32_t s[64];
-        tmem_ld32(tSw, s);
-        tmem_ld32(tSw + 32, s + 32);
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        uint32_t s[32];
+        tmem_ld32(tSw + c * 32, s);
         tc_wait_ld();
 #pragma unroll
-        for (int q4 = 0; q4 < 16; ++q4) {
-          const float4 L = aL[q4];
-          p[4 * q4 + 0] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 0]), prm.scale_log2, -L.x));
-          p[4 * q4 + 1] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 1]), prm.scale_log2, -L.y));
-          p[4 * q4 + 2] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 2]), prm.scale_log2, -L.z));
-          p[4 * q4 + 3] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 3]), prm.scale_log2, -L.w));
+        for (int q4 = 0; q4 < 8; ++q4) {
+          const float4 L = aL[c * 8 + q4];
+          p[c * 32 + 4 * q4 + 0] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 0]), prm.scale_log2, -L.x));
+          p[c * 32 + 4 * q4 + 1] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 1]), prm.scale_log2, -L.y));
+          p[c * 32 + 4 * q4 + 2] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 2]), prm.scale_log2, -L.z));
+          p[c * 32 + 4 * q4 + 3] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 3]), prm.scale_log2, -L.w));
         }
       }
       if (masked) {
@@ -332,8 +366,11 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_wait_st();
       tc_fence_before();
       mbar_arrive(bar(C_PF));
+      if (threadIdx.x == 0) TRACE(1, i, 2);
       mbar_wait(bar(C_DOF + st), ph);
+      if (threadIdx.x == 0) TRACE(1, i, 3);
       mbar_wait(bar(C_DPF), i & 1);
+      if (threadIdx.x == 0) TRACE(1, i, 4);
       tc_fence_after();
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
@@ -360,11 +397,12 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_fence_before();
       fence_proxy_async();
       mbar_arrive(bar(C_DSF));
+      if (threadIdx.x == 0) TRACE(1, i, 5);
       w.next();
     }
   } else {
     // =================================================================== dQ reducers (warps 8-11)
-    setmaxnreg_dec<96>();
+    setmaxnreg_inc<160>();
     const int q = threadIdx.x - 256;                 // query lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     Walk w(prm, it, g);
@@ -374,16 +412,17 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const uint32_t stage = sbase + oDO + st * kT;  // dO(i) is dead: its 32 KB stage two 16 KB quarter tiles
       float* dst = prm.dQacc + ((int64_t)w.h * (prm.aux_stride >> 7) + w.utile()) * 16384;
       mbar_wait(bar(C_DQF), i & 1);
+      if (q == 0) TRACE(2, i, 0);
       tc_fence_after();
+      uint32_t d[128];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_ld32(tdP + lane_base + c * 32, d + c * 32);
+      tc_wait_ld();
+      tc_fence_before();
+      mbar_arrive(bar(C_DQD));                       // TMEM is free for dP(i+1)
+      if (q == 0) TRACE(2, i, 1);
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        uint32_t d[32];
-        tmem_ld32(tdP + lane_base + c * 32, d);
-        tc_wait_ld();
-        if (c == 3) {
-          tc_fence_before();
-          mbar_arrive(bar(C_DQD));
-        }
         const uint32_t buf = stage + (c & 1) * kH;
         if (c >= 2) {                                // quarter c-2 must have left this buffer
           if (q == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
@@ -392,8 +431,8 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const uint32_t addr = buf + q * 128 + ((uint32_t)(j ^ (q & 7)) << 4);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(d[4 * j]), "r"(d[4 * j + 1]),
-                       "r"(d[4 * j + 2]), "r"(d[4 * j + 3]) : "memory");
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(d[c * 32 + 4 * j]),
+                       "r"(d[c * 32 + 4 * j + 1]), "r"(d[c * 32 + 4 * j + 2]), "r"(d[c * 32 + 4 * j + 3]) : "memory");
         }
         fence_proxy_async();
         asm volatile("bar.sync 1, 128;" ::: "memory");
@@ -406,12 +445,18 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       if (q == 0) {
         asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         mbar_arrive(bar(C_DOE + st));
+        TRACE(2, i, 2);
       }
       w.next();
     }
     if (q == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    asm volatile("bar.sync 2, 256;" ::: "memory");   // the dO stages may now be reused by the dK write-out
   }
   // ===================================================================== dK / dV write-out
+  // Every stage buffer is dead after the last MMA.  Thread = key row: TMEM -> registers -> its own
+  // padded row in shared memory -> ONE bulk operation per row: "+=" into the slot's fp32 gradient
+  // row (cp.reduce.async.bulk add.f32, 512 B; each row is owned by exactly one CTA, so the sum is
+  // deterministic) or, for a self tile, a 256 B bf16 bulk store into dK_self/dV_self.
   if (warp < 8) {
     const int k = threadIdx.x & 127;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
@@ -422,39 +467,55 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const float mul = isK ? prm.scale : 1.f;
     const int64_t row = ((int64_t)(it.tok + k) * prm.Hkv + g) * 128;
     const bool ok = k < it.len;
+    if (isK) asm volatile("bar.sync 2, 256;" ::: "memory");   // dK staging overlaps a dO stage: reducers must be done
+    if (it.kind == 0) {
+      const uint32_t srow = sbase + (isK ? 67584u : 0u) + k * 528;     // 528 B row pitch: conflict-free v4 stores
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      uint32_t d[32];
-      tmem_ld32(src + c * 32, d);
-      tc_wait_ld();
-      if (!ok) continue;
-      if (it.kind == 0) {
-        float* dst = (isK ? prm.gradK : prm.gradV) + row + c * 32;
+      for (int c = 0; c < 4; ++c) {
+        uint32_t d[32];
+        tmem_ld32(src + c * 32, d);
+        tc_wait_ld();
 #pragma unroll
-        for (int x = 0; x < 8; ++x) {
-          float4 a = *reinterpret_cast<float4*>(dst + 4 * x);
-          a.x += __uint_as_float(d[4 * x]) * mul;
-          a.y += __uint_as_float(d[4 * x + 1]) * mul;
-          a.z += __uint_as_float(d[4 * x + 2]) * mul;
-          a.w += __uint_as_float(d[4 * x + 3]) * mul;
-          *reinterpret_cast<float4*>(dst + 4 * x) = a;
-        }
-      } else if (prm.dKs != nullptr) {
-        __nv_bfloat16* dst = (isK ? prm.dKs : prm.dVs) + row + c * 32;
+        for (int x = 0; x < 8; ++x)
+          asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(srow + c * 128 + x * 16),
+                       "f"(__uint_as_float(d[4 * x]) * mul), "f"(__uint_as_float(d[4 * x + 1]) * mul),
+                       "f"(__uint_as_float(d[4 * x + 2]) * mul), "f"(__uint_as_float(d[4 * x + 3]) * mul) : "memory");
+      }
+      fence_proxy_async();
+      if (ok) {
+        asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+                     ::"l"((isK ? prm.gradK : prm.gradV) + row), "r"(srow), "r"(512u) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      }
+    } else if (prm.dKs != nullptr) {
+      const uint32_t srow = sbase + (isK ? 34816u : 0u) + k * 272;
 #pragma unroll
-        for (int x = 0; x < 4; ++x) {
-          uint4 u;
-          u.x = pack_bf16(__uint_as_float(d[8 * x]) * mul, __uint_as_float(d[8 * x + 1]) * mul);
-          u.y = pack_bf16(__uint_as_float(d[8 * x + 2]) * mul, __uint_as_float(d[8 * x + 3]) * mul);
-          u.z = pack_bf16(__uint_as_float(d[8 * x + 4]) * mul, __uint_as_float(d[8 * x + 5]) * mul);
-          u.w = pack_bf16(__uint_as_float(d[8 * x + 6]) * mul, __uint_as_float(d[8 * x + 7]) * mul);
-          *reinterpret_cast<uint4*>(dst + 8 * x) = u;
-        }
+      for (int c = 0; c < 4; ++c) {
+        uint32_t d[32];
+        tmem_ld32(src + c * 32, d);
+        tc_wait_ld();
+#pragma unroll
+        for (int x = 0; x < 4; ++x)
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(srow + c * 64 + x * 16),
+                       "r"(pack_bf16(__uint_as_float(d[8 * x]) * mul, __uint_as_float(d[8 * x + 1]) * mul)),
+                       "r"(pack_bf16(__uint_as_float(d[8 * x + 2]) * mul, __uint_as_float(d[8 * x + 3]) * mul)),
+                       "r"(pack_bf16(__uint_as_float(d[8 * x + 4]) * mul, __uint_as_float(d[8 * x + 5]) * mul)),
+                       "r"(pack_bf16(__uint_as_float(d[8 * x + 6]) * mul, __uint_as_float(d[8 * x + 7]) * mul)) : "memory");
+      }
+      fence_proxy_async();
+      if (ok) {
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                     ::"l"((isK ? prm.dKs : prm.dVs) + row), "r"(srow), "r"(256u) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
       }
     }
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
+#ifdef CAS_TRACE
+  if (threadIdx.x == 0) CTA_TRACE(4, gtime());
+#endif
   if (warp == 12) tmem_dealloc(tbase, 512);
 }
 
@@ -510,3 +571,12 @@ int tc_attn_bwd(const AttnArgs& a) {
 }
 
 }  // namespace cas
+
+#ifdef CAS_TRACE
+extern "C" int cas_debug_trace_read(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, cas::cas_trace_buf, sizeof(cas::cas_trace_buf));
+}
+extern "C" int cas_debug_cta_trace_read(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, cas::cas_cta_trace, sizeof(cas::cas_cta_trace));
+}
+#endif
