@@ -61,7 +61,7 @@ bool tc_supported(const cas_pool* p, const cas_slot_table*, int) {
 }
 
 // ------------------------------------------------------------------------------- kernel
-constexpr int kFwdThreads = 320;
+constexpr int kFwdThreads = 384;   // 3 warpgroups: two softmax groups + (TMA, MMA, 2 idle warps)
 constexpr uint32_t kTile = 32768, kHalf = 16384;
 constexpr uint32_t kOffQ = 0, kOffK = 2 * kTile, kOffV = 4 * kTile, kOffBar = 6 * kTile;
 constexpr uint32_t kFwdSmem = 6 * kTile + 256 + 1024;   // + barriers + alignment slack
@@ -91,7 +91,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* sptr = smem_raw + (sbase - smem_u32(smem_raw));
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sptr + kOffBar);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sptr + kOffBar + B_N * 8);
   auto bar = [&](int i) { return sbase + kOffBar + 8u * i; };
 
@@ -120,6 +119,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
 
+  if (warp >= 8) {
+  asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
   if (warp == 8) {
     // ===================================================================== TMA producer
     if (lane == 0) {
@@ -211,8 +212,10 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       }
       mma_commit(bar(B_OD));
     }
+  }
   } else {
     // ===================================================================== softmax + epilogue
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
     const int t = warp >> 2;
     if (t < nq) {
       const int r = threadIdx.x - 128 * t;
@@ -237,23 +240,18 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         tmem_ld32(tS + 64, s + 64);
         tmem_ld32(tS + 96, s + 96);
         tc_wait_ld();
-        float mx = -INFINITY;
-        if (__all_sync(0xffffffffu, limit >= 128)) {
+        if (!__all_sync(0xffffffffu, limit >= 128)) {
 #pragma unroll
-          for (int c = 0; c < 128; ++c) {
-            const float v = __uint_as_float(s[c]) * prm.scale_log2;
-            s[c] = __float_as_uint(v);
-            mx = fmaxf(mx, v);
-          }
-        } else {
-#pragma unroll
-          for (int c = 0; c < 128; ++c) {
-            const float v = c < limit ? __uint_as_float(s[c]) * prm.scale_log2 : -INFINITY;
-            s[c] = __float_as_uint(v);
-            mx = fmaxf(mx, v);
-          }
+          for (int c = 0; c < 128; ++c)
+            if (c >= limit) s[c] = 0xff800000u;      // -inf: masked key
         }
-        const float m_new = fmaxf(m, mx);
+        float mx0 = -INFINITY, mx1 = -INFINITY;      // max over the raw scores (scale > 0)
+#pragma unroll
+        for (int c = 0; c < 128; c += 4) {
+          mx0 = max3(mx0, __uint_as_float(s[c]), __uint_as_float(s[c + 1]));
+          mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
+        }
+        const float m_new = fmaxf(m, fmaxf(mx0, mx1) * prm.scale_log2);
         if (j == 0) {
           m = m_new;
         } else if (__any_sync(0xffffffffu, m_new > m + 8.f)) {
@@ -270,14 +268,25 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             tmem_st32(tO + c * 32, o);
           }
         }
-        float sum = 0.f;
+        // p = 2^(s*scale_log2 - m): one packed FFMA per two scores, one MUFU each, packed row sum
+        const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);
+        uint64_t sum2a = pack2(0.f, 0.f), sum2b = sum2a;
 #pragma unroll
-        for (int i = 0; i < 64; ++i) {
-          const float p0 = ex2(__uint_as_float(s[2 * i]) - m), p1 = ex2(__uint_as_float(s[2 * i + 1]) - m);
-          sum += p0 + p1;
-          s[i] = pack_bf16(p0, p1);
+        for (int i = 0; i < 64; i += 2) {
+          float a0, a1, b0, b1;
+          unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
+          unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
+          a0 = ex2(a0); a1 = ex2(a1); b0 = ex2(b0); b1 = ex2(b1);
+          sum2a = add2(sum2a, pack2(a0, a1));
+          sum2b = add2(sum2b, pack2(b0, b1));
+          s[i] = pack_bf16(a0, a1);
+          s[i + 1] = pack_bf16(b0, b1);
         }
-        l += sum;
+        {
+          float x0, x1;
+          unpack2(add2(sum2a, sum2b), x0, x1);
+          l += x0 + x1;
+        }
         tmem_st32(tS, s);
         tmem_st32(tS + 32, s + 32);
         tc_wait_st();
