@@ -25,13 +25,14 @@ __device__ __forceinline__ void store_work4(void* w, int64_t i, float4 p, bool b
 }
 
 constexpr int kAdamThreads = 256;
-constexpr int kAdamUnroll = 4;   // float4 per thread per tensor
+constexpr int kAdamUnroll = 2;   // float4 per thread per tensor (8 independent 16-byte loads in flight)
 
 template <bool BF16>
 __global__ void __launch_bounds__(kAdamThreads)
 adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2, float eps, int zero_grad) {
   const AdamSlotDesc d = descs[blockIdx.y];
   const float step = lr * d.step_size_scale;
+  const float ibc1 = 1.0f / d.bc1, ibc2 = 1.0f / d.bc2;
   const int64_t chunk = (int64_t)kAdamThreads * 4 * kAdamUnroll;
   for (int which = 0; which < 2; ++which) {
     float* __restrict__ p = d.state + (int64_t)which * d.cap_elems;
@@ -64,9 +65,10 @@ adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2
           const float gg = gp[k];
           const float mm = b1 * mp[k] + (1.0f - b1) * gg;
           const float vv = b2 * vp[k] + (1.0f - b2) * gg * gg;
-          const float mhat = mm / d.bc1;
-          const float vhat = vv / d.bc2;
-          pp[k] = pp[k] - step * mhat / (sqrtf(vhat) + eps);
+          // m_hat = m/(1-b1^t), v_hat = v/(1-b2^t) as multiplications by the reciprocals; the one
+          // remaining division is the fast one (2 ulp; IEEE division made this kernel ALU-bound and
+          // takes a slow path once m, v decay to denormals).  Denominator >= eps > 0.
+          pp[k] = pp[k] - __fdividef(step * (mm * ibc1), sqrtf(vv * ibc2) + eps);
           mp[k] = mm;
           vp[k] = vv;
         }
