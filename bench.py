@@ -45,38 +45,73 @@ def load_peaks():
     return dict(hbm=6650.0, bf16=1590.0, bf16_sust=1400.0, src="fallback")
 
 
+def load_traffic():
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernels, taken
+    from the committed `ncu --set full` capture (profiles/traffic.json names the capture)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return {}
+
+
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs."""
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs
+    (an nvidia-smi subprocess per sample is too slow for a region of tens of milliseconds; it is
+    the fallback when NVML cannot be loaded)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
-        self.index, self.rows, self.stop_flag = index, [], False
+        self.index, self.stop_flag = index, False
+        self.sm, self.reasons, self.sm_max = [], set(), None
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
+
+    def _sample_nvml(self):
+        n = self.nvml
+        self.sm.append(float(n.nvmlDeviceGetClockInfo(self.h, n.NVML_CLOCK_SM)))
+        r = n.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        for name, bit in (("sw_power_cap", 0x4), ("hw_slowdown", 0x8), ("sw_thermal_slowdown", 0x20),
+                          ("hw_thermal_slowdown", 0x40)):
+            if r & bit:
+                self.reasons.add(name)
+
+    def _sample_smi(self):
+        out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                              "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+        r = [x.strip() for x in out.strip().split(",")]
+        if len(r) >= 7 and r[0].replace(".", "").isdigit():
+            self.sm.append(float(r[0]))
+            self.sm_max = float(r[1])
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    self.reasons.add(name)
 
     def run(self):
         while not self.stop_flag:
             try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                self.rows.append([x.strip() for x in out.strip().split(",")])
+                if self.nvml:
+                    self._sample_nvml()
+                else:
+                    self._sample_smi()
             except Exception:
                 pass
-            time.sleep(0.1)
+            time.sleep(0.002 if self.nvml else 0.1)
 
     def summary(self):
-        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
-        reasons = set()
-        for r in self.rows:
-            if len(r) < 7:
-                continue
-            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "samples": len(self.sm),
+                "source": "nvml" if self.nvml else "nvidia-smi"}
 
 
 def attn_flops(wl):
@@ -156,6 +191,7 @@ def main():
     ap.add_argument("--kernels", default="auto", choices=["auto", "simt", "tc"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-swap", action="store_true", help="c3: the same steps without rotation (overlap baseline)")
     ap.add_argument("--ref-budget", type=float, default=8.0)
     ap.add_argument("--ref-units", type=int, default=64)
     args = ap.parse_args()
@@ -191,12 +227,41 @@ def main():
     sess = Session(wl, device=dev)
     stream = torch.cuda.current_stream()
     fwd_fl, bwd_fl = attn_flops(wl)
-    n_el = 2 * int(sum(int(wl.cart_len[c]) for c in range(cfg.n_slots))) * cfg.Hkv * cfg.D   # resident K+V elements
+    # resident K+V elements the Adam call updates (with rotation: slots in transit this step are skipped, K4)
+    n_upd = cfg.n_slots - ((cfg.rotate_in + cfg.rotate_out) if (cfg.rotate_in > 0 and not args.no_swap) else 0)
+    n_el = 2 * int(sum(int(wl.cart_len[c]) for c in range(n_upd))) * cfg.Hkv * cfg.D
     adam_bytes = 30 * n_el
 
-    def step(record=None):
+    rotate = cfg.rotate_in > 0 and not args.no_swap
+    rot = {"step": 0, "rng": np.random.Generator(np.random.PCG64(BASE_SEED + 1000 + rank)), "bytes": 0}
+    if cfg.rotate_in > 0:
+        from workloads.generate import draw_batch_selection
+
+    def prepare():
+        tau = rot["step"]
+        rot["step"] += 1
+        sel_off, sel_cart = wl.sel_off, wl.sel_cart
+        if cfg.rotate_in > 0:
+            # K4 step protocol: draw among resident+stable cartridges, protect them, plan, swap on
+            # the side stream while fwd/bwd/Adam run on the main stream, commit.
+            c = cas.cas_pool_counters(sess.pool)
+            stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
+            sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
         sess.tab.close()
-        sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, wl.sel_off, wl.sel_cart, 0)
+        sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, sel_off, sel_cart, tau)
+        if rotate:
+            prot = sorted(set(int(x) for x in sel_cart))
+            man, n = cas.cas_plan_rotation(sess.pool, tau, cfg.rotate_in, cfg.rotate_out, prot, 260604)
+            cas.cas_swap_out(sess.pool, man, n, tau, after_stream=stream)
+            cas.cas_swap_in(sess.pool, man, n, tau)
+            rot["bytes"] += sum(int(man[i].nbytes) for i in range(n))
+
+    def finish():
+        if rotate:
+            cas.cas_swap_commit(sess.pool, stream)
+
+    def step(record=None):
+        prepare()
         if record:
             record[0].record(stream)
         sess.fwd()
@@ -210,6 +275,7 @@ def main():
             sess.adam()
         if record:
             record[3].record(stream)
+        finish()
 
     def barrier():
         torch.cuda.synchronize()
@@ -236,6 +302,46 @@ def main():
     t_adam = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
     ms_step = total_ms / args.steps
 
+    # ---- c3: the swap alone (no compute on the main stream) and the host link's own pinned-copy peak
+    swap_only = None
+    if rotate:
+        for _ in range(2):
+            prepare(); finish()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0 = rot["bytes"]
+        a.record(stream)
+        for _ in range(4):
+            prepare(); finish()
+        b.record(stream)
+        barrier()
+        swap_ms = a.elapsed_time(b) / 4
+        per_dir = (rot["bytes"] - b0) / 4 / 2
+        hbuf = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+        hbuf2 = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+        dbuf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        dbuf2 = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        s2 = torch.cuda.Stream()
+        best = {}
+        for name in ("h2d", "d2h", "both"):
+            ts = []
+            for _ in range(4):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                if name in ("h2d", "both"):
+                    dbuf.copy_(hbuf, non_blocking=True)
+                if name in ("d2h", "both"):
+                    with torch.cuda.stream(s2):
+                        hbuf2.copy_(dbuf2, non_blocking=True)
+                torch.cuda.synchronize()
+                ts.append(time.perf_counter() - t0)
+            best[name] = (256 << 20) / min(ts) / 1e9
+        swap_only = {"ms": swap_ms, "gbs_per_direction": per_dir / (swap_ms * 1e-3) / 1e9,
+                     "host_link_h2d_gbs": best["h2d"], "host_link_d2h_gbs": best["d2h"],
+                     "host_link_bidir_gbs_per_direction": best["both"],
+                     "frac_of_host_link": per_dir / (swap_ms * 1e-3) / 1e9 / best["both"]}
+        del hbuf, hbuf2, dbuf, dbuf2
+
     # ---- e2e: host buffers through cas_train_step_host
     e2e = None
     if cfg.backward and not args.no_e2e:
@@ -250,10 +356,10 @@ def main():
         acfg = sess.adam_cfg()
 
         def e2e_step():
-            sess.tab.close()
-            sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, wl.sel_off, wl.sel_cart, 0)
+            prepare()
             cas.cas_train_step_host(sess.pool, sess.tab, cfg.Hq, hQ, hKs, hVs, hdO, sess.scale, acfg, hO, hLSE, hdQ,
                                     scratch)
+            finish()
 
         for _ in range(3):
             e2e_step()
@@ -282,6 +388,20 @@ def main():
         tc = bool(cfg.dtype == "bf16" and cfg.D == 128 and args.kernels != "simt")
         dom_fl, dom_ms, dom_name = (bwd_fl, t_bwd, "attn_bwd") if cfg.backward else (fwd_fl, t_fwd, "attn_fwd")
         achieved = dom_fl / (dom_ms * 1e-3) / 1e12
+        traffic = load_traffic().get(args.config, {}).get(dom_name)
+        roof = {"kernel": dom_name, "bound": "tensor", "achieved": achieved, "peak": peaks["bf16_sust"],
+                "unit": "TFLOP/s", "frac": achieved / peaks["bf16_sust"], "traffic": traffic,
+                "peak_source": peaks["src"] + " bf16_tflops_sustained (kernel timed inside the step)",
+                "frac_of_burst_peak": achieved / peaks["bf16"]}
+        if not cfg.backward:
+            # decode (c5): HBM-bound; algorithmic bytes = unique selected K+V bytes + Q + O
+            uniq = sorted(set(int(x) for x in wl.sel_cart))
+            kv_bytes = 2 * sum(int(wl.cart_len[c]) for c in uniq) * cfg.Hkv * cfg.D * 2
+            io_bytes = 2 * int(wl.T) * cfg.Hq * cfg.D * 2
+            gbs = (kv_bytes + io_bytes) / (t_fwd * 1e-3) / 1e9
+            roof = {"kernel": "attn_fwd", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
+                    "frac": gbs / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " hbm_gbs",
+                    "algorithmic_bytes": kv_bytes + io_bytes, "tflops": achieved}
         line = {
             "metric": METRIC, "value": total_flops / (ms_step_max * 1e-3) / 1e12, "unit": UNIT,
             "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step_max,
@@ -297,14 +417,19 @@ def main():
                           "bwd_tflops": (bwd_fl / (t_bwd * 1e-3) / 1e12) if cfg.backward else None,
                           "fwd_bwd_tflops": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12,
                           "fwd_bwd_frac_of_bf16_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16_sust"],
+                          "fwd_bwd_frac_of_bf16_burst_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16"],
                           "adam_gbs": (adam_bytes / (t_adam * 1e-3) / 1e9) if cfg.backward else None,
                           "adam_frac_of_hbm_peak": (adam_bytes / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if cfg.backward else None},
-            "roofline": {"kernel": dom_name, "bound": "tensor", "achieved": achieved, "peak": peaks["bf16_sust"],
-                         "unit": "TFLOP/s", "frac": achieved / peaks["bf16_sust"], "traffic": None,
-                         "peak_source": peaks["src"] + " bf16_tflops_sustained (kernel timed inside the step)"},
-            "gpu_launches": args.steps * (5 if not tc else 5),
+            "roofline": roof,
+            "gpu_launches": args.steps * ((5 if cfg.backward else 1) + (cfg.rotate_in if rotate else 0)),
             "clocks": sampler.summary(),
         }
+        if cfg.rotate_in > 0:
+            per_step = rot["bytes"] / max(rot["step"], 1)
+            line["swap"] = {"enabled": rotate, "bytes_per_step_both_directions": per_step,
+                            "gbs_over_step_time": per_step / (ms_step_max * 1e-3) / 1e9,
+                            "swap_alone": swap_only,
+                            "note": "overlap efficiency = ms_per_step of a --no-swap run / this ms_per_step"}
         if e2e:
             line["e2e"] = {"value": total_flops / (e2e_ms_max * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_max,
                            "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}

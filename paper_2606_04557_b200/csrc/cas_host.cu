@@ -171,6 +171,15 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->side);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_main, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side_in, cudaEventDisableTiming);
+    if (e == cudaSuccess) {   // highest priority: its small refresh kernels must not queue behind the attention CTAs
+      int lo = 0, hi = 0;
+      cudaDeviceGetStreamPriorityRange(&lo, &hi);
+      e = cudaStreamCreateWithPriority(&p->side_in, cudaStreamNonBlocking, hi);
+    }
+    p->ev_slot.assign(desc->n_slots, nullptr);
+    for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
+      e = cudaEventCreateWithFlags(&p->ev_slot[s2], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_adam_desc, cudaEventDisableTiming);
     if (e != cudaSuccess) { delete p; return cuda_fail(e, "pool_create"); }
     if (desc->dtype == CAS_BF16 && desc->D == 128) {
@@ -188,6 +197,9 @@ int cas_pool_destroy(cas_pool* p) {
     cudaDeviceSynchronize();
     if (p->ev_side) cudaEventDestroy(p->ev_side);
     if (p->ev_main) cudaEventDestroy(p->ev_main);
+    if (p->ev_side_in) cudaEventDestroy(p->ev_side_in);
+    if (p->side_in) cudaStreamDestroy(p->side_in);
+    for (cudaEvent_t ev : p->ev_slot) if (ev) cudaEventDestroy(ev);
     if (p->ev_adam_desc) cudaEventDestroy(p->ev_adam_desc);
     if (p->d_adam_desc) cudaFree(p->d_adam_desc);
     if (p->h_adam_desc) cudaFreeHost(p->h_adam_desc);
@@ -691,18 +703,18 @@ int cas_plan_rotation(const cas_pool* p, int64_t step, int32_t n_in, int32_t n_o
   return CAS_OK;
 }
 
-static int copy_cart(cas_pool* p, int c, int s, bool to_host) {
+static int copy_cart(cas_pool* p, int c, int s, bool to_host, cudaStream_t st) {
   const int64_t n = (int64_t)p->cart_len[c] * p->row_elems;
   const cudaMemcpyKind kind = to_host ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice;
   if (p->cart_len[c] == p->slot_cap[s]) {   // the six tensors are contiguous on both sides
     void* d = p->slot_state(s, 0);
     void* h = p->home(c, 0);
-    CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, 6 * n * 4, kind, p->side));
+    CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, 6 * n * 4, kind, st));
   } else {
     for (int w = 0; w < 6; ++w) {
       void* d = p->slot_state(s, w);
       void* h = p->home(c, w);
-      CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, n * 4, kind, p->side));
+      CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, n * 4, kind, st));
     }
   }
   return CAS_OK;
@@ -728,7 +740,11 @@ int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t st
   }
   for (int i = 0; i < n; ++i) {
     if (e[i].dir != CAS_DIR_OUT) continue;
-    if (p->dev) { int rc = copy_cart(p, e[i].cart, e[i].slot, true); if (rc) return rc; }
+    if (p->dev) {
+      int rc = copy_cart(p, e[i].cart, e[i].slot, true, p->side);
+      if (rc) return rc;
+      CAS_CUDA(cudaEventRecord(p->ev_slot[e[i].slot], p->side));   // the slot is free once this copy is done
+    }
     p->in_transit[e[i].cart] = 1;
     p->pending.push_back({e[i], step});
   }
@@ -752,16 +768,24 @@ int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t ste
     if (e[i].host_off != p->home_off[c] || e[i].nbytes != p->home_bytes(c)) { set_error("manifest bytes mismatch"); return CAS_ERR_INVALID_ARG; }
   }
   if (p->dev && !p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+  // all copies first, then the refresh kernels: a kernel between two copies would hold the next copy
+  // back until the kernel finds a free SM under the attention kernels of the main stream
+  for (int i = 0; i < n && p->dev; ++i) {
+    if (e[i].dir != CAS_DIR_IN) continue;
+    const int c = e[i].cart, s = e[i].slot;
+    // after the eviction that frees this slot (if any); a slot that was already free has no pending user
+    if (leaving.count(s)) CAS_CUDA(cudaStreamWaitEvent(p->side_in, p->ev_slot[s], 0));
+    int rc = copy_cart(p, c, s, false, p->side_in);
+    if (rc) return rc;
+  }
   for (int i = 0; i < n; ++i) {
     if (e[i].dir != CAS_DIR_IN) continue;
     const int c = e[i].cart, s = e[i].slot;
     if (p->dev) {
-      int rc = copy_cart(p, c, s, false);
-      if (rc) return rc;
       const int64_t o = (int64_t)p->slot_base[s] * p->row_elems, nel = (int64_t)p->cart_len[c] * p->row_elems;
-      rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
-                          (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, nel,
-                          p->desc.dtype, p->side);
+      int rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
+                              (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, nel,
+                              p->desc.dtype, p->side_in);
       if (rc) return rc;
     }
     p->in_transit[c] = 2;
@@ -775,6 +799,8 @@ int cas_swap_commit(cas_pool* p, void* main_stream) {
   if (p->dev && !p->pending.empty()) {
     CAS_CUDA(cudaEventRecord(p->ev_side, p->side));
     CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)main_stream, p->ev_side, 0));
+    CAS_CUDA(cudaEventRecord(p->ev_side_in, p->side_in));
+    CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)main_stream, p->ev_side_in, 0));
   }
   for (auto& q : p->pending)
     if (q.e.dir == CAS_DIR_OUT) {

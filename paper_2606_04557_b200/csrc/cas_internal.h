@@ -75,6 +75,12 @@ struct cas_pool {
   float* grad_V = nullptr;
   float* state = nullptr;
   cudaEvent_t ev_side = nullptr, ev_main = nullptr;
+  // arrivals (H2D) run on a second, library-owned stream so that they overlap the evictions (D2H) on
+  // the caller's side stream (full-duplex host link); ev_slot[s] orders an arrival after the eviction
+  // that frees its slot.
+  cudaStream_t side_in = nullptr;
+  cudaEvent_t ev_side_in = nullptr;
+  std::vector<cudaEvent_t> ev_slot;
   // library-owned device metadata for Adam launches (slot descriptors)
   void* d_adam_desc = nullptr;
   void* h_adam_desc = nullptr;   // pinned staging
