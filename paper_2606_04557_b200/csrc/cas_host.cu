@@ -455,7 +455,9 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
 
 int cas_slot_table_destroy(cas_slot_table* t) {
   if (!t) return CAS_OK;
-  if (t->d_blob) { cudaDeviceSynchronize(); cudaFree(t->d_blob); }
+  if (t->d_blob || t->d_dec_blob) cudaDeviceSynchronize();
+  if (t->d_blob) cudaFree(t->d_blob);
+  if (t->d_dec_blob) cudaFree(t->d_dec_blob);
   delete t;
   return CAS_OK;
 }
@@ -530,6 +532,7 @@ int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   a.stream = (cudaStream_t)stream;
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
+  if (tc && tc_decode_supported(p, t, Hq)) return tc_decode_fwd(a);
   return tc ? tc_attn_fwd(a) : simt_attn_fwd(a);
 }
 

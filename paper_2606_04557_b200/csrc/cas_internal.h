@@ -51,6 +51,17 @@ struct FwdItem {
   int32_t cost;
 };
 
+// Decode work item (cas_tc_decode.cu): one row block (<= 128/G sequences with the same selection
+// group) x one chunk of that group's KV tiles.
+struct DecItem {
+  int32_t seq_off;   // into dec_seqs
+  int32_t n_seqs;
+  int32_t tile_off;  // into dec_tiles
+  int32_t n_tiles;
+  int32_t row_off;   // first partial row of this item, in units of sequences (x G rows per sequence)
+  int32_t pad[3];
+};
+
 }  // namespace cas
 
 struct cas_pool {
@@ -122,6 +133,15 @@ struct cas_slot_table {
   cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
   cas::BwdItem* d_bwd_items = nullptr;
   int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
+  // decode-shaped batches: split-KV work items, built lazily for a given Hq by cas_tc_decode.cu
+  int32_t dec_Hq = 0;
+  int64_t dec_rows = 0;                       // partial rows per KV head = dec_seq_rows * G
+  std::vector<cas::DecItem> dec_items;
+  char* d_dec_blob = nullptr;
+  cas::DecItem* d_dec_items = nullptr;
+  int32_t *d_dec_seqs = nullptr, *d_comb_off = nullptr, *d_comb_row = nullptr;
+  cas::KvTile* d_dec_tiles = nullptr;
+  float* d_dec_part = nullptr;
 };
 
 namespace cas {
@@ -150,6 +170,8 @@ int tc_attn_fwd(const AttnArgs& a);
 int tc_attn_bwd(const AttnArgs& a);
 size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D);
 int tc_make_pool_maps(cas_pool* p);
+bool tc_decode_supported(const cas_pool* p, const cas_slot_table* t, int Hq);
+int tc_decode_fwd(const AttnArgs& a);
 
 // Adam / refresh / zero
 struct AdamSlotDesc {

@@ -105,6 +105,11 @@ def test_small_decode_shape(impl):
     check_attention(wl, impl, kv_heads=[0, 3, 7]).close()
     cfg = CONFIGS["c5_all"].scaled(name="c5_small_all", n_carts=6, n_slots=6, cart_len=130, B=3)
     check_attention(make_workload(cfg, 23), impl, kv_heads=[1]).close()
+    # more sequences than one 128-row block (128/G = 32 sequences), several KV chunks per group (split-KV
+    # partials + combine), a ragged last tile, and the prefix-only call (no self key)
+    cfg = CONFIGS["c5_all"].scaled(name="c5_small_rows", n_carts=5, n_slots=5, cart_len=300, B=40)
+    check_attention(make_workload(cfg, 24), impl, kv_heads=[0, 6]).close()
+    check_attention(make_workload(cfg, 25), impl, kv_heads=[2], self_block=False).close()
 
 
 # ------------------------------------------------------------------ full-size configs, one KV head
