@@ -342,15 +342,22 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
     const std::vector<KvTile>& tl = gtiles[gi++];
     const int nt = (int)tl.size();
     const int nchunk = (int)((nt + C - 1) / C);
+    // chunk-major: the row blocks that share a chunk of tiles get adjacent block indices, so they run in the
+    // same wave and the second read of a K/V tile hits L2 instead of HBM
+    std::vector<int> seq_offs;
     for (size_t r0 = 0; r0 < kv.first.size(); r0 += R) {
       const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
-      const int so = (int)seqs.size();
+      seq_offs.push_back((int)seqs.size());
       seqs.insert(seqs.end(), kv.first.begin() + r0, kv.first.begin() + r0 + ns);
-      for (int c = 0; c < nchunk; ++c) {
-        const int a = (int)((int64_t)nt * c / nchunk), b = (int)((int64_t)nt * (c + 1) / nchunk);
-        const int to = (int)tiles.size();
-        tiles.insert(tiles.end(), tl.begin() + a, tl.begin() + b);
-        items.push_back({so, ns, to, b - a, row_off, {0, 0, 0}});
+    }
+    for (int c = 0; c < nchunk; ++c) {
+      const int a = (int)((int64_t)nt * c / nchunk), b = (int)((int64_t)nt * (c + 1) / nchunk);
+      const int to = (int)tiles.size();
+      tiles.insert(tiles.end(), tl.begin() + a, tl.begin() + b);
+      for (size_t rb = 0; rb < seq_offs.size(); ++rb) {
+        const size_t r0 = rb * R;
+        const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
+        items.push_back({seq_offs[rb], ns, to, b - a, row_off, {0, 0, 0}});
         for (int j = 0; j < ns; ++j) comb[kv.first[r0 + j]].push_back(row_off + j);
         row_off += ns;
       }
