@@ -177,6 +177,9 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
       cudaDeviceGetStreamPriorityRange(&lo, &hi);
       e = cudaStreamCreateWithPriority(&p->side_in, cudaStreamNonBlocking, hi);
     }
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking);
+    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
     p->ev_slot.assign(desc->n_slots, nullptr);
     for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
       e = cudaEventCreateWithFlags(&p->ev_slot[s2], cudaEventDisableTiming);
@@ -199,6 +202,9 @@ int cas_pool_destroy(cas_pool* p) {
     if (p->ev_main) cudaEventDestroy(p->ev_main);
     if (p->ev_side_in) cudaEventDestroy(p->ev_side_in);
     if (p->side_in) cudaStreamDestroy(p->side_in);
+    if (p->st_h2d) cudaStreamDestroy(p->st_h2d);
+    if (p->st_d2h) cudaStreamDestroy(p->st_d2h);
+    for (cudaEvent_t ev : p->ev_step) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : p->ev_slot) if (ev) cudaEventDestroy(ev);
     if (p->ev_adam_desc) cudaEventDestroy(p->ev_adam_desc);
     if (p->d_adam_desc) cudaFree(p->d_adam_desc);
@@ -860,20 +866,38 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   char* d = (char*)scratch;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
-  CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, st));
-  CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, st));
-  CAS_CUDA(cudaMemcpyAsync(d + s.oVs, hVs, T * Hkv * D * eb, cudaMemcpyHostToDevice, st));
-  CAS_CUDA(cudaMemcpyAsync(d + s.odO, hdO, T * Hq * D * eb, cudaMemcpyHostToDevice, st));
+  // Inputs arrive on st_h2d (Q, K_self, V_self first: the forward pass starts as soon as they are in;
+  // dO lands under the forward pass), results leave on st_d2h (O and LSE under the backward pass, dQ
+  // under Adam).  The main stream ends by waiting for the last copy, so "main stream done" still
+  // means "everything done".
+  cudaEvent_t* ev = p->ev_step;
+  CAS_CUDA(cudaEventRecord(ev[0], st));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[0], 0));
+  CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
+  CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
+  CAS_CUDA(cudaMemcpyAsync(d + s.oVs, hVs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
+  CAS_CUDA(cudaEventRecord(ev[1], p->st_h2d));
+  CAS_CUDA(cudaMemcpyAsync(d + s.odO, hdO, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
+  CAS_CUDA(cudaEventRecord(ev[2], p->st_h2d));
+  CAS_CUDA(cudaStreamWaitEvent(st, ev[1], 0));
   rc = cas_prefix_attn_fwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, scale, d + s.oO, (float*)(d + s.oLSE), stream);
   if (rc) return rc;
+  CAS_CUDA(cudaEventRecord(ev[3], st));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[3], 0));
+  CAS_CUDA(cudaMemcpyAsync(hO, d + s.oO, T * Hq * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
+  CAS_CUDA(cudaMemcpyAsync(hLSE, d + s.oLSE, T * Hq * 4, cudaMemcpyDeviceToHost, p->st_d2h));
+  CAS_CUDA(cudaStreamWaitEvent(st, ev[2], 0));
   rc = cas_prefix_attn_bwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, d + s.oO, (float*)(d + s.oLSE), d + s.odO,
                            scale, d + s.odQ, d + s.odKs, d + s.odVs, d + s.oWs, s.ws_bytes, stream);
   if (rc) return rc;
+  CAS_CUDA(cudaEventRecord(ev[4], st));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[4], 0));
+  CAS_CUDA(cudaMemcpyAsync(hdQ, d + s.odQ, T * Hq * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
+  CAS_CUDA(cudaEventRecord(ev[5], p->st_d2h));
   rc = cas_adam_step(p, cfg, nullptr, 0, nullptr, stream);
   if (rc) return rc;
-  CAS_CUDA(cudaMemcpyAsync(hO, d + s.oO, T * Hq * D * eb, cudaMemcpyDeviceToHost, st));
-  CAS_CUDA(cudaMemcpyAsync(hLSE, d + s.oLSE, T * Hq * 4, cudaMemcpyDeviceToHost, st));
-  CAS_CUDA(cudaMemcpyAsync(hdQ, d + s.odQ, T * Hq * D * eb, cudaMemcpyDeviceToHost, st));
+  CAS_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
   return CAS_OK;
 }
 

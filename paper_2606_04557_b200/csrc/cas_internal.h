@@ -92,6 +92,9 @@ struct cas_pool {
   cudaStream_t side_in = nullptr;
   cudaEvent_t ev_side_in = nullptr;
   std::vector<cudaEvent_t> ev_slot;
+  // cas_train_step_host: input / output copies on their own streams so they overlap the kernels
+  cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
+  cudaEvent_t ev_step[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   // library-owned device metadata for Adam launches (slot descriptors)
   void* d_adam_desc = nullptr;
   void* h_adam_desc = nullptr;   // pinned staging

@@ -6,9 +6,10 @@ import pytest
 import torch
 
 from paper_2606_04557_b200 import _build, cas
+from paper_2606_04557_b200.harness import Session
 from workloads import CONFIGS, make_workload
 
-from parity_util import check_adam_isolated, check_attention
+from parity_util import check_adam_isolated, check_attention, rel_fro
 
 pytestmark = pytest.mark.gpu
 
@@ -136,3 +137,43 @@ def test_c5_full_size_decode():
         rep = {}
         check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[g], report=rep).close()
         print(name, rep)
+
+
+def test_train_step_host_matches_the_separate_calls():
+    """cas_train_step_host (pinned HOST buffers, copies overlapped on the library's copy streams) gives the
+    same O / LSE / dQ bits as fwd + bwd called one by one, leaves the same gradients consumed by the same
+    Adam step, and can be called back to back on the same scratch."""
+    cfg = CONFIGS["c2"].scaled(name="c2_host", n_carts=8, n_slots=8, cart_len=300, B=3, Lq=333, n_dist=2)
+    wl = make_workload(cfg, 41)
+    cas.cas_set_impl(cas.CAS_IMPL_AUTO)
+    ref = Session(wl)
+    ref.fwd()
+    ref.bwd()
+    ref.adam()
+    torch.cuda.synchronize()
+    sess = Session(wl)
+    tdt = sess.tdt
+    pin = lambda a: torch.from_numpy(a).to(tdt).pin_memory()
+    hQ, hKs, hVs, hdO = pin(wl.Q), pin(wl.K_self), pin(wl.V_self), pin(wl.dO)
+    hO, hdQ = torch.empty_like(hQ).pin_memory(), torch.empty_like(hQ).pin_memory()
+    hLSE = torch.empty((sess.tab.T, cfg.Hq), dtype=torch.float32).pin_memory()
+    scratch = torch.empty(cas.cas_train_step_host_scratch_bytes(sess.pool, sess.tab, cfg.Hq), dtype=torch.uint8,
+                          device="cuda")
+    cas.cas_train_step_host(sess.pool, sess.tab, cfg.Hq, hQ, hKs, hVs, hdO, sess.scale, sess.adam_cfg(), hO, hLSE,
+                            hdQ, scratch)
+    torch.cuda.synchronize()
+    assert torch.equal(hO, ref.O.cpu()) and torch.equal(hLSE, ref.LSE.cpu())
+    # dQ goes through fp32 L2 reductions whose order is not fixed: compare within bf16 rounding
+    assert rel_fro(hdQ.float().numpy(), ref.dQ.float().cpu().numpy()) < 1e-2
+    for c in sorted(set(wl.sel_cart.tolist()))[:3]:
+        for what in ("pK", "mV", "vK"):
+            a, b = sess.read(c, what), ref.read(c, what)
+            assert rel_fro(a, b) < 1e-5, (c, what)
+    O1 = hO.clone()
+    for _ in range(2):      # back to back on the same scratch; parameters moved, so O changes but stays finite
+        cas.cas_train_step_host(sess.pool, sess.tab, cfg.Hq, hQ, hKs, hVs, hdO, sess.scale, sess.adam_cfg(), hO,
+                                hLSE, hdQ, scratch)
+    torch.cuda.synchronize()
+    assert torch.isfinite(hO.float()).all() and not torch.equal(hO, O1)
+    ref.close()
+    sess.close()
