@@ -182,8 +182,11 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + oBar + C_N * 8);
   auto bar = [&](int i) { return sbase + oBar + 8u * i; };
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int g = blockIdx.x % prm.Hkv;
-  const BwdItem it = prm.items[blockIdx.x / prm.Hkv];
+  // KV-head-major block order: the CTAs in flight share one KV group, so the Q / dO / LSE / delta rows they
+  // re-read (G heads of every selecting sequence) stay in L2
+  const int n_items = gridDim.x / prm.Hkv;
+  const int g = blockIdx.x / n_items;
+  const BwdItem it = prm.items[blockIdx.x % n_items];
   if (it.kind == 1 && !prm.has_self) return;     // prefix-only call: no self tiles (block-uniform)
 
   if (threadIdx.x == 0) {
