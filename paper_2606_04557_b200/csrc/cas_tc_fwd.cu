@@ -104,7 +104,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   auto bar = [&](int i) { return sbase + kOffBar + 8u * i; };
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int item_idx = blockIdx.x / prm.Hq, h = blockIdx.x % prm.Hq, g = h / (prm.Hq / prm.Hkv);
+  // KV-group-major block order (inside a group: items longest first, the G heads of an item adjacent): the CTAs
+  // in flight work on one KV group at a time, so its K/V tiles (shared by the G heads and by every sequence that
+  // selected the cartridge) stay in L2
+  const int Gq = prm.Hq / prm.Hkv, per_group = gridDim.x / prm.Hkv;      // blocks of one KV group: items x G heads
+  const int g = blockIdx.x / per_group, rem = blockIdx.x % per_group;
+  const int item_idx = rem / Gq, h = g * Gq + rem % Gq;
   const FwdItem it = prm.items[item_idx];
   const int t0 = prm.seq_off[it.seq], lq = prm.seq_off[it.seq + 1] - t0;
   const int n_pre = prm.kv_tile_off[it.seq + 1] - prm.kv_tile_off[it.seq];
