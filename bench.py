@@ -247,8 +247,13 @@ def main():
             c = cas.cas_pool_counters(sess.pool)
             stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
             sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
-        sess.tab.close()
-        sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, sel_off, sel_cart, tau)
+        if cfg.backward or tau == 0:
+            # training: a new batch and a new slot table every step.  Decode (c5): the selection is fixed while
+            # a request generates, so the table (and its split-KV work list) is built once and reused per token.
+            t_host = time.perf_counter()
+            sess.tab.close()
+            sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, sel_off, sel_cart, tau)
+            rot["table_ms"] = (time.perf_counter() - t_host) * 1e3
         if rotate:
             prot = sorted(set(int(x) for x in sel_cart))
             man, n = cas.cas_plan_rotation(sess.pool, tau, cfg.rotate_in, cfg.rotate_out, prot, 260604)
@@ -411,6 +416,9 @@ def main():
                        "n_slots": cfg.n_slots, "B": cfg.B, "T": int(wl.T), "pairs_per_head": int(wl.pairs_per_head()),
                        "kernels": "tcgen05" if tc else "simt",
                        "l2": "inputs larger than L2 (pool + optimizer state > 1 GB per step)",
+                       "slot_table": ("rebuilt every step (inside the timed region)" if cfg.backward else
+                                      "built once before the timed region (selection fixed during generation)"),
+                       "slot_table_build_host_ms": rot.get("table_ms"),
                        "parallelism": "replicas" if world > 1 else "single"},
             "breakdown": {"fwd_ms": t_fwd, "bwd_ms": t_bwd, "adam_ms": t_adam,
                           "fwd_tflops": fwd_fl / (t_fwd * 1e-3) / 1e12,

@@ -4,6 +4,8 @@
 // Roofline: HBM.  Adam moves 30 B per element (read g,p,m,v = 16 B; write p,m,v = 12 B + bf16
 // working copy 2 B), 34 B with the fused gradient zeroing.  All accesses are 16-byte vectors,
 // fully coalesced, one (slot, chunk) per block; grid.y enumerates the slots.
+#include <algorithm>
+
 #include "cas_internal.h"
 
 namespace cas {
@@ -29,8 +31,8 @@ constexpr int kAdamUnroll = 2;   // float4 per thread per tensor (8 independent 
 
 template <bool BF16>
 __global__ void __launch_bounds__(kAdamThreads)
-adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2, float eps, int zero_grad) {
-  const AdamSlotDesc d = descs[blockIdx.y];
+adam_kernel(const __grid_constant__ AdamBatch batch, float lr, float b1, float b2, float eps, int zero_grad) {
+  const AdamSlotDesc& d = batch.d[blockIdx.y];
   const float step = lr * d.step_size_scale;
   const float ibc1 = 1.0f / d.bc1, ibc2 = 1.0f / d.bc2;
   const int64_t chunk = (int64_t)kAdamThreads * 4 * kAdamUnroll;
@@ -82,19 +84,29 @@ adam_kernel(const AdamSlotDesc* __restrict__ descs, float lr, float b1, float b2
   }
 }
 
-int launch_adam(const AdamSlotDesc* d_desc, int n, int64_t max_elems, const cas_adam_cfg& cfg, int dtype,
-                cudaStream_t st) {
-  if (n <= 0 || max_elems <= 0) return CAS_OK;
+// The slot descriptors travel as KERNEL PARAMETERS (<= 256 slots = 20 KB per launch): no descriptor
+// upload, so an Adam step never queues behind the 48 MiB swap copies on the host-to-device copy engine.
+int launch_adam(const AdamSlotDesc* h_desc, int n, const cas_adam_cfg& cfg, int dtype, cudaStream_t st) {
   const int64_t chunk = (int64_t)kAdamThreads * 4 * kAdamUnroll;
-  int64_t gx = (max_elems + chunk - 1) / chunk;
-  if (gx > 65535) gx = 65535;
-  dim3 grid((unsigned)gx, (unsigned)n);
-  if (dtype == CAS_BF16)
-    adam_kernel<true><<<grid, kAdamThreads, 0, st>>>(d_desc, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
-  else
-    adam_kernel<false><<<grid, kAdamThreads, 0, st>>>(d_desc, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return cuda_fail(e, "adam_kernel launch");
+  for (int i0 = 0; i0 < n; i0 += kAdamBatch) {
+    const int cnt = std::min(kAdamBatch, n - i0);
+    AdamBatch batch;
+    int64_t max_elems = 0;
+    for (int i = 0; i < cnt; ++i) {
+      batch.d[i] = h_desc[i0 + i];
+      max_elems = std::max(max_elems, h_desc[i0 + i].n_elems);
+    }
+    if (max_elems <= 0) continue;
+    int64_t gx = (max_elems + chunk - 1) / chunk;
+    if (gx > 65535) gx = 65535;
+    dim3 grid((unsigned)gx, (unsigned)cnt);
+    if (dtype == CAS_BF16)
+      adam_kernel<true><<<grid, kAdamThreads, 0, st>>>(batch, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
+    else
+      adam_kernel<false><<<grid, kAdamThreads, 0, st>>>(batch, cfg.lr, cfg.beta1, cfg.beta2, cfg.eps, cfg.zero_grad);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "adam_kernel launch");
+  }
   return CAS_OK;
 }
 

@@ -178,12 +178,12 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
       e = cudaStreamCreateWithPriority(&p->side_in, cudaStreamNonBlocking, hi);
     }
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_upload, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking);
     for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
     p->ev_slot.assign(desc->n_slots, nullptr);
     for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
       e = cudaEventCreateWithFlags(&p->ev_slot[s2], cudaEventDisableTiming);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_adam_desc, cudaEventDisableTiming);
     if (e != cudaSuccess) { delete p; return cuda_fail(e, "pool_create"); }
     if (desc->dtype == CAS_BF16 && desc->D == 128) {
       rc = tc_make_pool_maps(p);
@@ -203,12 +203,17 @@ int cas_pool_destroy(cas_pool* p) {
     if (p->ev_side_in) cudaEventDestroy(p->ev_side_in);
     if (p->side_in) cudaStreamDestroy(p->side_in);
     if (p->st_h2d) cudaStreamDestroy(p->st_h2d);
+    if (p->st_upload) cudaStreamDestroy(p->st_upload);
+    for (TabBlob& b : p->tab_free) {
+      if (b.d) cudaFree(b.d);
+      if (b.h) cudaFreeHost(b.h);
+      if (b.done) cudaEventDestroy(b.done);
+      if (b.ready) cudaEventDestroy(b.ready);
+    }
+    p->tab_free.clear();
     if (p->st_d2h) cudaStreamDestroy(p->st_d2h);
     for (cudaEvent_t ev : p->ev_step) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : p->ev_slot) if (ev) cudaEventDestroy(ev);
-    if (p->ev_adam_desc) cudaEventDestroy(p->ev_adam_desc);
-    if (p->d_adam_desc) cudaFree(p->d_adam_desc);
-    if (p->h_adam_desc) cudaFreeHost(p->h_adam_desc);
   }
   delete p;
   return CAS_OK;
@@ -419,8 +424,43 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
                  o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off);
     const size_t o_cnt = off;
     off += 256;
-    std::vector<char> h(off, 0);
-    auto put = [&](size_t o, const void* src, size_t n) { if (n) memcpy(h.data() + o, src, n); };
+    // a recycled blob whose last reader has finished, else a new one (device memory + pinned mirror)
+    TabBlob blob;
+    for (size_t i = 0; i < p->tab_free.size(); ++i) {
+      TabBlob& b = p->tab_free[i];
+      if (b.cap >= off && (!b.has_done || cudaEventQuery(b.done) == cudaSuccess)) {
+        blob = b;
+        p->tab_free.erase(p->tab_free.begin() + i);
+        break;
+      }
+    }
+    (void)cudaGetLastError();   // cudaEventQuery reports "not ready" as an error code
+    if (!blob.d && p->tab_free.size() >= 3) {
+      // the host runs several steps ahead of the GPU: wait for the oldest blob instead of growing the ring
+      for (size_t i = 0; i < p->tab_free.size(); ++i)
+        if (p->tab_free[i].cap >= off) {
+          blob = p->tab_free[i];
+          p->tab_free.erase(p->tab_free.begin() + i);
+          if (blob.has_done) cudaEventSynchronize(blob.done);
+          break;
+        }
+    }
+    if (!blob.d) {
+      blob.cap = std::max<size_t>(off + off / 2, 1 << 20);
+      cudaError_t e = cudaMalloc((void**)&blob.d, blob.cap);
+      if (e == cudaSuccess) e = cudaHostAlloc((void**)&blob.h, blob.cap, cudaHostAllocDefault);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&blob.done, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&blob.ready, cudaEventDisableTiming);
+      if (e != cudaSuccess) {
+        if (blob.d) cudaFree(blob.d);
+        if (blob.h) cudaFreeHost(blob.h);
+        delete t;
+        return cuda_fail(e, "slot table blob");
+      }
+    }
+    blob.has_done = false;
+    memset(blob.h + o_cnt, 0, 256);
+    auto put = [&](size_t o, const void* src, size_t n) { if (n) memcpy(blob.h + o, src, n); };
     put(o_seq, t->seq_off.data(), t->seq_off.size() * 4);
     put(o_sel, t->sel_off.data(), t->sel_off.size() * 4);
     put(o_base, t->sel_base.data(), t->sel_base.size() * 4);
@@ -435,9 +475,11 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
     put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
     put(o_qt, t->qtile_off.data(), t->qtile_off.size() * 4);
-    cudaError_t e = cudaMalloc((void**)&t->d_blob, off);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_blob, h.data(), off, cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) { if (t->d_blob) cudaFree(t->d_blob); delete t; return cuda_fail(e, "slot table upload"); }
+    cudaError_t e = cudaMemcpyAsync(blob.d, blob.h, off, cudaMemcpyHostToDevice, p->st_upload);
+    if (e == cudaSuccess) e = cudaEventRecord(blob.ready, p->st_upload);
+    if (e != cudaSuccess) { p->tab_free.push_back(blob); delete t; return cuda_fail(e, "slot table upload"); }
+    t->blob = blob;
+    t->d_blob = blob.d;
     char* d = t->d_blob;
     t->d_seq_off = (int32_t*)(d + o_seq);
     t->d_sel_off = (int32_t*)(d + o_sel);
@@ -461,8 +503,12 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
 
 int cas_slot_table_destroy(cas_slot_table* t) {
   if (!t) return CAS_OK;
-  if (t->d_blob || t->d_dec_blob) cudaDeviceSynchronize();
-  if (t->d_blob) cudaFree(t->d_blob);
+  if (t->d_blob) {   // back to the pool; reusable once the last kernel that read it is done
+    if (t->used && cudaEventRecord(t->blob.done, t->last_stream) == cudaSuccess) t->blob.has_done = true;
+    else if (t->used) cudaDeviceSynchronize();
+    t->pool->tab_free.push_back(t->blob);
+  }
+  if (t->d_dec_blob) cudaDeviceSynchronize();
   if (t->d_dec_blob) cudaFree(t->d_dec_blob);
   delete t;
   return CAS_OK;
@@ -519,6 +565,20 @@ static int check_attn(const cas_pool* p, const cas_slot_table* t, int Hq, const 
   return CAS_OK;
 }
 
+// The table's device blob is uploaded asynchronously: every stream that reads it first waits for the
+// upload, and the table remembers the stream so that the blob is recycled only after its last reader.
+static int table_on_stream(const cas_slot_table* t, void* stream) {
+  if (!t->d_blob) return CAS_OK;
+  CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)stream, t->blob.ready, 0));
+  if (t->used && t->last_stream != (cudaStream_t)stream) {   // keep one "last reader": chain the streams
+    CAS_CUDA(cudaEventRecord(t->blob.done, t->last_stream));
+    CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)stream, t->blob.done, 0));
+  }
+  t->last_stream = (cudaStream_t)stream;
+  t->used = true;
+  return CAS_OK;
+}
+
 static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) {
   *rc = CAS_OK;
   if (g_impl == CAS_IMPL_SIMT) return false;
@@ -530,6 +590,8 @@ static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) 
 int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
                         const void* Vs, float scale, void* O, float* LSE, void* stream) {
   int rc = check_attn(p, t, Hq, Ks, Vs);
+  if (rc) return rc;
+  rc = table_on_stream(t, stream);
   if (rc) return rc;
   if (!Q || !O || !LSE) { set_error("null Q/O/LSE"); return CAS_ERR_INVALID_ARG; }
   AttnArgs a{};
@@ -552,6 +614,8 @@ int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
                         const void* Vs, const void* O, const float* LSE, const void* dO, float scale,
                         void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes, void* stream) {
   int rc = check_attn(p, t, Hq, Ks, Vs);
+  if (rc) return rc;
+  rc = table_on_stream(t, stream);
   if (rc) return rc;
   if (!Q || !O || !LSE || !dO || !dQ) { set_error("null Q/O/LSE/dO/dQ"); return CAS_ERR_INVALID_ARG; }
   if ((dKs == nullptr) != (dVs == nullptr) || (dKs && !Ks)) { set_error("dK_self/dV_self: both or none, and only with K_self"); return CAS_ERR_INVALID_ARG; }
@@ -597,17 +661,7 @@ int cas_adam_step(cas_pool* p, const cas_adam_cfg* cfg, const int32_t* slots, in
   }
   const int cnt = (int)list.size();
   if (p->dev && cnt) {
-    if (cnt > p->adam_desc_cap) {
-      CAS_CUDA(cudaDeviceSynchronize());
-      if (p->d_adam_desc) cudaFree(p->d_adam_desc);
-      if (p->h_adam_desc) cudaFreeHost(p->h_adam_desc);
-      p->adam_desc_cap = std::max(cnt, p->desc.n_slots);
-      CAS_CUDA(cudaMalloc(&p->d_adam_desc, p->adam_desc_cap * sizeof(AdamSlotDesc)));
-      CAS_CUDA(cudaHostAlloc(&p->h_adam_desc, p->adam_desc_cap * sizeof(AdamSlotDesc), cudaHostAllocDefault));
-    }
-    CAS_CUDA(cudaEventSynchronize(p->ev_adam_desc));   // previous upload has left the staging buffer
-    AdamSlotDesc* h = (AdamSlotDesc*)p->h_adam_desc;
-    int64_t max_elems = 0;
+    std::vector<AdamSlotDesc> h(cnt);
     for (int i = 0; i < cnt; ++i) {
       const int s = list[i], c = p->cart_in[s];
       const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
@@ -624,12 +678,8 @@ int cas_adam_step(cas_pool* p, const cas_adam_cfg* cfg, const int32_t* slots, in
       h[i].bc1 = (float)(1.0 - pow((double)cfg->beta1, t));
       h[i].bc2 = (float)(1.0 - pow((double)cfg->beta2, t));
       h[i].pad = 0;
-      max_elems = std::max(max_elems, h[i].n_elems);
     }
-    cudaStream_t st = (cudaStream_t)stream;
-    CAS_CUDA(cudaMemcpyAsync(p->d_adam_desc, h, cnt * sizeof(AdamSlotDesc), cudaMemcpyHostToDevice, st));
-    CAS_CUDA(cudaEventRecord(p->ev_adam_desc, st));
-    int rc = launch_adam((const AdamSlotDesc*)p->d_adam_desc, cnt, max_elems, *cfg, p->desc.dtype, st);
+    int rc = launch_adam(h.data(), cnt, *cfg, p->desc.dtype, (cudaStream_t)stream);
     if (rc) return rc;
   }
   for (int s : list) {

@@ -64,6 +64,17 @@ struct DecItem {
 
 }  // namespace cas
 
+// Device blob + pinned mirror of one slot table.  Blobs are recycled through the pool (no cudaMalloc /
+// cudaFree / device-wide synchronisation per step): `done` marks the last kernel that read the blob,
+// `ready` the end of its asynchronous upload.
+struct TabBlob {
+  char* d = nullptr;
+  char* h = nullptr;
+  size_t cap = 0;
+  cudaEvent_t done = nullptr, ready = nullptr;
+  bool has_done = false;
+};
+
 struct cas_pool {
   cas_pool_desc desc;
   std::vector<int32_t> cart_len;
@@ -92,14 +103,11 @@ struct cas_pool {
   cudaStream_t side_in = nullptr;
   cudaEvent_t ev_side_in = nullptr;
   std::vector<cudaEvent_t> ev_slot;
+  std::vector<TabBlob> tab_free;     // recycled slot-table blobs
+  cudaStream_t st_upload = nullptr;  // slot-table uploads
   // cas_train_step_host: input / output copies on their own streams so they overlap the kernels
   cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
   cudaEvent_t ev_step[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-  // library-owned device metadata for Adam launches (slot descriptors)
-  void* d_adam_desc = nullptr;
-  void* h_adam_desc = nullptr;   // pinned staging
-  int adam_desc_cap = 0;
-  cudaEvent_t ev_adam_desc = nullptr;
   // TMA descriptors over the working copy (bf16, D==128 only)
   bool has_tma = false;
   CUtensorMap tm_K, tm_V;
@@ -127,8 +135,11 @@ struct cas_slot_table {
   std::vector<cas::BwdItem> bwd_items;        // longest first
   int64_t pairs = 0, prefix_tokens = 0, unique_prefix_tokens = 0;
   int32_t max_lq = 0;
-  // one device blob holding all the arrays above
+  // one device blob holding all the arrays above (recycled through the pool)
+  TabBlob blob;
   char* d_blob = nullptr;
+  mutable cudaStream_t last_stream = nullptr;   // stream of the last kernel that read the blob
+  mutable bool used = false;
   int32_t *d_seq_off = nullptr, *d_sel_off = nullptr, *d_sel_base = nullptr, *d_sel_len = nullptr,
           *d_inv_off = nullptr, *d_inv_seq = nullptr, *d_kv_tile_off = nullptr,
           *d_used_slots = nullptr, *d_sel_slot = nullptr, *d_qtile_off = nullptr;
@@ -190,8 +201,11 @@ struct AdamSlotDesc {
   float bc1, bc2;     // 1-beta1^t, 1-beta2^t
   int32_t pad;
 };
-int launch_adam(const AdamSlotDesc* d_desc, int n, int64_t max_elems, const cas_adam_cfg& cfg,
-                int dtype, cudaStream_t st);
+constexpr int kAdamBatch = 256;   // slot descriptors per launch, passed as kernel parameters (20 KB)
+struct AdamBatch {
+  AdamSlotDesc d[kAdamBatch];
+};
+int launch_adam(const AdamSlotDesc* h_desc, int n, const cas_adam_cfg& cfg, int dtype, cudaStream_t st);
 int launch_refresh(float* pK, float* pV, void* wK, void* wV, float* gK, float* gV, int64_t n,
                    int dtype, cudaStream_t st);
 int launch_zero(float* p, int64_t n, cudaStream_t st);
