@@ -7,12 +7,20 @@
  *   - plain C, no exceptions; every call returns an int: CAS_OK (0) or a negative CAS_ERR_* code;
  *     cas_last_error() returns the text of the last failure of the calling thread.
  *   - "device" pointers are CUDA device memory, "host" pointers ordinary host memory, "pinned"
- *     page-locked host memory (cudaHostAlloc).  THE CALLER OWNS every data buffer and every stream
- *     (allocate with PyTorch or cudaMalloc); the library owns only host metadata behind the opaque
- *     handles plus small device-side index tables (slot tables, tile lists, work lists) that it
- *     cudaMalloc's in cas_slot_table_build / cas_pool_create and frees in the matching destroy.
- *   - compute calls are asynchronous on the caller's stream (cudaStream_t passed as void*);
- *     swap calls are asynchronous on the side stream given at pool creation.
+ *     page-locked host memory (cudaHostAlloc).  THE CALLER OWNS every data buffer (pool arenas,
+ *     Q/K/V/O/gradients, workspaces: allocate with PyTorch or cudaMalloc) and the main and side
+ *     streams.  The library owns host metadata behind the opaque handles plus (a) device-side index
+ *     tables (slot tables, tile lists, work lists) with pinned mirrors, kept in a small ring of blobs
+ *     per pool that is recycled from table to table (cudaMalloc only while the ring warms up, freed in
+ *     cas_pool_destroy); (b) for decode-shaped tables the split-KV work list and its partial-result
+ *     scratch, allocated at the first forward call and freed with the table; (c) four internal
+ *     non-blocking streams and their events: arrivals of a swap (high priority), slot-table uploads,
+ *     and the input / output copies of cas_train_step_host.
+ *   - compute calls are asynchronous on the caller's stream (cudaStream_t passed as void*): a
+ *     stream that uses a slot table first waits (event) for the table's asynchronous upload.
+ *     Evictions run on the side stream given at pool creation, arrivals on the library's own
+ *     arrival stream (both directions of the host link are used at once).
+ *   - destroy every slot table of a pool before the pool itself.
  *   - tensors are row-major, innermost dimension last:  Q/O/dO/dQ [T, Hq, D];  K_self/V_self and
  *     their grads [T, Hkv, D];  LSE [T, Hq] fp32;  pool tensors [pool_tokens, Hkv, D].
  *     T = total packed query tokens, sequence b owns tokens seq_off[b] .. seq_off[b+1]-1.
@@ -204,22 +212,26 @@ int cas_grad_zero(cas_pool* pool, const int32_t* slots, int32_t n, void* stream)
 int cas_plan_rotation(const cas_pool* pool, int64_t step, int32_t n_in, int32_t n_out,
                       const int32_t* protect_carts, int32_t n_protect, uint64_t seed,
                       cas_manifest_entry* entries, int32_t capacity, int32_t* n_entries);
-/* Enqueue the OUT (resp. IN) entries of a manifest on the side stream, in order, one
- * cudaMemcpyAsync per contiguous piece.  An arrival is followed by a kernel (side stream) that
- * derives the working copy and zeroes the gradient slot.  swap_out first waits (event) for work
- * already enqueued on `after_stream` (the stream whose Adam last wrote the evictees; may be NULL).
+/* Enqueue the OUT entries of a manifest on the side stream (resp. the IN entries on the library's
+ * arrival stream), in order, one cudaMemcpyAsync per contiguous piece.  An arrival into a slot that
+ * an eviction of the same round frees waits (per-slot event) for that eviction only.  After all
+ * arrival copies, one kernel per arrival derives the working copy and zeroes the gradient slot.
+ * swap_out first waits (event) for work already enqueued on `after_stream` (the stream whose Adam
+ * last wrote the evictees; may be NULL).
  * CAS_ERR_BUSY: evictee has un-consumed gradients / cartridge already in transit / slot occupied. */
 int cas_swap_out(cas_pool* pool, const cas_manifest_entry* entries, int32_t n, int64_t step,
                  void* after_stream);
 int cas_swap_in(cas_pool* pool, const cas_manifest_entry* entries, int32_t n, int64_t step);
-/* Makes main_stream wait for everything enqueued on the side stream and flips residency:
+/* Makes main_stream wait for everything enqueued on the side and arrival streams and flips residency:
  * evictees leave, arrivals become selectable with last_used = the step of their swap_in. */
 int cas_swap_commit(cas_pool* pool, void* main_stream);
 
 /* ---- end-to-end convenience: one training step from HOST buffers --------------------------------
  * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
- * resident slots, D2H of O, LSE, dQ -- all on `stream`.  dev_scratch must hold
- * cas_train_step_host_scratch_bytes().  Asynchronous; synchronise the stream before reading. */
+ * resident slots, D2H of O, LSE, dQ.  Kernels run on `stream`; the copies run on two internal copy
+ * streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and dQ
+ * leaves under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
+ * cas_train_step_host_scratch_bytes().  Asynchronous; synchronise `stream` before reading. */
 int cas_train_step_host_scratch_bytes(const cas_pool* pool, const cas_slot_table* table, int32_t Hq,
                                       size_t* bytes);
 int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,
