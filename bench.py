@@ -161,6 +161,22 @@ def oracle_sample(wl, budget_s=12.0, max_units=64):
     return done_flops / t_used / 1e12, desc, t_used, threads
 
 
+def reduce_over_ranks(ms_step, e2e_ms, flops, world, device):
+    """Replica aggregation: every rank ran its own batch on its own pool, so the job's
+    time is the MAX over ranks and its work the SUM over ranks.  No data-path collective: these two
+    all-reduces only combine the measurements.  Returns (ms_step_max, e2e_ms_max, total_flops)."""
+    import torch
+
+    times = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device=device)
+    work = torch.tensor([flops], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    return float(times[0]), float(times[1]), float(work[0])
+
+
 def run_reference(args, wl):
     """The reference arm of this tier = the oracle, timed on the host cores."""
     tf, desc, secs, threads = 0.0, "", 0.0, 1
@@ -380,13 +396,8 @@ def main():
         d2h = sum(t.numel() * t.element_size() for t in (hO, hdQ, hLSE))
         e2e = (e2e_ms, h2d, d2h)
 
-    times = torch.tensor([ms_step, e2e[0] if e2e else 0.0], dtype=torch.float64, device=dev)
-    flops = torch.tensor([fwd_fl + bwd_fl], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-        dist.all_reduce(flops, op=dist.ReduceOp.SUM)
-    ms_step_max, e2e_ms_max = float(times[0]), float(times[1])
-    total_flops = float(flops[0])
+    ms_step_max, e2e_ms_max, total_flops = reduce_over_ranks(ms_step, e2e[0] if e2e else 0.0, fwd_fl + bwd_fl,
+                                                             world, dev)
 
     if rank == 0:
         peaks = load_peaks()
