@@ -192,3 +192,40 @@ def adam_step(p, m, v, g, t: int, lr: float, beta1: float, beta2: float, eps: fl
 def cartridge_bytes(n_layers: int, tokens: int, Hkv: int, D: int, bytes_per_el: int = 2) -> int:
     """Exact byte size of a cartridge Z in R^{L x p x d x 2}, d = Hkv*D."""
     return n_layers * tokens * Hkv * D * 2 * bytes_per_el
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1 (SURVEY.md 8(f)): RoPE with the cartridge position offset
+# ---------------------------------------------------------------------------------------------
+def rope(X, seq_off, pos_off, base: float, layout: int = 0, inverse: bool = False):
+    """Rotary position embedding of the packed tokens X [T, H, D] (RoFormer, Su et al. 2024, cited at
+    PAPER.md:77 and :320), with the paper's offset: "query token position IDs must be offset by the total
+    number of active cartridge KV tokens, which occupy the prefix of the sequence".
+
+    Token i of sequence b has position id m = pos_off[b] + i (R7: the caller passes either the
+    sum of resident cartridge lengths or the visible prefix P_b from cas_position_offsets).  RoFormer
+    Eq. 13/34: dimension pair k (k = 0..D/2-1) is rotated by the angle m * theta_k, theta_k = base^(-2k/D):
+        [x_a']   [cos  -sin] [x_a]
+        [x_b'] = [sin   cos] [x_b]
+    layout 0: the pair is (x[2k], x[2k+1]) (RoFormer's interleaved form); layout 1: (x[k], x[k+D/2]) (the
+    "rotate-half" storage convention of the Qwen3 checkpoints the paper trains on -- a fixed permutation of
+    the dimensions).  inverse=True rotates by -m*theta_k: the transpose, i.e. the backward pass of the map.
+    Plain float64 loops over the pairs; no tables, no fusion."""
+    X = np.asarray(X, dtype=F64)
+    T, H, D = X.shape
+    assert D % 2 == 0
+    out = np.empty_like(X)
+    B = len(seq_off) - 1
+    for b in range(B):
+        for t in range(int(seq_off[b]), int(seq_off[b + 1])):
+            m = float(int(pos_off[b]) + (t - int(seq_off[b])))
+            for k in range(D // 2):
+                ang = m * (float(base) ** (-2.0 * k / D))
+                if inverse:
+                    ang = -ang
+                c, s = np.cos(ang), np.sin(ang)
+                ia, ib = (2 * k, 2 * k + 1) if layout == 0 else (k, k + D // 2)
+                xa, xb = X[t, :, ia], X[t, :, ib]
+                out[t, :, ia] = xa * c - xb * s
+                out[t, :, ib] = xa * s + xb * c
+    return out

@@ -396,3 +396,65 @@ def test_p9_cartridge_bytes_vs_paper():
     # "x4 with gradients and Adam moments": ~551 MiB printed, exact 562.5 (2% off)
     four = 4 * orc.cartridge_bytes(36, 1000, 8, 128) / 2 ** 20
     assert abs(four - 551) / 551 < 0.03
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: RoPE with the cartridge offset (oracle.rope) -- pinned by an independent complex-number
+# formulation, the closed form at D = 2, and the properties RoFormer proves
+# ---------------------------------------------------------------------------------------------
+def _rope_inputs(seed=5, T=11, H=3, D=8):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((T, H, D)), np.array([0, 4, 11]), np.array([7, 130])
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+def test_rope_equals_complex_multiplication(layout):
+    # RoFormer Eq. 12: f(x, m) = x * e^{i m theta} on the complexified pairs -- a different formulation
+    X, so, po = _rope_inputs()
+    T, H, D = X.shape
+    base = 10000.0
+    got = orc.rope(X, so, po, base, layout)
+    k = np.arange(D // 2)
+    theta = base ** (-2.0 * k / D)
+    pos = np.concatenate([po[b] + np.arange(so[b + 1] - so[b]) for b in range(2)]).astype(np.float64)
+    z = (X[:, :, 0::2] + 1j * X[:, :, 1::2]) if layout == 0 else (X[:, :, :D // 2] + 1j * X[:, :, D // 2:])
+    w = z * np.exp(1j * pos[:, None, None] * theta[None, None, :])
+    want = np.empty_like(X)
+    if layout == 0:
+        want[:, :, 0::2], want[:, :, 1::2] = w.real, w.imag
+    else:
+        want[:, :, :D // 2], want[:, :, D // 2:] = w.real, w.imag
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-12)
+
+
+def test_rope_closed_form_d2_and_offset():
+    # D = 2: theta_0 = 1, so token i of a sequence with offset P is rotated by exactly (P + i) radians
+    X = np.array([[[1.0, 0.0]], [[0.0, 2.0]]])
+    got = orc.rope(X, np.array([0, 2]), np.array([3]), 10000.0, 0)
+    np.testing.assert_allclose(got[0, 0], [np.cos(3.0), np.sin(3.0)], atol=1e-15)
+    np.testing.assert_allclose(got[1, 0], [-2 * np.sin(4.0), 2 * np.cos(4.0)], atol=1e-15)
+
+
+@pytest.mark.parametrize("layout", [0, 1])
+def test_rope_properties(layout):
+    X, so, po = _rope_inputs(seed=6)
+    base = 1.0e6
+    Y = orc.rope(X, so, po, base, layout)
+    # rotation: norms of every (token, head) row are preserved; position 0 is the identity
+    np.testing.assert_allclose(np.linalg.norm(Y, axis=-1), np.linalg.norm(X, axis=-1), rtol=1e-13)
+    np.testing.assert_allclose(orc.rope(X[:1], np.array([0, 1]), np.array([0]), base, layout), X[:1], atol=0)
+    # inverse = transpose: undoes the map, and <rope(x), y> = <x, rope^T(y)>
+    np.testing.assert_allclose(orc.rope(Y, so, po, base, layout, inverse=True), X, atol=1e-12)
+    Z = np.random.default_rng(9).standard_normal(X.shape)
+    np.testing.assert_allclose(np.sum(Y * Z), np.sum(X * orc.rope(Z, so, po, base, layout, inverse=True)), rtol=1e-12)
+    # relative-position property (RoFormer Eq. 11): <f(q,m), f(k,n)> depends on m - n only, so shifting
+    # every offset by the same number of cartridge tokens leaves all q.k scores of a sequence unchanged
+    Y2 = orc.rope(X, so, po + 512, base, layout)
+    s1 = np.einsum("thd,uhd->htu", Y[:4], Y[:4])
+    s2 = np.einsum("thd,uhd->htu", Y2[:4], Y2[:4])
+    np.testing.assert_allclose(s1, s2, atol=1e-9)
+    # the two layouts are the same map up to the fixed permutation of dimensions
+    D = X.shape[-1]
+    perm = np.concatenate([np.arange(0, D, 2), np.arange(1, D, 2)])      # interleaved -> half-split
+    np.testing.assert_allclose(orc.rope(X, so, po, base, 0)[:, :, perm], orc.rope(X[:, :, perm], so, po, base, 1),
+                               atol=1e-12)
