@@ -169,6 +169,20 @@ int cas_slot_table_export(const cas_slot_table* table, int32_t* sel_slot, int32_
 int cas_position_offsets(const cas_pool* pool, const cas_slot_table* table,
                          int64_t* total_resident, int64_t* P);
 
+/* RoPE with that offset (RoFormer, Su et al. 2024, Eq. 34, cited at PAPER.md:77,
+ * :320).  In place on X, device [T, H, D] dtype (Q with H = Hq, or K_self with H = Hkv; apply before
+ * cas_prefix_attn_fwd -- the cartridge K in the pool are trained as they are and are not rotated).
+ * Token i of sequence b gets position id m = pos_off[b] + i (host arrays; pos_off[b] = total_resident
+ * or P[b] of cas_position_offsets, R7) and dimension pair k (k < D/2) is rotated by the angle
+ * m * base^(-2k/D):  (a, b) -> (a cos - b sin, a sin + b cos).  layout 0: pair k = dims (2k, 2k+1)
+ * (RoFormer's interleaved form); layout 1: pair k = dims (k, k + D/2) (the rotate-half storage of the
+ * Qwen3 checkpoints).  inverse = 1 rotates by the negative angle = the transposed map: apply it to dQ and
+ * dK_self to carry gradients back through the embedding.  Angles are formed in double precision.
+ * D must be a multiple of 16 bytes of dtype per pair half (bf16: D % 8 == 0 for layout 0, D % 16 == 0 for
+ * layout 1) and D <= 256, else CAS_ERR_SHAPE.  Asynchronous on `stream`. */
+int cas_rope_apply(int32_t dtype, int32_t B, const int32_t* seq_off, const int64_t* pos_off, int32_t H,
+                   int32_t D, double base, int32_t layout, int32_t inverse, void* X, void* stream);
+
 /* ---- attention ------------------------------------------------------------------------------ */
 /* Forward.  For every sequence b, query head h, row i (token t):
  *   visible keys = all tokens of the slots selected by b (read IN PLACE from the pool, no concat)

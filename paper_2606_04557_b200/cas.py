@@ -244,6 +244,15 @@ def cas_position_offsets(pool: Pool, tab: Optional[SlotTable]):
     return tot.value, P
 
 
+def cas_rope_apply(dtype: int, seq_off, pos_off, H: int, D: int, base: float, layout: int, inverse: bool, X,
+                   stream=None):
+    so = _i32(seq_off)
+    po = np.ascontiguousarray(np.asarray(pos_off, dtype=np.int64))
+    _check(lib().cas_rope_apply(C.c_int32(dtype), C.c_int32(len(so) - 1), _p(so), _p(po, C.c_int64), C.c_int32(H),
+                                C.c_int32(D), C.c_double(base), C.c_int32(layout), C.c_int32(1 if inverse else 0),
+                                _dptr(X), _stream(stream)))
+
+
 def cas_prefix_attn_fwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, scale: float, O, LSE,
                         stream=None):
     _check(lib().cas_prefix_attn_fwd(pool.handle, tab.handle, C.c_int32(Hq), _dptr(Q), _dptr(K_self),
