@@ -244,3 +244,60 @@ def position_offsets(book: PoolBook, P: Sequence[int]):
     cartridge sits in the prompt], per-sequence visible prefix lengths P_b)  -- DESIGN.md R7."""
     tot = sum(book.cart_len[c] for c in range(book.n_carts) if book.slot_of[c] >= 0)
     return tot, list(P)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3 (SURVEY.md 8(f)): Eq. 1 mixture sampler and the learning-rate schedules
+# ---------------------------------------------------------------------------------------------
+def _draw(seed: int, step: int, b: int, d: int) -> int:
+    """d-th 64-bit draw of example b at step `step`: mix64(mix64(seed, step, b), d, 0)  (R31)."""
+    return mix64(mix64(seed, step, b), d, 0)
+
+
+def sample_selection(book: PoolBook, targets: Sequence[int], p_iso: float, k_min: int, k_max: int, seed: int,
+                     step: int):
+    """PAPER.md:64-66, Eq. 1: with probability P_iso the example sees only its target cartridge Z*; otherwise
+    Z* plus S ~ U(Z_dist, k), k ~ U(k_min, k_max), Z_dist = pool \\ Z*.  Readings (R31):
+    the pool is the set of resident, stable cartridges; k's endpoints are inclusive integers; k is clamped to
+    card(Z_dist); S is drawn without replacement by a partial Fisher-Yates shuffle of Z_dist in ascending id
+    order; the target comes first, distractors in draw order.  All randomness comes from the counter-based
+    generator above: draw 0 decides isolation (top 53 bits < floor(P_iso * 2^53)), draw 1 gives k, draw 2+j
+    the j-th swap; an integer in [0, n) is ((x >> 32) * n) >> 32.  Returns (sel_off, sel_cart)."""
+    stable = book.stable_resident()
+    sel_off, sel_cart = [0], []
+    thr = int(p_iso * (1 << 53))
+    for b, tgt in enumerate(targets):
+        if book.slot_of[tgt] < 0 or book.in_transit[tgt]:
+            raise BookError("NOT_RESIDENT", f"target {tgt}")
+        sel_cart.append(tgt)
+        if (_draw(seed, step, b, 0) >> 11) >= thr:
+            cand = [c for c in stable if c != tgt]
+            k = k_min + (((_draw(seed, step, b, 1) >> 32) * (k_max - k_min + 1)) >> 32)
+            k = min(k, len(cand))
+            for j in range(k):
+                r = j + (((_draw(seed, step, b, 2 + j) >> 32) * (len(cand) - j)) >> 32)
+                cand[j], cand[r] = cand[r], cand[j]
+                sel_cart.append(cand[j])
+        sel_off.append(len(sel_cart))
+    return sel_off, sel_cart
+
+
+def lr_global(t: int, eta0: float, warmup_steps: int, warmup_min_lr: float, alpha_f: float, total_steps: int) -> float:
+    """PAPER.md:83 "slow linear decay schedule" with Table 5 (:368-372): global warmup over W steps, final LR
+    multiplier alpha_f, "Warmup minimum LR".  Reading DESIGN.md R29: eta rises linearly from warmup_min_lr at
+    t = 0 to eta0 at t = W, then falls linearly to alpha_f * eta0 at t = total_steps and stays there."""
+    if t < warmup_steps:
+        return warmup_min_lr + (eta0 - warmup_min_lr) * (t / warmup_steps)
+    if t >= total_steps:
+        return alpha_f * eta0
+    return eta0 * (1.0 - (1.0 - alpha_f) * ((t - warmup_steps) / (total_steps - warmup_steps)))
+
+
+def warmup_scale(s: int, w_c: int, n_b: int) -> float:
+    """eta_eff = eta_t * min(1, s / W_c) for a cartridge with s optimizer steps, bucketed into N_b
+    levels.  Reading SURVEY.md A12 / DESIGN.md R30: the step being taken counts (s + 1), so a fresh cartridge does
+    not get a zero learning rate, and the scale is rounded UP to the next of the N_b levels 1/N_b .. 1:
+    ceil(min(1, (s+1)/W_c) * N_b) / N_b, in exact integer arithmetic."""
+    num = min(s + 1, w_c) * n_b                      # min(1,(s+1)/W_c) * N_b = num / w_c
+    level = -(-num // w_c)                           # ceil
+    return level / n_b

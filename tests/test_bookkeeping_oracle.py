@@ -117,3 +117,72 @@ def test_rotation_properties_random():
         assert all(bk.cart_in[bk.slot_of[c]] == c for c in res)
     # least-trained-first gives near-uniform coverage ("ensuring uniform coverage")
     assert max(bk.opt_steps) - min(bk.opt_steps) <= 12
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3 pins: Eq. 1 sampler and schedules
+# ---------------------------------------------------------------------------------------------
+def _book(n=12, slots=12):
+    from oracle.bookkeeping import PoolBook
+    return PoolBook([64] * n, slots, 2, 32)
+
+
+def test_sampler_structure_and_distribution():
+    from oracle.bookkeeping import sample_selection
+    bk = _book()
+    n_ex = 6000
+    targets = [i % 12 for i in range(n_ex)]
+    so, sc = sample_selection(bk, targets, 0.75, 1, 10, 260604, 3)
+    sizes = np.diff(so)
+    iso = 0
+    kcount = np.zeros(11)
+    dist_hits = np.zeros(12)
+    for b in range(n_ex):
+        sel = sc[so[b]:so[b + 1]]
+        assert sel[0] == targets[b] and len(set(sel)) == len(sel)          # target first, a SET (Eq. 1)
+        if len(sel) == 1:
+            iso += 1
+        else:
+            kcount[len(sel) - 1] += 1
+            for c in sel[1:]:
+                dist_hits[c] += 1
+    # Eq. 1: isolation w.p. P_iso = 0.75 (binomial std 0.0056); k uniform on {1..10}; distractors uniform
+    assert abs(iso / n_ex - 0.75) < 0.02
+    mixed = n_ex - iso
+    assert kcount[0] == 0 and np.all(np.abs(kcount[1:] / mixed - 0.1) < 0.03)
+    assert np.all(np.abs(dist_hits / dist_hits.sum() - 1 / 12) < 0.01)
+    assert sizes.max() <= 11
+
+
+def test_sampler_edge_cases_and_determinism():
+    from oracle.bookkeeping import sample_selection, BookError
+    bk = _book(n=4, slots=4)
+    so, sc = sample_selection(bk, [0, 1, 2, 3] * 50, 0.0, 5, 9, 7, 0)       # k > card(Z_dist) = 3 -> clamp (A6)
+    assert all(sorted(sc[so[b]:so[b + 1]]) == [0, 1, 2, 3] for b in range(200))
+    assert sample_selection(bk, [2], 1.0, 1, 3, 7, 0) == ([0, 1], [2])        # P_iso = 1: target only
+    a = sample_selection(bk, [0, 1], 0.5, 1, 3, 11, 5)
+    assert a == sample_selection(bk, [0, 1], 0.5, 1, 3, 11, 5)                # same counters, same draw
+    bk2 = _book(n=6, slots=3)                                                 # cartridges 3..5 are not resident
+    with pytest.raises(BookError):
+        sample_selection(bk2, [4], 0.5, 1, 2, 1, 0)
+    so, sc = sample_selection(bk2, [0] * 300, 0.0, 2, 2, 1, 0)
+    assert set(sc) == {0, 1, 2}                                               # distractors only among residents
+
+
+def test_lr_schedule_table5_values():
+    from oracle.bookkeeping import lr_global, warmup_scale
+    # Table 5: eta0 = 0.1, W = 200, warmup minimum 0.002, alpha_f = 0.02; 14,200 steps (:338)
+    args = (0.1, 200, 0.002, 0.02, 14200)
+    assert lr_global(0, *args) == 0.002
+    assert abs(lr_global(100, *args) - 0.051) < 1e-15                         # halfway up the warmup
+    assert lr_global(200, *args) == 0.1
+    assert abs(lr_global(7200, *args) - 0.1 * (1 - 0.98 * 0.5)) < 1e-15       # halfway down: 0.051
+    assert abs(lr_global(14200, *args) - 0.002) < 1e-15 and lr_global(10 ** 6, *args) == lr_global(14200, *args)
+    ts = np.arange(200, 14201, 500)
+    assert np.all(np.diff([lr_global(int(t), *args) for t in ts]) < 0)        # strictly decreasing after warmup
+    # PAPER.md:85 with W_c = 20, N_b = 4: levels 1/4, 1/2, 3/4, 1; never zero; >= the unbucketed min(1,(s+1)/W_c)
+    got = [warmup_scale(s, 20, 4) for s in range(25)]
+    assert got[:5] == [0.25] * 5 and got[5:10] == [0.5] * 5 and got[10:15] == [0.75] * 5 and got[15:] == [1.0] * 10
+    assert all(warmup_scale(s, 20, 4) >= min(1.0, (s + 1) / 20) for s in range(60))
+    assert len({warmup_scale(s, 20, 4) for s in range(100)}) == 4             # "at most N_b param groups"
+    assert warmup_scale(0, 1, 4) == 1.0
