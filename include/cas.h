@@ -240,6 +240,37 @@ int cas_swap_in(cas_pool* pool, const cas_manifest_entry* entries, int32_t n, in
  * evictees leave, arrivals become selectable with last_used = the step of their swap_in. */
 int cas_swap_commit(cas_pool* pool, void* main_stream);
 
+/* ---- policy helpers (host only) ---------------------------------------- */
+/* Eq. 1 mixture sampler: example b with target cartridge targets[b] sees only its target
+ * with probability p_iso, else the target plus S ~ U(Z_dist, k), k ~ U{k_min..k_max} (inclusive), where
+ * Z_dist = the resident, stable cartridges without the target; k is clamped to card(Z_dist); S is drawn
+ * without replacement (partial Fisher-Yates over Z_dist in ascending id order).  Output in the layout
+ * cas_slot_table_build takes: sel_off[B+1], sel_cart (target first, then the distractors in draw order).
+ * Randomness is the counter-based generator of DESIGN.md R31 (seed, step, b, draw index), so a call is a
+ * pure function of its arguments and the pool's residency.  CAS_ERR_NOT_RESIDENT: a target is not resident;
+ * CAS_ERR_CAPACITY: sel_cart is too small. */
+int cas_sample_selection(const cas_pool* pool, int32_t B, const int32_t* targets, double p_iso,
+                         int32_t k_min, int32_t k_max, uint64_t seed, int64_t step, int32_t* sel_off,
+                         int32_t* sel_cart, int32_t capacity);
+
+/* Global learning rate ("slow linear decay schedule", Table 5 :366-373): linear from
+ * warmup_min_lr at t = 0 to eta0 at t = warmup_steps, then linear down to alpha_f * eta0 at total_steps,
+ * constant afterwards (R29). */
+typedef struct cas_lr_cfg {
+  double eta0;            /* peak learning rate (0.05 - 0.1) */
+  int64_t warmup_steps;   /* W = 200 */
+  double warmup_min_lr;   /* 0.002 */
+  double alpha_f;         /* final LR multiplier 0.02 */
+  int64_t total_steps;
+} cas_lr_cfg;
+int cas_lr_schedule(const cas_lr_cfg* cfg, int64_t t, double* eta);
+
+/* Per-cartridge warmup: scale[i] for the cartridge in slots[i] with s optimizer steps =
+ * ceil(min(1, (s+1)/w_c) * n_b) / n_b -- min(1, s/W_c) counted with the step being taken and rounded up to
+ * one of n_b levels (N_b = 4 in the paper; R30).  Feed the result to cas_adam_step's lr_scale. */
+int cas_warmup_scales(const cas_pool* pool, const int32_t* slots, int32_t n, int32_t w_c, int32_t n_b,
+                      float* scale);
+
 /* ---- end-to-end convenience: one training step from HOST buffers --------------------------------
  * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
  * resident slots, D2H of O, LSE, dQ.  Kernels run on `stream`; the copies run on two internal copy

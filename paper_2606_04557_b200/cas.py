@@ -313,6 +313,37 @@ def cas_swap_commit(pool: Pool, main_stream=None, host_only=False):
     _check(lib().cas_swap_commit(pool.handle, st))
 
 
+class LrCfg(C.Structure):
+    _fields_ = [("eta0", C.c_double), ("warmup_steps", C.c_int64), ("warmup_min_lr", C.c_double),
+                ("alpha_f", C.c_double), ("total_steps", C.c_int64)]
+
+
+def cas_sample_selection(pool: Pool, targets, p_iso: float, k_min: int, k_max: int, seed: int, step: int):
+    tg = _i32(targets)
+    B = len(tg)
+    cap = B * (1 + max(k_max, 0))
+    sel_off = np.empty(B + 1, np.int32)
+    sel_cart = np.empty(max(cap, 1), np.int32)
+    _check(lib().cas_sample_selection(pool.handle, C.c_int32(B), _p(tg), C.c_double(p_iso), C.c_int32(k_min),
+                                      C.c_int32(k_max), C.c_uint64(seed), C.c_int64(step), _p(sel_off),
+                                      _p(sel_cart), C.c_int32(cap)))
+    return sel_off, sel_cart[:sel_off[B]].copy()
+
+
+def cas_lr_schedule(cfg: LrCfg, t: int) -> float:
+    eta = C.c_double(0.0)
+    _check(lib().cas_lr_schedule(C.byref(cfg), C.c_int64(t), C.byref(eta)))
+    return eta.value
+
+
+def cas_warmup_scales(pool: Pool, slots, w_c: int, n_b: int) -> np.ndarray:
+    sl = _i32(slots)
+    out = np.empty(len(sl), np.float32)
+    _check(lib().cas_warmup_scales(pool.handle, _p(sl), C.c_int32(len(sl)), C.c_int32(w_c), C.c_int32(n_b),
+                                   _p(out, C.c_float)))
+    return out
+
+
 def cas_train_step_host_scratch_bytes(pool: Pool, tab: SlotTable, Hq: int) -> int:
     n = C.c_size_t(0)
     _check(lib().cas_train_step_host_scratch_bytes(pool.handle, tab.handle, C.c_int32(Hq), C.byref(n)))

@@ -164,3 +164,41 @@ def test_busy_and_data_errors():
     assert ei.value.name == "CAS_ERR_INVALID_ARG"
     with pytest.raises(cas.CasError):
         cas.Pool(cas.CAS_BF16, 2, 48, [64], 1, device=None)  # D not a multiple of 32
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: Eq. 1 sampler, LR schedule, per-cartridge warmup -- the library against the oracle, bit-exact
+# ---------------------------------------------------------------------------------------------
+def test_sampler_bit_exact_against_oracle():
+    from oracle.bookkeeping import PoolBook, sample_selection
+    cart_len = [64] * 30
+    pool = host_pool(cart_len, 20)                         # cartridges 0..19 resident
+    bk = PoolBook(cart_len, 20, 2, 32)
+    rng = np.random.default_rng(5)
+    for step, (p_iso, kmin, kmax) in enumerate([(0.75, 1, 10), (0.0, 3, 3), (1.0, 1, 5), (0.3, 0, 25), (0.5, 19, 40)]):
+        targets = rng.integers(0, 20, size=257).tolist()
+        so, sc = cas.cas_sample_selection(pool, targets, p_iso, kmin, kmax, 260604 + step, step)
+        wo, wc = sample_selection(bk, targets, p_iso, kmin, kmax, 260604 + step, step)
+        assert so.tolist() == wo and sc.tolist() == wc
+        tab = cas.cas_slot_table_build(pool, np.arange(258, dtype=np.int32), so, sc, step)   # a valid selection
+        tab.close()
+    with pytest.raises(cas.CasError) as e:
+        cas.cas_sample_selection(pool, [25], 0.5, 1, 2, 1, 0)                                # not resident
+    assert e.value.name == "CAS_ERR_NOT_RESIDENT"
+    pool.close()
+
+
+def test_lr_schedule_and_warmup_scales_against_oracle():
+    from oracle.bookkeeping import lr_global, warmup_scale
+    cfg = cas.LrCfg(0.1, 200, 0.002, 0.02, 14200)
+    for t in [0, 1, 57, 199, 200, 201, 5000, 14199, 14200, 99999]:
+        assert cas.cas_lr_schedule(cfg, t) == lr_global(t, 0.1, 200, 0.002, 0.02, 14200)
+    pool = host_pool([32] * 8, 8)
+    for c, s in enumerate([0, 1, 4, 5, 9, 14, 19, 400]):
+        cas.cas_pool_set_counters(pool, c, s, 0)
+    got = cas.cas_warmup_scales(pool, list(range(8)), 20, 4)
+    want = [warmup_scale(s, 20, 4) for s in [0, 1, 4, 5, 9, 14, 19, 400]]
+    assert got.tolist() == [np.float32(w) for w in want]
+    assert cas.cas_warmup_scales(pool, [3, 0], 7, 3).tolist() == [np.float32(warmup_scale(5, 7, 3)),
+                                                                  np.float32(warmup_scale(0, 7, 3))]
+    pool.close()
