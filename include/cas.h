@@ -284,6 +284,11 @@ int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq,
                         const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ,
                         void* dev_scratch, size_t scratch_bytes, void* stream);
 
+/* ---- hardware self-test (not on the hot path) --------------------------------------------------
+ * D[256,128] fp32 = A[256,64] * B[128,64]^T (bf16, row-major, device) computed by ONE tcgen05.mma.cta_group::2
+ * stream on a 2-CTA cluster: proves the CTA-pair primitives of csrc/cas_sm100.cuh on the GPU at hand. */
+int cas_selftest_cta_pair_mma(const void* A, const void* B, float* D, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -313,6 +313,10 @@ def cas_swap_commit(pool: Pool, main_stream=None, host_only=False):
     _check(lib().cas_swap_commit(pool.handle, st))
 
 
+def cas_selftest_cta_pair_mma(A, B, D, stream=None):
+    _check(lib().cas_selftest_cta_pair_mma(_dptr(A), _dptr(B), _dptr(D), _stream(stream)))
+
+
 class LrCfg(C.Structure):
     _fields_ = [("eta0", C.c_double), ("warmup_steps", C.c_int64), ("warmup_min_lr", C.c_double),
                 ("alpha_f", C.c_double), ("total_steps", C.c_int64)]

@@ -177,3 +177,16 @@ def test_train_step_host_matches_the_separate_calls():
     assert torch.isfinite(hO.float()).all() and not torch.equal(hO, O1)
     ref.close()
     sess.close()
+
+
+def test_cta_pair_mma_selftest():
+    """tcgen05.mma.cta_group::2 on a 2-CTA cluster (the primitives kept in cas_sm100.cuh for the next kernels):
+    exact against an integer-valued reference."""
+    g = torch.Generator().manual_seed(3)
+    A = (torch.randint(-8, 9, (256, 64), generator=g).float() / 8).to(torch.bfloat16).cuda()
+    B = (torch.randint(-6, 7, (128, 64), generator=g).float() / 4).to(torch.bfloat16).cuda()
+    D = torch.zeros((256, 128), dtype=torch.float32, device="cuda")
+    cas.cas_selftest_cta_pair_mma(A, B, D)
+    torch.cuda.synchronize()
+    want = A.double().cpu() @ B.double().cpu().T
+    assert torch.equal(D.double().cpu(), want)
