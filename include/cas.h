@@ -276,7 +276,9 @@ int cas_warmup_scales(const cas_pool* pool, const int32_t* slots, int32_t n, int
  * resident slots, D2H of O, LSE, dQ.  Kernels run on `stream`; the copies run on two internal copy
  * streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and dQ
  * leaves under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
- * cas_train_step_host_scratch_bytes().  Asynchronous; synchronise `stream` before reading. */
+ * cas_train_step_host_scratch_bytes() and belongs to the library between back-to-back calls that reuse it
+ * (the next call's input copies start as soon as the previous backward pass is done).  Asynchronous;
+ * synchronise `stream` before reading the host results or overwriting the host inputs. */
 int cas_train_step_host_scratch_bytes(const cas_pool* pool, const cas_slot_table* table, int32_t Hq,
                                       size_t* bytes);
 int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,

@@ -922,7 +922,15 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   // means "everything done".
   cudaEvent_t* ev = p->ev_step;
   CAS_CUDA(cudaEventRecord(ev[0], st));
-  CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
+  if (p->step_prev_scratch == scratch && p->step_prev_stream == st) {
+    // back-to-back steps on the same scratch: the input buffers are free as soon as the PREVIOUS backward pass
+    // is done (ev[4] still holds that record), so these copies run under the previous Adam and dQ read-back
+    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[4], 0));
+  } else {
+    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
+  }
+  p->step_prev_scratch = scratch;
+  p->step_prev_stream = st;
   CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[0], 0));
   CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
   CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));

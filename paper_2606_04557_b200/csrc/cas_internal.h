@@ -108,6 +108,8 @@ struct cas_pool {
   // cas_train_step_host: input / output copies on their own streams so they overlap the kernels
   cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
   cudaEvent_t ev_step[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* step_prev_scratch = nullptr;     // scratch / stream of the previous cas_train_step_host call
+  cudaStream_t step_prev_stream = nullptr;
   // TMA descriptors over the working copy (bf16, D==128 only)
   bool has_tma = false;
   CUtensorMap tm_K, tm_V;
