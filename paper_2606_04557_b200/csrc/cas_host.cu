@@ -391,10 +391,16 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
       const int nq = (rows + 127) / 128;
       t->fwd_items.push_back({b, r, rows, nq * npre + (r / 128) * nq + (nq == 2 ? 3 : 1)});
     }
+    for (int r = 0; r < lq; r += 512) {
+      const int rows = (int)std::min<int64_t>(512, lq - r);
+      const int nq = (rows + 127) / 128;
+      if (rows > 256) t->fwd2_items.push_back({b, r, rows, nq * npre + (r / 128) * nq});
+      else t->fwd_rest_items.push_back({b, r, rows, nq * npre + (r / 128) * nq});
+    }
     for (int r = 0; r < lq; r += 32) t->simt_items.push_back({b, r, (int)std::min<int64_t>(32, lq - r), 0});
   }
-  std::stable_sort(t->fwd_items.begin(), t->fwd_items.end(),
-                   [](const FwdItem& a, const FwdItem& b) { return a.cost > b.cost; });
+  for (auto* v : {&t->fwd_items, &t->fwd2_items, &t->fwd_rest_items})
+    std::stable_sort(v->begin(), v->end(), [](const FwdItem& a, const FwdItem& b) { return a.cost > b.cost; });
   for (int s : t->used_slots) {
     int cost = 0;
     for (int e = t->inv_off[s]; e < t->inv_off[s + 1]; ++e) {
@@ -421,7 +427,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
                  o_iseq = blob_add(off, t->inv_seq, 1), o_kto = blob_add(off, t->kv_tile_off),
                  o_kt = blob_add(off, t->kv_tiles, 1), o_fw = blob_add(off, t->fwd_items),
                  o_si = blob_add(off, t->simt_items), o_bw = blob_add(off, t->bwd_items),
-                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off);
+                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off),
+                 o_f2 = blob_add(off, t->fwd2_items, 1), o_fr = blob_add(off, t->fwd_rest_items, 1);
     const size_t o_cnt = off;
     off += 256;
     // a recycled blob whose last reader has finished, else a new one (device memory + pinned mirror)
@@ -475,6 +482,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
     put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
     put(o_qt, t->qtile_off.data(), t->qtile_off.size() * 4);
+    put(o_f2, t->fwd2_items.data(), t->fwd2_items.size() * sizeof(FwdItem));
+    put(o_fr, t->fwd_rest_items.data(), t->fwd_rest_items.size() * sizeof(FwdItem));
     cudaError_t e = cudaMemcpyAsync(blob.d, blob.h, off, cudaMemcpyHostToDevice, p->st_upload);
     if (e == cudaSuccess) e = cudaEventRecord(blob.ready, p->st_upload);
     if (e != cudaSuccess) { p->tab_free.push_back(blob); delete t; return cuda_fail(e, "slot table upload"); }
@@ -495,6 +504,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     t->d_bwd_items = (BwdItem*)(d + o_bw);
     t->d_used_slots = (int32_t*)(d + o_us);
     t->d_qtile_off = (int32_t*)(d + o_qt);
+    t->d_fwd2_items = (FwdItem*)(d + o_f2);
+    t->d_fwd_rest_items = (FwdItem*)(d + o_fr);
     t->d_counters = (int32_t*)(d + o_cnt);
   }
   *out = t;

@@ -16,6 +16,7 @@
 // rescaled when the running max grows by more than 2^8).
 #include "cas_sm100.cuh"
 #include "cas_tc_common.cuh"
+#include <cstdlib>
 
 namespace cas {
 using namespace sm100;
@@ -350,6 +351,18 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
 int tc_attn_fwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
+  // Opt-in (CAS_FWD_PAIRS=1): 512-row blocks go to the CTA-pair kernel (cas_tc_fwd2.cu), the rest to this one.
+  // Off by default: the pair kernel is parity-green but slower here (c2 0.90 vs 0.78 ms).
+  static const bool pairs = getenv("CAS_FWD_PAIRS") && getenv("CAS_FWD_PAIRS")[0] == '1';
+  const FwdItem* items = t->d_fwd_items;
+  size_t n_items = t->fwd_items.size();
+  if (pairs && !t->fwd2_items.empty()) {
+    const int rc2 = tc_attn_fwd_pairs(a, (int)t->fwd2_items.size());
+    if (rc2) return rc2;
+    items = t->d_fwd_rest_items;
+    n_items = t->fwd_rest_items.size();
+    if (n_items == 0) return CAS_OK;
+  }
   static bool attr_set = false;
   if (!attr_set) {
     CAS_CUDA(cudaFuncSetAttribute(tc_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFwdSmem));
@@ -367,9 +380,9 @@ int tc_attn_fwd(const AttnArgs& a) {
     tmKs = a.pool->tm_K;
     tmVs = a.pool->tm_V;
   }
-  FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, t->d_fwd_items, (__nv_bfloat16*)a.O_out, a.LSE_out,
+  FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale * 1.4426950408889634f};
-  const unsigned grid = (unsigned)(t->fwd_items.size() * a.Hq);
+  const unsigned grid = (unsigned)(n_items * a.Hq);
   tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc fwd launch");

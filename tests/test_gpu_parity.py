@@ -190,3 +190,28 @@ def test_cta_pair_mma_selftest():
     torch.cuda.synchronize()
     want = A.double().cpu() @ B.double().cpu().T
     assert torch.equal(D.double().cpu(), want)
+
+
+def test_forward_cta_pair_kernel_parity():
+    """The opt-in CTA-pair forward kernel (CAS_FWD_PAIRS=1, cas_tc_fwd2.cu) against the oracle: ragged lengths,
+    512-row blocks with 257..512 rows, leftover blocks on the single-CTA kernel, prefix-only call.  Runs in a
+    subprocess because the switch is read once per process."""
+    import os
+    import subprocess
+    import sys
+    code = (
+        "import sys; sys.path.insert(0, 'tests')\n"
+        "from parity_util import check_attention\n"
+        "from paper_2606_04557_b200 import cas\n"
+        "from workloads import CONFIGS, make_workload\n"
+        "cfg = CONFIGS['c4'].scaled(name='c4_pairs', n_carts=10, n_slots=10, B=5, len_mu=5.5, len_min=40, len_max=500,\n"
+        "                           lq_min=200, lq_max=1300, n_dist_max=4)\n"
+        "check_attention(make_workload(cfg, 61), cas.CAS_IMPL_AUTO, kv_heads=[1, 6], backward=False).close()\n"
+        "check_attention(make_workload(cfg, 62), cas.CAS_IMPL_AUTO, kv_heads=[3], backward=False, self_block=False).close()\n"
+        "cfg = CONFIGS['c2'].scaled(name='c2_pairs', n_carts=6, n_slots=6, cart_len=384, B=2, Lq=1024, n_dist=2)\n"
+        "check_attention(make_workload(cfg, 63), cas.CAS_IMPL_AUTO, kv_heads=[0, 7], backward=False).close()\n"
+        "print('pairs ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, CAS_FWD_PAIRS="1"),
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "pairs ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
