@@ -40,6 +40,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // generic-proxy writes to smem -> visible to the async proxy (TMA / tcgen05 operand reads)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// One lane of a converged warp (elect.sync).  Single-thread roles (MMA issuer, TMA producer) must be entered as
+//   if (warp_uniform == ROLE) { if (elect_one()) { ... } }
+// and NOT as `if (warp == ROLE && lane == 0)`: with a per-thread condition ptxas cannot prove that one thread
+// issues a tcgen05.mma / TMA instruction, keeps the descriptors in vector registers and wraps every instruction
+// in an R2UR + ELECT + BRA.U.ANY loop (~100 clk per MMA instruction -- the issuing thread, not the tensor pipe,
+// then limits the kernel).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "elect.sync _|p, 0xffffffff;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ int warp_id_uniform() { return __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0); }
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");

@@ -181,7 +181,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   const uint32_t sbase = smem_u32(smem);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + oBar + C_N * 8);
   auto bar = [&](int i) { return sbase + oBar + 8u * i; };
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_id_uniform(), lane = threadIdx.x & 31;
   // KV-head-major block order: the CTAs in flight share one KV group, so the Q / dO / LSE / delta rows they
   // re-read (G heads of every selecting sequence) stay in L2
   const int n_items = gridDim.x / prm.Hkv;
@@ -210,7 +210,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
   if (warp >= 12) {
     setmaxnreg_dec<56>();
-    if (warp == 12 && lane == 0) {
+    if (warp == 12) { if (elect_one()) {
       // ================================================================= TMA producer
       const CUtensorMap* mk = it.kind == 0 ? &tmKp : &tmKs;
       const CUtensorMap* mv = it.kind == 0 ? &tmVp : &tmVs;
@@ -238,7 +238,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         bulk_load(sbase + oAuxD + st * 512, prm.auxD + w.aux(), 512, bar(C_DOF + st));
         w.next();
       }
-    } else if (warp == 13 && lane == 0) {
+    } } else if (warp == 13) { if (elect_one()) {
       // ================================================================= MMA issuer
       constexpr uint32_t id_kk = make_idesc(128, 128, 0, 0), id_kmn = make_idesc(128, 128, 0, 1),
                          id_mnmn = make_idesc(128, 128, 1, 1);
@@ -310,7 +310,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #ifdef CAS_TRACE
       CTA_TRACE(3, gtime());
 #endif
-    }
+    } }
   } else if (warp < 8) {
     // =================================================================== compute: P^T, dS^T
     setmaxnreg_inc<144>();

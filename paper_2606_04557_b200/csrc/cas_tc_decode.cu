@@ -50,7 +50,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
   const uint32_t sbase = smem_u32(smem);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + dOffBar + D_N * 8);
   auto bar = [&](int i) { return sbase + dOffBar + 8u * i; };
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_id_uniform(), lane = threadIdx.x & 31;
   const int g = blockIdx.x % prm.Hkv, G = prm.Hq / prm.Hkv;
   const DecItem it = prm.items[blockIdx.x / prm.Hkv];
   const KvTile* tiles = prm.tiles + it.tile_off;
@@ -73,7 +73,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
 
   if (warp == 4) {
     // ===================================================================== TMA producer
-    if (lane == 0) {
+    if (elect_one()) {
       tma_prefetch_desc(&tmK);
       tma_prefetch_desc(&tmV);
       for (int j = 0; j < n; ++j) {
@@ -93,7 +93,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
     }
   } else if (warp == 5) {
     // ===================================================================== MMA issuer
-    if (lane == 0) {
+    if (elect_one()) {
       constexpr uint32_t idesc_qk = make_idesc(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc(128, 128, 0, 1);
       auto issue_qk = [&](int j) {

@@ -104,7 +104,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sptr + kOffBar + B_N * 8);
   auto bar = [&](int i) { return sbase + kOffBar + 8u * i; };
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_id_uniform(), lane = threadIdx.x & 31;
   // KV-group-major block order (inside a group: items longest first, the G heads of an item adjacent): the CTAs
   // in flight work on one KV group at a time, so its K/V tiles (shared by the G heads and by every sequence that
   // selected the cartridge) stay in L2
@@ -138,7 +138,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
   if (warp == 8) {
     // ===================================================================== TMA producer
-    if (lane == 0) {
+    if (elect_one()) {
       tma_prefetch_desc(&tmQ);
       tma_prefetch_desc(&tmKp);
       tma_prefetch_desc(&tmVp);
@@ -166,7 +166,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     }
   } else if (warp == 9) {
     // ===================================================================== MMA issuer
-    if (lane == 0) {
+    if (elect_one()) {
       constexpr uint32_t idesc_qk = make_idesc(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = make_idesc(128, 128, 0, 1);
       auto issue_qk = [&](int t, int j) {

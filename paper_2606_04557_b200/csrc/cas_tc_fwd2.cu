@@ -98,7 +98,7 @@ tc_fwd2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
   const uint32_t sbase = smem_u32(smem);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + pOffBar + P_N * 8);
   auto bar = [&](int i) { return sbase + pOffBar + 8u * i; };
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = warp_id_uniform(), lane = threadIdx.x & 31;
   const uint32_t rank = cluster_ctarank();
   // KV-group-major cluster order (as tc_fwd_kernel): cluster id -> (g, item, head of group)
   const int cid = blockIdx.x >> 1, n_clusters = gridDim.x >> 1;
@@ -129,7 +129,7 @@ tc_fwd2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
     asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     if (warp == 8) {
       // =================================================================== TMA producer (each CTA: its halves)
-      if (lane == 0) {
+      if (elect_one()) {
         tma_prefetch_desc(&tmQ);
         tma_prefetch_desc(&tmKp64);
         tma_prefetch_desc(&tmVp);
@@ -155,7 +155,7 @@ tc_fwd2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           tma_load_3d(sbase + pOffV + s * pHalf, mv, bar(P_VF + s), 64 * (int)rank, g, tok);
         }
       }
-    } else if (warp == 9 && lane == 0) {
+    } else if (warp == 9) { if (elect_one()) {
       if (rank == 0) {
         // ================================================================= MMA issuer (leader, both SMs)
         constexpr uint32_t idesc_qk = make_idesc(256, 128, 0, 0);
@@ -237,7 +237,7 @@ tc_fwd2_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ 
           }
         }
       }
-    }
+    } }
   } else {
     // ===================================================================== softmax + epilogue (as tc_fwd_kernel)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 208;");
