@@ -15,13 +15,15 @@
 //   S^T  = K  Q^T        (SS)            dP^T = V  dO^T      (SS)
 //   dV  += P^T dO        (P^T from TMEM) dK  += dS^T Q       (dS^T from SMEM, K-major)
 //   dQ   = dS  K         (the same dS^T bytes in SMEM read as an MN-major A operand)
-// TMEM (512 cols): [S^T / P^T] [dP^T / dQ] [dV] [dK].   SMEM (226 KB): K,V | 2 x Q | 2 x dO | dS^T.
+// TMEM (512 cols): [S^T / P^T] [dP^T / dQ] [dV] [dK].   SMEM (226 KB): K,V | 2 x Q | dO | dQ staging | dS^T.
+// dO needs ONE stage: its readers are dP(i) (issued at the end of iteration i-1) and dV(i) (start of iteration
+// i), so dO(i+1) can be fetched while S(i+1), dQ(i), dK(i) run.
 // Warps: 0-3 / 4-7 two compute warpgroups (thread = key; group w owns query columns [64w, 64w+64)):
 // exp -> P^T, then dS^T; 8-11 dQ reducers (thread = query); 12 TMA producer; 13 MMA issuer.
 // Issue order:  dV(i)  S(i+1)  dQ(i) dK(i)  [dQ drained]  dP(i+1)   -- the exp of tile i+1 overlaps
-// dQ/dK of tile i, the dQ drain overlaps dK.  The dQ staging buffer of iteration i is the dO stage of
-// iteration i (dead once dV(i) has been issued); that stage is handed back to the producer when the
-// bulk reductions have finished reading it.
+// dQ/dK of tile i, the dQ drain overlaps dK.  dQ is staged in its own 32 KB (two 16 KB quarter-tile buffers): the
+// bulk-reduction engine drains shared memory at only ~20 B/clk per SM (measured), so a staging buffer stays
+// busy for most of an iteration and must not be one of the pipeline stages.
 #include <cstdlib>
 
 #include "cas_sm100.cuh"
@@ -109,7 +111,7 @@ dq_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dQ,
 // ------------------------------------------------------------------------------- main kernel
 constexpr int kBwdThreads = 512;   // 4 warpgroups (setmaxnreg works on whole warpgroups); warps 14,15 idle
 constexpr uint32_t kT = 32768, kH = 16384;
-constexpr uint32_t oK = 0, oV = kT, oQ = 2 * kT, oDO = 4 * kT, oDS = 6 * kT, oAuxL = 7 * kT, oAuxD = 7 * kT + 1024,
+constexpr uint32_t oK = 0, oV = kT, oQ = 2 * kT, oDO = 4 * kT, oStg = 5 * kT, oDS = 6 * kT, oAuxL = 7 * kT, oAuxD = 7 * kT + 1024,
                    oBar = 7 * kT + 2048;
 constexpr uint32_t kBwdSmem = oBar + 256;
 enum { C_KV = 0, C_QF = 1, C_DOF = 3, C_QE = 5, C_DOE = 7, C_SF = 9, C_DPF = 10, C_PF = 11, C_DSF = 12, C_DQF = 13,
@@ -230,12 +232,12 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         tma_load_3d(sbase + oQ + st * kT, &tmQ, bar(C_QF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oQ + st * kT + kH, &tmQ, bar(C_QF + st), 64, w.h, w.tok());
         bulk_load(sbase + oAuxL + st * 512, prm.auxL + w.aux(), 512, bar(C_QF + st));
-        mbar_wait(bar(C_DOE + st), eph);
+        if (i > 0) mbar_wait(bar(C_DOE), (i - 1) & 1);   // dV(i-1) has read dO(i-1): the single dO stage is free
         TRACE(3, i, 1);
-        mbar_expect_tx(bar(C_DOF + st), kT + 512);
-        tma_load_3d(sbase + oDO + st * kT, &tmdO, bar(C_DOF + st), 0, w.h, w.tok());
-        tma_load_3d(sbase + oDO + st * kT + kH, &tmdO, bar(C_DOF + st), 64, w.h, w.tok());
-        bulk_load(sbase + oAuxD + st * 512, prm.auxD + w.aux(), 512, bar(C_DOF + st));
+        mbar_expect_tx(bar(C_DOF), kT + 512);
+        tma_load_3d(sbase + oDO, &tmdO, bar(C_DOF), 0, w.h, w.tok());
+        tma_load_3d(sbase + oDO + kH, &tmdO, bar(C_DOF), 64, w.h, w.tok());
+        bulk_load(sbase + oAuxD + st * 512, prm.auxD + w.aux(), 512, bar(C_DOF));
         w.next();
       }
     } } else if (warp == 13) { if (elect_one()) {
@@ -252,7 +254,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       };
       auto mma_dP = [&](int st) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) mma_ss(tdP, kmaj(sbase + oV, kk), kmaj(sbase + oDO + st * kT, kk), id_kk, kk > 0);
+        for (int kk = 0; kk < 8; ++kk) mma_ss(tdP, kmaj(sbase + oV, kk), kmaj(sbase + oDO, kk), id_kk, kk > 0);
       };
       mbar_wait(bar(C_KV), 0);
       mbar_wait(bar(C_QF), 0);
@@ -275,8 +277,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         // dV += P^T dO ; P^T (bf16) of query columns [0,64) sits at tS+[0,32), of [64,128) at tS+64+[0,32)
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)
-          mma_ts(tdV, tS + (kk >> 2) * 64 + (kk & 3) * 8, mnmaj(sbase + oDO + st * kT, kk), id_kmn,
+          mma_ts(tdV, tS + (kk >> 2) * 64 + (kk & 3) * 8, mnmaj(sbase + oDO, kk), id_kmn,
                  (i > 0 || kk > 0) ? 1u : 0u);
+        mma_commit(bar(C_DOE));               // dO(i) is dead: dP(i) was issued before, dV(i) is its last reader
         if (i + 1 < n) {
           mbar_wait(bar(C_QF + st1), ph1);
           tc_fence_after();
@@ -297,7 +300,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         mma_commit(bar(C_QE + st));
         TRACE(0, i, 3);
         if (i + 1 < n) {
-          mbar_wait(bar(C_DOF + st1), ph1);
+          mbar_wait(bar(C_DOF), (i + 1) & 1);
           TRACE(0, i, 4);
           mbar_wait(bar(C_DQD), i & 1);
           TRACE(0, i, 5);
@@ -370,7 +373,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_fence_before();
       mbar_arrive(bar(C_PF));
       if (threadIdx.x == 0) TRACE(1, i, 2);
-      mbar_wait(bar(C_DOF + st), ph);
+      mbar_wait(bar(C_DOF), i & 1);
       if (threadIdx.x == 0) TRACE(1, i, 3);
       mbar_wait(bar(C_DPF), i & 1);
       if (threadIdx.x == 0) TRACE(1, i, 4);
@@ -412,7 +415,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int n = w.total();
     for (int i = 0; i < n; ++i) {
       const int st = i & 1;
-      const uint32_t stage = sbase + oDO + st * kT;  // dO(i) is dead: its 32 KB stage two 16 KB quarter tiles
+      const uint32_t stage = sbase + oStg;           // dedicated staging: two 16 KB quarter-tile buffers
       float* dst = prm.dQacc + ((int64_t)w.h * (prm.aux_stride >> 7) + w.utile()) * 16384;
       mbar_wait(bar(C_DQF), i & 1);
       if (q == 0) TRACE(2, i, 0);
@@ -427,7 +430,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         const uint32_t buf = stage + (c & 1) * kH;
-        if (c >= 2) {                                // quarter c-2 must have left this buffer
+        if (c >= 2 || i > 0) {                       // the quarter staged two steps ago must have left this buffer
           if (q == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
           asm volatile("bar.sync 1, 128;" ::: "memory");
         }
@@ -445,15 +448,10 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
       }
-      if (q == 0) {
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-        mbar_arrive(bar(C_DOE + st));
-        TRACE(2, i, 2);
-      }
+      if (q == 0) TRACE(2, i, 2);
       w.next();
     }
     if (q == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    asm volatile("bar.sync 2, 256;" ::: "memory");   // the dO stages may now be reused by the dK write-out
   }
   // ===================================================================== dK / dV write-out
   // Every stage buffer is dead after the last MMA.  Thread = key row: TMEM -> registers -> its own
@@ -470,7 +468,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const float mul = isK ? prm.scale : 1.f;
     const int64_t row = ((int64_t)(it.tok + k) * prm.Hkv + g) * 128;
     const bool ok = k < it.len;
-    if (isK) asm volatile("bar.sync 2, 256;" ::: "memory");   // dK staging overlaps a dO stage: reducers must be done
     if (it.kind == 0) {
       const uint32_t srow = sbase + (isK ? 67584u : 0u) + k * 528;     // 528 B row pitch: conflict-free v4 stores
 #pragma unroll
