@@ -50,7 +50,7 @@ __device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u6
 #endif
 
 // delta[t,h] = sum_d dO*O (B1), stored head-major and padded per sequence to whole 128-row tiles
-// (so each (head, Q tile) is one aligned 512-byte run): auxD[h][tile*128 + r]; auxL = LSE*log2(e).
+// (so each (head, Q tile) is one aligned 512-byte run): auxD[h][tile*128 + r] = -delta; auxL = -LSE*log2(e).
 __global__ void __launch_bounds__(256)
 bwd_prep_kernel(const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __restrict__ dO,
                 const float* __restrict__ LSE, const int32_t* __restrict__ seq_off,
@@ -76,8 +76,8 @@ bwd_prep_kernel(const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __rest
       if (seq_off[mid] <= t) lo = mid; else hi = mid - 1;
     }
     const int64_t pos = (int64_t)h * aux_stride + (int64_t)qtile_off[lo] * 128 + (t - seq_off[lo]);
-    auxD[pos] = s;
-    auxL[pos] = LSE[w] * kLog2e;
+    auxD[pos] = -s;                    // negated: the main kernel adds them with packed FADD2 / FFMA2
+    auxL[pos] = -LSE[w] * kLog2e;
   }
 }
 
@@ -342,6 +342,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       if (threadIdx.x == 0) TRACE(1, i, 1);
       tc_fence_after();
       float p[64];
+      const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2);
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
         uint32_t s[32];
@@ -349,11 +350,14 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         tc_wait_ld();
 #pragma unroll
         for (int q4 = 0; q4 < 8; ++q4) {
-          const float4 L = aL[c * 8 + q4];
-          p[c * 32 + 4 * q4 + 0] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 0]), prm.scale_log2, -L.x));
-          p[c * 32 + 4 * q4 + 1] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 1]), prm.scale_log2, -L.y));
-          p[c * 32 + 4 * q4 + 2] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 2]), prm.scale_log2, -L.z));
-          p[c * 32 + 4 * q4 + 3] = ex2_approx(fmaf(__uint_as_float(s[4 * q4 + 3]), prm.scale_log2, -L.w));
+          const float4 L = aL[c * 8 + q4];          // -LSE*log2(e) of four query columns
+          float e0, e1, e2, e3;
+          unpack2(fma2(pack2(__uint_as_float(s[4 * q4 + 0]), __uint_as_float(s[4 * q4 + 1])), sc2, pack2(L.x, L.y)), e0, e1);
+          unpack2(fma2(pack2(__uint_as_float(s[4 * q4 + 2]), __uint_as_float(s[4 * q4 + 3])), sc2, pack2(L.z, L.w)), e2, e3);
+          p[c * 32 + 4 * q4 + 0] = ex2_approx(e0);
+          p[c * 32 + 4 * q4 + 1] = ex2_approx(e1);
+          p[c * 32 + 4 * q4 + 2] = ex2_approx(e2);
+          p[c * 32 + 4 * q4 + 3] = ex2_approx(e3);
         }
       }
       if (masked) {
@@ -385,17 +389,19 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         tc_wait_ld();
 #pragma unroll
         for (int q8 = 0; q8 < 4; ++q8) {
-          const float4 D0 = aD[c * 8 + q8 * 2], D1 = aD[c * 8 + q8 * 2 + 1];
+          const float4 D0 = aD[c * 8 + q8 * 2], D1 = aD[c * 8 + q8 * 2 + 1];   // -delta of eight query columns
           const int q = c * 32 + q8 * 8;
           uint32_t pk[4];
-          pk[0] = pack_bf16(p[q + 0] * (__uint_as_float(d[q8 * 8 + 0]) - D0.x),
-                            p[q + 1] * (__uint_as_float(d[q8 * 8 + 1]) - D0.y));
-          pk[1] = pack_bf16(p[q + 2] * (__uint_as_float(d[q8 * 8 + 2]) - D0.z),
-                            p[q + 3] * (__uint_as_float(d[q8 * 8 + 3]) - D0.w));
-          pk[2] = pack_bf16(p[q + 4] * (__uint_as_float(d[q8 * 8 + 4]) - D1.x),
-                            p[q + 5] * (__uint_as_float(d[q8 * 8 + 5]) - D1.y));
-          pk[3] = pack_bf16(p[q + 6] * (__uint_as_float(d[q8 * 8 + 6]) - D1.z),
-                            p[q + 7] * (__uint_as_float(d[q8 * 8 + 7]) - D1.w));
+          float x0, x1;
+          // dS = P * (dP - delta): packed FADD2 + FMUL2 on two columns at a time
+          unpack2(mul2(pack2(p[q + 0], p[q + 1]), add2(pack2(__uint_as_float(d[q8 * 8 + 0]), __uint_as_float(d[q8 * 8 + 1])), pack2(D0.x, D0.y))), x0, x1);
+          pk[0] = pack_bf16(x0, x1);
+          unpack2(mul2(pack2(p[q + 2], p[q + 3]), add2(pack2(__uint_as_float(d[q8 * 8 + 2]), __uint_as_float(d[q8 * 8 + 3])), pack2(D0.z, D0.w))), x0, x1);
+          pk[1] = pack_bf16(x0, x1);
+          unpack2(mul2(pack2(p[q + 4], p[q + 5]), add2(pack2(__uint_as_float(d[q8 * 8 + 4]), __uint_as_float(d[q8 * 8 + 5])), pack2(D1.x, D1.y))), x0, x1);
+          pk[2] = pack_bf16(x0, x1);
+          unpack2(mul2(pack2(p[q + 6], p[q + 7]), add2(pack2(__uint_as_float(d[q8 * 8 + 6]), __uint_as_float(d[q8 * 8 + 7])), pack2(D1.z, D1.w))), x0, x1);
+          pk[3] = pack_bf16(x0, x1);
           const uint32_t addr = ds_row + ((uint32_t)((c * 4 + q8) ^ (k & 7)) << 4);
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
         }
