@@ -316,7 +316,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     } }
   } else if (warp < 8) {
     // =================================================================== compute: P^T, dS^T
-    setmaxnreg_inc<144>();
+    setmaxnreg_inc<152>();
     const int wg = warp >> 2;                        // query-column half owned by this warpgroup
     const int k = threadIdx.x & 127;                 // key lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
@@ -344,10 +344,13 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       float p[64];
       const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2);
 #pragma unroll
+      uint32_t sall[64];
+      tmem_ld32(tSw, sall);                           // both 32-column loads in flight, one wait
+      tmem_ld32(tSw + 32, sall + 32);
+      tc_wait_ld();
+#pragma unroll
       for (int c = 0; c < 2; ++c) {
-        uint32_t s[32];
-        tmem_ld32(tSw + c * 32, s);
-        tc_wait_ld();
+        const uint32_t* s = sall + c * 32;
 #pragma unroll
         for (int q4 = 0; q4 < 8; ++q4) {
           const float4 L = aL[c * 8 + q4];          // -LSE*log2(e) of four query columns
@@ -383,10 +386,13 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       if (threadIdx.x == 0) TRACE(1, i, 4);
       tc_fence_after();
 #pragma unroll
+      uint32_t dall[64];
+      tmem_ld32(tdPw, dall);
+      tmem_ld32(tdPw + 32, dall + 32);
+      tc_wait_ld();
+#pragma unroll
       for (int c = 0; c < 2; ++c) {
-        uint32_t d[32];
-        tmem_ld32(tdPw + c * 32, d);
-        tc_wait_ld();
+        const uint32_t* d = dall + c * 32;
 #pragma unroll
         for (int q8 = 0; q8 < 4; ++q8) {
           const float4 D0 = aD[c * 8 + q8 * 2], D1 = aD[c * 8 + q8 * 2 + 1];   // -delta of eight query columns
@@ -406,15 +412,17 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
         }
       }
+      if (threadIdx.x == 0) TRACE(1, i, 6);
       tc_fence_before();
       fence_proxy_async();
+      if (threadIdx.x == 0) TRACE(1, i, 7);
       mbar_arrive(bar(C_DSF));
       if (threadIdx.x == 0) TRACE(1, i, 5);
       w.next();
     }
   } else {
     // =================================================================== dQ reducers (warps 8-11)
-    setmaxnreg_inc<160>();
+    setmaxnreg_inc<152>();
     const int q = threadIdx.x - 256;                 // query lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     Walk w(prm, it, g);
