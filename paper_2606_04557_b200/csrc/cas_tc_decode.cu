@@ -174,13 +174,15 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         for (int c = 0; c < 128; ++c)
           if (c >= limit) s[c] = 0xff800000u;
       }
-      float mx0 = -INFINITY, mx1 = -INFINITY;
+      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;   // four independent chains
 #pragma unroll
-      for (int c = 0; c < 128; c += 4) {
+      for (int c = 0; c < 128; c += 8) {
         mx0 = max3(mx0, __uint_as_float(s[c]), __uint_as_float(s[c + 1]));
         mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
+        mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
+        mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
       }
-      const float m_new = fmaxf(m, fmaxf(mx0, mx1) * prm.scale_log2);
+      const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * prm.scale_log2);
       if (j == 0) {
         m = m_new;
       } else if (__any_sync(0xffffffffu, m_new > m + 8.f)) {
