@@ -246,7 +246,9 @@ def main():
     # resident K+V elements the Adam call updates (with rotation: slots in transit this step are skipped, K4)
     n_upd = cfg.n_slots - ((cfg.rotate_in + cfg.rotate_out) if (cfg.rotate_in > 0 and not args.no_swap) else 0)
     n_el = 2 * int(sum(int(wl.cart_len[c]) for c in range(n_upd))) * cfg.Hkv * cfg.D
-    adam_bytes = 30 * n_el
+    # algorithmic bytes: 30 B per element of a slot that holds gradients this step (read g,p,m,v,
+    # write p,m,v + bf16 copy), 26 B per element of a clean slot (g = 0 is not read).  Counted per step in prepare().
+    adam_acc = {"bytes": 0, "steps": 0}
 
     rotate = cfg.rotate_in > 0 and not args.no_swap
     rot = {"step": 0, "rng": np.random.Generator(np.random.PCG64(BASE_SEED + 1000 + rank)), "bytes": 0}
@@ -263,6 +265,15 @@ def main():
             c = cas.cas_pool_counters(sess.pool)
             stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
             sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
+        if cfg.backward:
+            used = set(int(x) for x in sel_cart)
+            el = lambda c: 2 * int(wl.cart_len[c]) * cfg.Hkv * cfg.D
+            if cfg.rotate_in > 0:       # uniform lengths: n_upd slots are updated, the selected ones hold gradients
+                per = el(0)
+                adam_acc["bytes"] += 30 * per * len(used) + 26 * per * (n_upd - len(used))
+            else:
+                adam_acc["bytes"] += sum((30 if c in used else 26) * el(c) for c in range(cfg.n_slots))
+            adam_acc["steps"] += 1
         if cfg.backward or tau == 0:
             # training: a new batch and a new slot table every step.  Decode (c5): the selection is fixed while
             # a request generates, so the table (and its split-KV work list) is built once and reused per token.
@@ -318,6 +329,7 @@ def main():
     barrier()
     sampler.stop_flag = True
     total_ms = e0.elapsed_time(e1)
+    adam_bytes = adam_acc["bytes"] / max(adam_acc["steps"], 1)
     t_fwd = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     t_bwd = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     t_adam = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))

@@ -81,7 +81,9 @@ typedef struct {
 typedef struct {
   void* pool_K;             /* working copy [pool_tokens,Hkv,D], dtype */
   void* pool_V;
-  float* grad_K;            /* fp32 gradient slots [pool_tokens,Hkv,D] */
+  float* grad_K;            /* fp32 gradient slots [pool_tokens,Hkv,D]; the rows of a slot are defined only
+                               while the slot is grad-dirty (see cas_prefix_attn_bwd); a clean slot's
+                               gradient is zero by definition and its rows hold stale bytes */
   float* grad_V;
   float* state;             /* per slot s at state + 6*slot_base[s]*Hkv*D: six fp32 tensors of
                                slot_cap[s]*Hkv*D elements each: pK, pV, mK, mV, vK, vV */
@@ -104,7 +106,7 @@ typedef struct {
 typedef struct {
   float lr, beta1, beta2, eps;
   int32_t n_frozen;         /* first n_frozen tokens of every cartridge are not updated */
-  int32_t zero_grad;        /* 1: gradient slots are zeroed by the same kernel */
+  int32_t zero_grad;        /* 1: the step consumes the gradients: the slots become clean (gradient = 0) */
 } cas_adam_cfg;
 
 typedef struct {
@@ -134,11 +136,12 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
 int cas_pool_destroy(cas_pool* pool);
 int cas_pool_layout_get(const cas_pool* pool, cas_pool_layout* out);
 /* Initialise cartridge `cart` from host fp32 K,V [cart_len,Hkv,D]: master params <- K,V; moments
- * <- 0; resident: working copy <- cast(master), grads <- 0.  Synchronous. */
+ * <- 0; resident: working copy <- cast(master), slot clean (gradient 0).  Synchronous. */
 int cas_pool_load(cas_pool* pool, int32_t cart, const float* K, const float* V);
 /* Read back one tensor of a cartridge into host memory.  Synchronous (device-wide). `what`:
  * 0..5 = pK,pV,mK,mV,vK,vV (fp32, from the slot if resident else from the pinned home);
- * 6,7 = grad_K, grad_V (fp32, resident only); 8,9 = working copy K,V (pool dtype, resident only). */
+ * 6,7 = grad_K, grad_V (fp32, resident only; zeros for a clean slot); 8,9 = working copy K,V (pool dtype,
+ * resident only). */
 int cas_pool_read(cas_pool* pool, int32_t cart, int32_t what, void* out);
 /* Export integer state; any pointer may be NULL.  slot_of[n_carts] (-1 = not resident),
  * cart_in[n_slots] (-1 = free), opt_steps[n_carts], last_used[n_carts],
@@ -201,7 +204,10 @@ int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* pool, const cas_slot_tab
  * keys are ACCUMULATED (+=) into the pool's fp32 gradient slots of the selected slots, summed over
  * the Hq/Hkv heads of a group and over every sequence that selected the slot; slots selected by no
  * sequence are not touched.  dK_self/dV_self [T,Hkv,D] dtype are overwritten (may both be NULL).
- * Marks the selected slots grad-dirty. */
+ * Marks the selected slots grad-dirty.  "+=" is implemented without ever zeroing a buffer: a CLEAN slot
+ * (never touched, or consumed by cas_adam_step / cas_grad_zero, or just arrived) has gradient zero by
+ * definition, so the first backward pass that selects it OVERWRITES its rows and marks it dirty; later
+ * passes add.  Read gradients through cas_pool_read (zeros for clean slots), not through the raw rows. */
 int cas_prefix_attn_bwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
                         const void* K_self, const void* V_self, const void* O, const float* LSE,
                         const void* dO, float scale, void* dQ, void* dK_self, void* dV_self,
@@ -210,10 +216,12 @@ int cas_prefix_attn_bwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq,
 /* ---- optimizer ------------------------------------------------------------------------------ */
 /* One fused Adam step over the listed slots (slots == NULL: every resident slot whose cartridge
  * is not in transit).  Per cartridge: t = ++opt_steps; m = b1 m + (1-b1) g; v = b2 v + (1-b2) g^2;
- * p -= lr*lr_scale[i]*(m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps); working copy = RNE(p); g = 0 if
- * zero_grad.  lr_scale: host [n] per listed slot (PAPER.md:85 per-cartridge warmup), NULL = 1. */
+ * p -= lr*lr_scale[i]*(m/(1-b1^t)) / (sqrt(v/(1-b2^t)) + eps); working copy = RNE(p); with zero_grad
+ * the slot becomes clean (g = 0; nothing is written to the gradient rows).  A clean slot is updated with
+ * g = 0 and its gradient rows are not read.  lr_scale: host [n] per listed slot (PAPER.md:85 per-cartridge warmup), NULL = 1. */
 int cas_adam_step(cas_pool* pool, const cas_adam_cfg* cfg, const int32_t* slots, int32_t n,
                   const float* lr_scale, void* stream);
+/* Discards the gradients of the listed slots (NULL: all): the slots become clean.  Host bookkeeping only. */
 int cas_grad_zero(cas_pool* pool, const int32_t* slots, int32_t n, void* stream);
 
 /* ---- rotation (sec. 2.1 "Pool rotation"; Table 5 :377-381) ------------------------ */
@@ -229,7 +237,7 @@ int cas_plan_rotation(const cas_pool* pool, int64_t step, int32_t n_in, int32_t 
 /* Enqueue the OUT entries of a manifest on the side stream (resp. the IN entries on the library's
  * arrival stream), in order, one cudaMemcpyAsync per contiguous piece.  An arrival into a slot that
  * an eviction of the same round frees waits (per-slot event) for that eviction only.  After all
- * arrival copies, one kernel per arrival derives the working copy and zeroes the gradient slot.
+ * arrival copies, one kernel per arrival derives the working copy; the slot starts clean (gradient 0).
  * swap_out first waits (event) for work already enqueued on `after_stream` (the stream whose Adam
  * last wrote the evictees; may be NULL).
  * CAS_ERR_BUSY: evictee has un-consumed gradients / cartridge already in transit / slot occupied. */

@@ -1,8 +1,9 @@
 // HBM-bound elementwise kernels: fused Adam (sec. 2.2), arrival refresh (derive the
 // working copy + zero the gradient slot after a swap-in), zero fill.
 //
-// Roofline: HBM.  Adam moves 30 B per element (read g,p,m,v = 16 B; write p,m,v = 12 B + bf16
-// working copy 2 B), 34 B with the fused gradient zeroing.  All accesses are 16-byte vectors,
+// Roofline: HBM.  Adam moves 30 B per element of a slot that holds gradients (read g,p,m,v = 16 B; write p,m,v
+// = 12 B + bf16 working copy 2 B) and 26 B per element of a clean slot (g = 0 is not read).  Gradients are not
+// zeroed: consuming them = clearing the slot's dirty flag; the next backward pass overwrites a clean slot.  All accesses are 16-byte vectors,
 // fully coalesced, one (slot, chunk) per block; grid.y enumerates the slots.
 #include <algorithm>
 
@@ -42,17 +43,18 @@ adam_kernel(const __grid_constant__ AdamBatch batch, float lr, float b1, float b
     float* __restrict__ v = d.state + (int64_t)(4 + which) * d.cap_elems;
     float* __restrict__ g = which ? d.gV : d.gK;
     void* w = which ? d.wV : d.wK;
-    if (zero_grad)   // frozen tokens are not updated, but their gradients are consumed
-      for (int64_t i = ((int64_t)blockIdx.x * kAdamThreads + threadIdx.x) * 4; i < d.frozen_elems;
-           i += (int64_t)gridDim.x * kAdamThreads * 4)
-        st4(g + i, make_float4(0.f, 0.f, 0.f, 0.f));
+    // frozen tokens are not updated; gradients are consumed by clearing the slot's dirty flag on
+    // the host (a clean slot's buffer is undefined and overwritten by the next backward pass): nothing is zeroed
     for (int64_t base = d.frozen_elems + (int64_t)blockIdx.x * chunk; base < d.n_elems;
          base += (int64_t)gridDim.x * chunk) {
       float4 G[kAdamUnroll], P[kAdamUnroll], M[kAdamUnroll], V[kAdamUnroll];
 #pragma unroll
       for (int u = 0; u < kAdamUnroll; ++u) {
         const int64_t i = base + ((int64_t)u * kAdamThreads + threadIdx.x) * 4;
-        if (i < d.n_elems) { G[u] = ld4(g + i); P[u] = ld4(p + i); M[u] = ld4(m + i); V[u] = ld4(v + i); }
+        if (i < d.n_elems) {
+          G[u] = d.has_grad ? ld4(g + i) : make_float4(0.f, 0.f, 0.f, 0.f);   // clean slot: g = 0, not read
+          P[u] = ld4(p + i); M[u] = ld4(m + i); V[u] = ld4(v + i);
+        }
       }
 #pragma unroll
       for (int u = 0; u < kAdamUnroll; ++u) {
@@ -78,7 +80,6 @@ adam_kernel(const __grid_constant__ AdamBatch batch, float lr, float b1, float b
         st4(m + i, M[u]);
         st4(v + i, V[u]);
         store_work4(w, i, P[u], BF16);
-        if (zero_grad) st4(g + i, make_float4(0.f, 0.f, 0.f, 0.f));
       }
     }
   }
@@ -118,8 +119,6 @@ refresh_kernel(const float* __restrict__ pK, const float* __restrict__ pV, void*
   for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n; i += stride) {
     store_work4(wK, i, ld4(pK + i), BF16);
     store_work4(wV, i, ld4(pV + i), BF16);
-    st4(gK + i, make_float4(0.f, 0.f, 0.f, 0.f));
-    st4(gV + i, make_float4(0.f, 0.f, 0.f, 0.f));
   }
 }
 

@@ -62,6 +62,7 @@ static int check_desc(const cas_pool_desc* d) {
   if (d->dtype != CAS_F32 && d->dtype != CAS_BF16) { set_error("bad dtype"); return CAS_ERR_INVALID_ARG; }
   if (d->Hkv < 1 || d->D < 32 || d->D > 128 || d->D % 32) { set_error("Hkv>=1, D in {32,64,96,128}"); return CAS_ERR_SHAPE; }
   if (d->n_carts < 1 || d->n_slots < 1 || d->n_slots > d->n_carts) { set_error("need 1 <= n_slots <= n_carts"); return CAS_ERR_INVALID_ARG; }
+  if (d->n_slots > kMaxSlots) { set_error("at most %d slots", kMaxSlots); return CAS_ERR_CAPACITY; }
   if (d->tile_tokens < 0 || (d->tile_tokens && d->tile_tokens % 16)) { set_error("tile_tokens must be a multiple of 16"); return CAS_ERR_INVALID_ARG; }
   for (int i = 0; i < d->n_carts; ++i)
     if (d->cart_len[i] < 1) { set_error("cart_len[%d] < 1", i); return CAS_ERR_INVALID_ARG; }
@@ -285,6 +286,10 @@ int cas_pool_read(cas_pool* p, int32_t cart, int32_t what, void* out) {
   }
   if (s < 0) { set_error("cartridge %d not resident", cart); return CAS_ERR_NOT_RESIDENT; }
   const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
+  if ((what == 6 || what == 7) && !p->grad_dirty[s]) {   // a clean slot's buffer is undefined: its gradient is zero
+    memset(out, 0, (size_t)n * 4);
+    return CAS_OK;
+  }
   if (what == 6) CAS_CUDA(cudaMemcpy(out, p->grad_K + o, n * 4, cudaMemcpyDeviceToHost));
   if (what == 7) CAS_CUDA(cudaMemcpy(out, p->grad_V + o, n * 4, cudaMemcpyDeviceToHost));
   if (what == 8) CAS_CUDA(cudaMemcpy(out, (char*)p->pool_K + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
@@ -640,6 +645,15 @@ int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   a.stream = (cudaStream_t)stream;
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
+  if (!tc) {
+    // the CUDA-core path accumulates read-modify-write: give the clean slots it is about to touch real zeros
+    for (int sl : t->used_slots)
+      if (!p->grad_dirty[sl]) {
+        const int64_t o = (int64_t)p->slot_base[sl] * p->row_elems, nb = (int64_t)p->slot_cap[sl] * p->row_elems * 4;
+        CAS_CUDA(cudaMemsetAsync(p->grad_K + o, 0, nb, (cudaStream_t)stream));
+        CAS_CUDA(cudaMemsetAsync(p->grad_V + o, 0, nb, (cudaStream_t)stream));
+      }
+  }
   rc = tc ? tc_attn_bwd(a) : simt_attn_bwd(a);
   if (rc) return rc;
   for (int s : t->used_slots) p->grad_dirty[s] = 1;
@@ -688,7 +702,7 @@ int cas_adam_step(cas_pool* p, const cas_adam_cfg* cfg, const int32_t* slots, in
       h[i].step_size_scale = lr_scale ? lr_scale[i] : 1.0f;
       h[i].bc1 = (float)(1.0 - pow((double)cfg->beta1, t));
       h[i].bc2 = (float)(1.0 - pow((double)cfg->beta2, t));
-      h[i].pad = 0;
+      h[i].has_grad = p->grad_dirty[s] ? 1 : 0;
     }
     int rc = launch_adam(h.data(), cnt, *cfg, p->desc.dtype, (cudaStream_t)stream);
     if (rc) return rc;
@@ -708,10 +722,7 @@ int cas_grad_zero(cas_pool* p, const int32_t* slots, int32_t n, void* stream) {
   else for (int s = 0; s < p->desc.n_slots; ++s) list.push_back(s);
   for (int s : list) {
     if (s < 0 || s >= p->desc.n_slots) { set_error("bad slot"); return CAS_ERR_INVALID_ARG; }
-    const int64_t o = (int64_t)p->slot_base[s] * p->row_elems, nb = (int64_t)p->slot_cap[s] * p->row_elems * 4;
-    CAS_CUDA(cudaMemsetAsync(p->grad_K + o, 0, nb, (cudaStream_t)stream));
-    CAS_CUDA(cudaMemsetAsync(p->grad_V + o, 0, nb, (cudaStream_t)stream));
-    p->grad_dirty[s] = 0;
+    p->grad_dirty[s] = 0;   // clean = zero gradient; the buffer itself is overwritten by the next backward pass
   }
   return CAS_OK;
 }

@@ -165,6 +165,13 @@ struct cas_slot_table {
 namespace cas {
 
 // ---- kernel launchers (each returns CAS_OK / CAS_ERR_*) -------------------------------------
+// Slots whose gradient buffer holds valid data at the time of a backward launch (grad-dirty).  A CLEAN slot's
+// buffer is undefined: the first backward pass that touches it OVERWRITES, later ones accumulate.
+constexpr int kMaxSlots = 8192;
+struct SlotMask {
+  uint32_t w[kMaxSlots / 32];
+};
+
 struct AttnArgs {
   const cas_pool* pool;
   const cas_slot_table* tab;
@@ -204,7 +211,7 @@ struct AdamSlotDesc {
   int64_t frozen_elems;
   float step_size_scale;  // lr_scale
   float bc1, bc2;     // 1-beta1^t, 1-beta2^t
-  int32_t pad;
+  int32_t has_grad;   // 0: the slot's gradient buffer is not valid (clean slot): g = 0, nothing read or written
 };
 constexpr int kAdamBatch = 256;   // slot descriptors per launch, passed as kernel parameters (20 KB)
 struct AdamBatch {

@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1)
 tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmdO,
               const __grid_constant__ CUtensorMap tmKp, const __grid_constant__ CUtensorMap tmVp,
               const __grid_constant__ CUtensorMap tmKs, const __grid_constant__ CUtensorMap tmVs,
-              const BwdParams prm) {
+              const BwdParams prm, const __grid_constant__ SlotMask dirty) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + oBar + C_N * 8);
@@ -497,8 +497,13 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       }
       fence_proxy_async();
       if (ok) {
-        asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
-                     ::"l"((isK ? prm.gradK : prm.gradV) + row), "r"(srow), "r"(512u) : "memory");
+        // a slot that already holds gradients is added to; a clean slot's buffer is undefined and is overwritten
+        if ((dirty.w[it.id >> 5] >> (it.id & 31)) & 1u)
+          asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+                       ::"l"((isK ? prm.gradK : prm.gradV) + row), "r"(srow), "r"(512u) : "memory");
+        else
+          asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                       ::"l"((isK ? prm.gradK : prm.gradV) + row), "r"(srow), "r"(512u) : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
       }
     } else if (prm.dKs != nullptr) {
@@ -577,7 +582,10 @@ int tc_attn_bwd(const AttnArgs& a) {
                 a.pool->grad_K, a.pool->grad_V, (__nv_bfloat16*)a.dKs, (__nv_bfloat16*)a.dVs, (int64_t)nqt * 128,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale, a.scale * kLog2e};
   const unsigned grid = (unsigned)(t->bwd_items.size() * a.Hkv);
-  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm);
+  SlotMask dirty{};
+  for (int sl = 0; sl < a.pool->desc.n_slots; ++sl)
+    if (a.pool->grad_dirty[sl]) dirty.w[sl >> 5] |= 1u << (sl & 31);
+  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm, dirty);
   dq_convert_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
       dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows);
   cudaError_t e = cudaGetLastError();

@@ -215,3 +215,44 @@ def test_forward_cta_pair_kernel_parity():
     r = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, CAS_FWD_PAIRS="1"),
                        capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "pairs ok" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+def test_gradient_slots_accumulate_then_overwrite_after_adam():
+    """Gradient-slot life cycle on the tensor-core path: a second backward pass accumulates (+=), Adam consumes
+    the gradients (the slot becomes clean = zero gradient, its buffer is NOT zeroed), the next backward pass
+    overwrites the stale buffer, an untouched slot reads as exactly zero throughout, and a clean slot updated by
+    Adam behaves as g = 0."""
+    cfg = CONFIGS["c2"].scaled(name="c2_life", n_carts=6, n_slots=6, cart_len=200, B=2, Lq=260, n_dist=1)
+    wl = make_workload(cfg, 51)
+    cas.cas_set_impl(cas.CAS_IMPL_AUTO)
+    sess = Session(wl)
+    used = sorted(set(wl.sel_cart.tolist()))
+    unused = [c for c in range(cfg.n_carts) if c not in used]
+    assert unused
+    sess.fwd()
+    sess.bwd()
+    torch.cuda.synchronize()
+    g1 = {c: (sess.read(c, "gK").copy(), sess.read(c, "gV").copy()) for c in used}
+    assert all(np.abs(g1[c][0]).max() > 0 for c in used)
+    sess.bwd()                                   # accumulate: exactly twice (same summands, fp32 adds of equal values)
+    torch.cuda.synchronize()
+    for c in used:
+        np.testing.assert_allclose(sess.read(c, "gK"), 2 * g1[c][0], rtol=1e-6, atol=1e-12)
+        np.testing.assert_allclose(sess.read(c, "gV"), 2 * g1[c][1], rtol=1e-6, atol=1e-12)
+    for c in unused:
+        assert not sess.read(c, "gK").any() and not sess.read(c, "gV").any()
+    p_unused = sess.read(unused[0], "pK").copy()
+    sess.adam()                                  # consumes the gradients; clean slots are updated with g = 0
+    torch.cuda.synchronize()
+    for c in used:
+        assert not sess.read(c, "gK").any()      # clean slot reads as zero although its buffer still holds 2*g1
+    np.testing.assert_array_equal(sess.read(unused[0], "pK"), p_unused)   # g = 0 from m = v = 0: exact no-op
+    assert np.abs(sess.read(unused[0], "mK")).max() == 0
+    sess.fwd()
+    sess.bwd()                                   # first touch after Adam: overwrite, not 2*g1 + g
+    torch.cuda.synchronize()
+    for c in used:
+        g = sess.read(c, "gK")
+        assert rel_fro(g, g1[c][0]) < 0.5        # same order as one backward pass (parameters moved by one step)
+        assert rel_fro(g, 3 * g1[c][0]) > 0.5
+    sess.close()
