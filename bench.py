@@ -383,6 +383,7 @@ def main():
         hQ, hKs, hVs, hdO = pin(wl.Q), pin(wl.K_self), pin(wl.V_self), pin(wl.dO)
         hO = torch.empty_like(hQ).pin_memory()
         hdQ = torch.empty_like(hQ).pin_memory()
+        hdKs, hdVs = torch.empty_like(hKs).pin_memory(), torch.empty_like(hKs).pin_memory()
         hLSE = torch.empty((sess.tab.T, cfg.Hq), dtype=torch.float32).pin_memory()
         nb = cas.cas_train_step_host_scratch_bytes(sess.pool, sess.tab, cfg.Hq)
         scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
@@ -391,7 +392,7 @@ def main():
         def e2e_step():
             prepare()
             cas.cas_train_step_host(sess.pool, sess.tab, cfg.Hq, hQ, hKs, hVs, hdO, sess.scale, acfg, hO, hLSE, hdQ,
-                                    scratch)
+                                    hdKs, hdVs, scratch)
             finish()
 
         for _ in range(3):
@@ -405,7 +406,7 @@ def main():
         barrier()
         e2e_ms = a.elapsed_time(b) / args.steps
         h2d = sum(t.numel() * t.element_size() for t in (hQ, hKs, hVs, hdO))
-        d2h = sum(t.numel() * t.element_size() for t in (hO, hdQ, hLSE))
+        d2h = sum(t.numel() * t.element_size() for t in (hO, hdQ, hLSE, hdKs, hdVs))
         e2e = (e2e_ms, h2d, d2h)
 
     ms_step_max, e2e_ms_max, total_flops = reduce_over_ranks(ms_step, e2e[0] if e2e else 0.0, fwd_fl + bwd_fl,

@@ -192,7 +192,10 @@ int cas_rope_apply(int32_t dtype, int32_t B, const int32_t* seq_off, const int64
  *                  U own tokens seq_off[b]..t of K_self/V_self (causal, diagonal included);
  *   s_j = scale*q.k_j ; LSE[t,h] = ln sum_j exp(s_j) ; O[t,h,:] = sum_j exp(s_j-LSE) v_j.
  * Q,O device [T,Hq,D] dtype; K_self,V_self device [T,Hkv,D] dtype or both NULL (prefix only; then
- * every sequence must select >= 1 cartridge); LSE device [T,Hq] fp32. */
+ * every sequence must select >= 1 cartridge); LSE device [T,Hq] fp32.  scale must be positive and finite
+ * (CAS_ERR_INVALID_ARG otherwise: the kernels take row maxima on the raw scores).  Pool rows past a cartridge's
+ * length inside its slot are read by the tile loads and masked; they must stay finite (the arena is zero-filled at
+ * creation and the library never writes there). */
 int cas_prefix_attn_fwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
                         const void* K_self, const void* V_self, float scale, void* O, float* LSE,
                         void* stream);
@@ -207,7 +210,11 @@ int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* pool, const cas_slot_tab
  * Marks the selected slots grad-dirty.  "+=" is implemented without ever zeroing a buffer: a CLEAN slot
  * (never touched, or consumed by cas_adam_step / cas_grad_zero, or just arrived) has gradient zero by
  * definition, so the first backward pass that selects it OVERWRITES its rows and marks it dirty; later
- * passes add.  Read gradients through cas_pool_read (zeros for clean slots), not through the raw rows. */
+ * passes add.  Read gradients through cas_pool_read (zeros for clean slots), not through the raw rows.
+ * Determinism: dK/dV (pool slots and self) are bit-reproducible run to run -- every gradient row is produced by
+ * exactly one CTA in a fixed order.  dQ on the tensor-core path is NOT: the per-KV-tile partial dQ tiles are summed
+ * by fp32 reductions in L2 whose order depends on CTA scheduling, so two runs can differ in the last fp32 bits
+ * before the final rounding to bf16 (within 1 bf16 ulp per element; CAS_IMPL_SIMT is deterministic). */
 int cas_prefix_attn_bwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
                         const void* K_self, const void* V_self, const void* O, const float* LSE,
                         const void* dO, float scale, void* dQ, void* dK_self, void* dV_self,
@@ -281,18 +288,21 @@ int cas_warmup_scales(const cas_pool* pool, const int32_t* slots, int32_t n, int
 
 /* ---- end-to-end convenience: one training step from HOST buffers --------------------------------
  * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
- * resident slots, D2H of O, LSE, dQ.  Kernels run on `stream`; the copies run on two internal copy
- * streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and dQ
- * leaves under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
- * cas_train_step_host_scratch_bytes() and belongs to the library between back-to-back calls that reuse it
- * (the next call's input copies start as soon as the previous backward pass is done).  Asynchronous;
- * synchronise `stream` before reading the host results or overwriting the host inputs. */
+ * resident slots, D2H of O, LSE, dQ and (when hdK_self/hdV_self are given: both or neither) dK_self, dV_self --
+ * every result of the backward pass that does not stay in the pool.  Kernels run on `stream`; the copies run on
+ * two internal copy streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and
+ * dQ, dK_self, dV_self leave under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
+ * cas_train_step_host_scratch_bytes() and belongs to the library between back-to-back calls that reuse it: when
+ * the next call has the SAME scratch layout (same T, Hq, workspace size) its input copies start as soon as the
+ * previous backward pass is done; with a different layout (ragged batches) they wait for the previous call's last
+ * read-back, because the regions move.  Asynchronous; synchronise `stream` before reading the host results or
+ * overwriting the host inputs. */
 int cas_train_step_host_scratch_bytes(const cas_pool* pool, const cas_slot_table* table, int32_t Hq,
                                       size_t* bytes);
 int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,
                         const void* hK_self, const void* hV_self, const void* hdO, float scale,
-                        const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ,
-                        void* dev_scratch, size_t scratch_bytes, void* stream);
+                        const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ, void* hdK_self,
+                        void* hdV_self, void* dev_scratch, size_t scratch_bytes, void* stream);
 
 /* ---- hardware self-test (not on the hot path) --------------------------------------------------
  * D[256,128] fp32 = A[256,64] * B[128,64]^T (bf16, row-major, device) computed by ONE tcgen05.mma.cta_group::2

@@ -3,7 +3,7 @@
 Pure-Python (arbitrary-precision ints, lists, sorts) restatement of the budget manager's integer
 state machine: slot tables (K1), swap round-trip accounting (K2), the rotation plan (K3) and the
 per-step protocol (K4) of DESIGN.md "Bookkeeping".  The CUDA library implements the same rules
-independently in C++ (``csrc/cas_host.cpp``); the two share no code and are compared bit-exactly.
+independently in C++ (``csrc/cas_host.cu``); the two share no code and are compared bit-exactly.
 
 Passages followed:
   * PAPER.md:73 (sec. 2.1 Budget Manager): "maintains a fixed GPU pool of B <= N cartridges, keeping

@@ -355,8 +355,8 @@ def cas_train_step_host_scratch_bytes(pool: Pool, tab: SlotTable, Hq: int) -> in
 
 
 def cas_train_step_host(pool: Pool, tab: SlotTable, Hq: int, hQ, hKs, hVs, hdO, scale: float, cfg: AdamCfg,
-                        hO, hLSE, hdQ, scratch, stream=None):
+                        hO, hLSE, hdQ, hdKs, hdVs, scratch, stream=None):
     _check(lib().cas_train_step_host(pool.handle, tab.handle, C.c_int32(Hq), _dptr(hQ), _dptr(hKs),
                                      _dptr(hVs), _dptr(hdO), C.c_float(scale), C.byref(cfg), _dptr(hO),
-                                     _dptr(hLSE), _dptr(hdQ), _dptr(scratch),
+                                     _dptr(hLSE), _dptr(hdQ), _dptr(hdKs), _dptr(hdVs), _dptr(scratch),
                                      C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)))

@@ -182,6 +182,7 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_upload, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking);
     for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
+    p->ev_cart.assign(desc->n_carts, nullptr);   // created at a cartridge's first eviction
     p->ev_slot.assign(desc->n_slots, nullptr);
     for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
       e = cudaEventCreateWithFlags(&p->ev_slot[s2], cudaEventDisableTiming);
@@ -215,6 +216,7 @@ int cas_pool_destroy(cas_pool* p) {
     if (p->st_d2h) cudaStreamDestroy(p->st_d2h);
     for (cudaEvent_t ev : p->ev_step) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : p->ev_slot) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : p->ev_cart) if (ev) cudaEventDestroy(ev);
   }
   delete p;
   return CAS_OK;
@@ -396,16 +398,9 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
       const int nq = (rows + 127) / 128;
       t->fwd_items.push_back({b, r, rows, nq * npre + (r / 128) * nq + (nq == 2 ? 3 : 1)});
     }
-    for (int r = 0; r < lq; r += 512) {
-      const int rows = (int)std::min<int64_t>(512, lq - r);
-      const int nq = (rows + 127) / 128;
-      if (rows > 256) t->fwd2_items.push_back({b, r, rows, nq * npre + (r / 128) * nq});
-      else t->fwd_rest_items.push_back({b, r, rows, nq * npre + (r / 128) * nq});
-    }
     for (int r = 0; r < lq; r += 32) t->simt_items.push_back({b, r, (int)std::min<int64_t>(32, lq - r), 0});
   }
-  for (auto* v : {&t->fwd_items, &t->fwd2_items, &t->fwd_rest_items})
-    std::stable_sort(v->begin(), v->end(), [](const FwdItem& a, const FwdItem& b) { return a.cost > b.cost; });
+  std::stable_sort(t->fwd_items.begin(), t->fwd_items.end(), [](const FwdItem& a, const FwdItem& b) { return a.cost > b.cost; });
   for (int s : t->used_slots) {
     int cost = 0;
     for (int e = t->inv_off[s]; e < t->inv_off[s + 1]; ++e) {
@@ -432,8 +427,7 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
                  o_iseq = blob_add(off, t->inv_seq, 1), o_kto = blob_add(off, t->kv_tile_off),
                  o_kt = blob_add(off, t->kv_tiles, 1), o_fw = blob_add(off, t->fwd_items),
                  o_si = blob_add(off, t->simt_items), o_bw = blob_add(off, t->bwd_items),
-                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off),
-                 o_f2 = blob_add(off, t->fwd2_items, 1), o_fr = blob_add(off, t->fwd_rest_items, 1);
+                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off);
     const size_t o_cnt = off;
     off += 256;
     // a recycled blob whose last reader has finished, else a new one (device memory + pinned mirror)
@@ -487,8 +481,6 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
     put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
     put(o_qt, t->qtile_off.data(), t->qtile_off.size() * 4);
-    put(o_f2, t->fwd2_items.data(), t->fwd2_items.size() * sizeof(FwdItem));
-    put(o_fr, t->fwd_rest_items.data(), t->fwd_rest_items.size() * sizeof(FwdItem));
     cudaError_t e = cudaMemcpyAsync(blob.d, blob.h, off, cudaMemcpyHostToDevice, p->st_upload);
     if (e == cudaSuccess) e = cudaEventRecord(blob.ready, p->st_upload);
     if (e != cudaSuccess) { p->tab_free.push_back(blob); delete t; return cuda_fail(e, "slot table upload"); }
@@ -509,8 +501,6 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     t->d_bwd_items = (BwdItem*)(d + o_bw);
     t->d_used_slots = (int32_t*)(d + o_us);
     t->d_qtile_off = (int32_t*)(d + o_qt);
-    t->d_fwd2_items = (FwdItem*)(d + o_f2);
-    t->d_fwd_rest_items = (FwdItem*)(d + o_fr);
     t->d_counters = (int32_t*)(d + o_cnt);
   }
   *out = t;
@@ -565,9 +555,11 @@ int cas_position_offsets(const cas_pool* p, const cas_slot_table* t, int64_t* to
 // ---------------------------------------------------------------------------------------------
 // attention dispatch
 // ---------------------------------------------------------------------------------------------
-static int check_attn(const cas_pool* p, const cas_slot_table* t, int Hq, const void* Ks, const void* Vs) {
+static int check_attn(const cas_pool* p, const cas_slot_table* t, int Hq, const void* Ks, const void* Vs, float scale) {
   int rc = need_data(p);
   if (rc) return rc;
+  // the kernels take the row maximum on the raw scores and multiply by scale afterwards: correct for scale > 0 only
+  if (!(scale > 0.f) || !std::isfinite(scale)) { set_error("scale must be positive and finite"); return CAS_ERR_INVALID_ARG; }
   if (!t || t->pool != p) { set_error("table does not belong to this pool"); return CAS_ERR_INVALID_ARG; }
   if (Hq < 1 || Hq % p->desc.Hkv) { set_error("Hq must be a positive multiple of Hkv"); return CAS_ERR_SHAPE; }
   if ((Ks == nullptr) != (Vs == nullptr)) { set_error("K_self and V_self must both be given or both NULL"); return CAS_ERR_INVALID_ARG; }
@@ -605,7 +597,7 @@ static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) 
 
 int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
                         const void* Vs, float scale, void* O, float* LSE, void* stream) {
-  int rc = check_attn(p, t, Hq, Ks, Vs);
+  int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
   rc = table_on_stream(t, stream);
   if (rc) return rc;
@@ -629,7 +621,7 @@ int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* p, const cas_slot_table*
 int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
                         const void* Vs, const void* O, const float* LSE, const void* dO, float scale,
                         void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes, void* stream) {
-  int rc = check_attn(p, t, Hq, Ks, Vs);
+  int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
   rc = table_on_stream(t, stream);
   if (rc) return rc;
@@ -825,6 +817,10 @@ int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t st
       int rc = copy_cart(p, e[i].cart, e[i].slot, true, p->side);
       if (rc) return rc;
       CAS_CUDA(cudaEventRecord(p->ev_slot[e[i].slot], p->side));   // the slot is free once this copy is done
+      // ... and so is the cartridge's pinned home complete: a later arrival of the SAME cartridge (into any slot)
+      // must not read its home before this copy has landed
+      if (!p->ev_cart[e[i].cart]) CAS_CUDA(cudaEventCreateWithFlags(&p->ev_cart[e[i].cart], cudaEventDisableTiming));
+      CAS_CUDA(cudaEventRecord(p->ev_cart[e[i].cart], p->side));
     }
     p->in_transit[e[i].cart] = 1;
     p->pending.push_back({e[i], step});
@@ -854,8 +850,11 @@ int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t ste
   for (int i = 0; i < n && p->dev; ++i) {
     if (e[i].dir != CAS_DIR_IN) continue;
     const int c = e[i].cart, s = e[i].slot;
-    // after the eviction that frees this slot (if any); a slot that was already free has no pending user
-    if (leaving.count(s)) CAS_CUDA(cudaStreamWaitEvent(p->side_in, p->ev_slot[s], 0));
+    // after the eviction that freed this slot -- in this round or in an EARLIER, already committed one (its D2H copy
+    // may still be running, and it is also what carries the wait on the main-stream work that last used the slot).
+    // ev_slot[s] holds the record of the slot's last eviction copy; waiting on a never-recorded event is a no-op.
+    CAS_CUDA(cudaStreamWaitEvent(p->side_in, p->ev_slot[s], 0));
+    if (p->ev_cart[c]) CAS_CUDA(cudaStreamWaitEvent(p->side_in, p->ev_cart[c], 0));   // its own last eviction copy
     int rc = copy_cart(p, c, s, false, p->side_in);
     if (rc) return rc;
   }
@@ -903,10 +902,6 @@ int cas_swap_commit(cas_pool* p, void* main_stream) {
 // ---------------------------------------------------------------------------------------------
 // end-to-end step from host buffers
 // ---------------------------------------------------------------------------------------------
-struct StepScratch {
-  size_t oQ, oKs, oVs, odO, oO, oLSE, odQ, odKs, odVs, oWs, ws_bytes, total;
-};
-
 static StepScratch step_scratch(const cas_pool* p, const cas_slot_table* t, int Hq) {
   StepScratch s{};
   const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
@@ -929,30 +924,38 @@ int cas_train_step_host_scratch_bytes(const cas_pool* p, const cas_slot_table* t
 
 int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
                         const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
-                        float* hLSE, void* hdQ, void* scratch, size_t scratch_bytes, void* stream) {
+                        float* hLSE, void* hdQ, void* hdKs, void* hdVs, void* scratch, size_t scratch_bytes,
+                        void* stream) {
   int rc = need_data(p);
   if (rc) return rc;
   if (!t || !hQ || !hKs || !hVs || !hdO || !cfg || !hO || !hLSE || !hdQ || !scratch) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  if ((hdKs == nullptr) != (hdVs == nullptr)) { set_error("hdK_self / hdV_self: both or none"); return CAS_ERR_INVALID_ARG; }
   const StepScratch s = step_scratch(p, t, Hq);
   if (scratch_bytes < s.total) { set_error("scratch too small: need %zu", s.total); return CAS_ERR_CAPACITY; }
   char* d = (char*)scratch;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
   // Inputs arrive on st_h2d (Q, K_self, V_self first: the forward pass starts as soon as they are in;
-  // dO lands under the forward pass), results leave on st_d2h (O and LSE under the backward pass, dQ
-  // under Adam).  The main stream ends by waiting for the last copy, so "main stream done" still
-  // means "everything done".
+  // dO lands under the forward pass), results leave on st_d2h (O and LSE under the backward pass, dQ and
+  // dK_self/dV_self under Adam).  The main stream ends by waiting for the last copy, so "main stream done"
+  // still means "everything done".
   cudaEvent_t* ev = p->ev_step;
   CAS_CUDA(cudaEventRecord(ev[0], st));
-  if (p->step_prev_scratch == scratch && p->step_prev_stream == st) {
-    // back-to-back steps on the same scratch: the input buffers are free as soon as the PREVIOUS backward pass
-    // is done (ev[4] still holds that record), so these copies run under the previous Adam and dQ read-back
+  const bool same_layout = p->step_prev_scratch == scratch && p->step_prev_stream == st &&
+                           memcmp(&p->step_prev_layout, &s, sizeof(StepScratch)) == 0;
+  if (same_layout) {
+    // back-to-back steps on the same scratch WITH THE SAME LAYOUT (same T, Hq, workspace size): the input regions
+    // are free as soon as the PREVIOUS backward pass is done (ev[4] still holds that record) and they do not
+    // overlap the output regions the previous step's read-back may still be copying from, so these copies run
+    // under the previous Adam and dQ read-back.  With a different layout (ragged batches: T changes per step) the
+    // regions move and may overlap O / LSE / dQ of the previous step: wait for its last read-back instead.
     CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[4], 0));
   } else {
     CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
   }
   p->step_prev_scratch = scratch;
   p->step_prev_stream = st;
+  p->step_prev_layout = s;
   CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[0], 0));
   CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
   CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
@@ -974,6 +977,10 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   CAS_CUDA(cudaEventRecord(ev[4], st));
   CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[4], 0));
   CAS_CUDA(cudaMemcpyAsync(hdQ, d + s.odQ, T * Hq * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
+  if (hdKs) {
+    CAS_CUDA(cudaMemcpyAsync(hdKs, d + s.odKs, T * Hkv * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
+    CAS_CUDA(cudaMemcpyAsync(hdVs, d + s.odVs, T * Hkv * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
+  }
   CAS_CUDA(cudaEventRecord(ev[5], p->st_d2h));
   rc = cas_adam_step(p, cfg, nullptr, 0, nullptr, stream);
   if (rc) return rc;

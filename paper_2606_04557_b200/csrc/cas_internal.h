@@ -75,6 +75,11 @@ struct TabBlob {
   bool has_done = false;
 };
 
+// Layout of cas_train_step_host's device scratch (byte offsets of the staged inputs, outputs and workspace).
+struct StepScratch {
+  size_t oQ, oKs, oVs, odO, oO, oLSE, odQ, odKs, odVs, oWs, ws_bytes, total;
+};
+
 struct cas_pool {
   cas_pool_desc desc;
   std::vector<int32_t> cart_len;
@@ -103,6 +108,7 @@ struct cas_pool {
   cudaStream_t side_in = nullptr;
   cudaEvent_t ev_side_in = nullptr;
   std::vector<cudaEvent_t> ev_slot;
+  std::vector<cudaEvent_t> ev_cart;   // end of a cartridge's last eviction copy (its pinned home is complete)
   std::vector<TabBlob> tab_free;     // recycled slot-table blobs
   cudaStream_t st_upload = nullptr;  // slot-table uploads
   // cas_train_step_host: input / output copies on their own streams so they overlap the kernels
@@ -110,6 +116,7 @@ struct cas_pool {
   cudaEvent_t ev_step[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
   void* step_prev_scratch = nullptr;     // scratch / stream of the previous cas_train_step_host call
   cudaStream_t step_prev_stream = nullptr;
+  StepScratch step_prev_layout{};
   // TMA descriptors over the working copy (bf16, D==128 only)
   bool has_tma = false;
   CUtensorMap tm_K, tm_V;
@@ -133,8 +140,6 @@ struct cas_slot_table {
   std::vector<int32_t> qtile_off;             // [B+1] 128-row query tiles before sequence b
   std::vector<cas::KvTile> kv_tiles;
   std::vector<cas::FwdItem> fwd_items;        // 256-row blocks, longest first
-  std::vector<cas::FwdItem> fwd2_items;       // 512-row blocks with > 256 rows (CTA-pair kernel), longest first
-  std::vector<cas::FwdItem> fwd_rest_items;   // the 256-row blocks the pair kernel does not cover
   std::vector<cas::FwdItem> simt_items;       // 32-row blocks
   std::vector<cas::BwdItem> bwd_items;        // longest first
   int64_t pairs = 0, prefix_tokens = 0, unique_prefix_tokens = 0;
@@ -148,7 +153,7 @@ struct cas_slot_table {
           *d_inv_off = nullptr, *d_inv_seq = nullptr, *d_kv_tile_off = nullptr,
           *d_used_slots = nullptr, *d_sel_slot = nullptr, *d_qtile_off = nullptr;
   cas::KvTile* d_kv_tiles = nullptr;
-  cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr, *d_fwd2_items = nullptr, *d_fwd_rest_items = nullptr;
+  cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
   cas::BwdItem* d_bwd_items = nullptr;
   int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
   // decode-shaped batches: split-KV work items, built lazily for a given Hq by cas_tc_decode.cu
@@ -192,7 +197,6 @@ size_t simt_bwd_workspace(const cas_slot_table* t, int Hq);
 
 bool tc_supported(const cas_pool* p, const cas_slot_table* t, int Hq);
 int tc_attn_fwd(const AttnArgs& a);
-int tc_attn_fwd_pairs(const AttnArgs& a, int n_items);
 int tc_attn_bwd(const AttnArgs& a);
 size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D);
 int tc_make_pool_maps(cas_pool* p);

@@ -34,20 +34,6 @@ using namespace sm100;
 
 constexpr float kLog2e = 1.4426950408889634f;
 
-#ifdef CAS_TRACE
-// developer timeline: clock64 at the hand-offs of one CTA (role, iteration, event)
-__device__ long long cas_trace_buf[4 * 32 * 8];
-__device__ long long cas_cta_trace[8192 * 6];   // smid, t_start, t_loop0, t_loop1, t_end, n (globaltimer ns)
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define CTA_TRACE(slot, val) do { if (blockIdx.x < 8192) cas_cta_trace[blockIdx.x * 6 + (slot)] = (val); } while (0)
-#define TRACE(role, i, ev)                                                                   \
-  do {                                                                                       \
-    if (blockIdx.x == 777 && (i) < 32) cas_trace_buf[((role) * 32 + (i)) * 8 + (ev)] = clock64(); \
-  } while (0)
-#else
-#define TRACE(role, i, ev) do {} while (0)
-#define CTA_TRACE(slot, val) do {} while (0)
-#endif
 
 // delta[t,h] = sum_d dO*O (B1), stored head-major and padded per sequence to whole 128-row tiles
 // (so each (head, Q tile) is one aligned 512-byte run): auxD[h][tile*128 + r] = -delta; auxL = -LSE*log2(e).
@@ -192,9 +178,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   if (it.kind == 1 && !prm.has_self) return;     // prefix-only call: no self tiles (block-uniform)
 
   if (threadIdx.x == 0) {
-#ifdef CAS_TRACE
-    { unsigned sm; asm volatile("mov.u32 %0, %smid;" : "=r"(sm)); CTA_TRACE(0, sm); CTA_TRACE(1, gtime()); }
-#endif
     if (sbase & 1023u) __trap();
     for (int i = 0; i < C_N; ++i)
       mbar_init(bar(i), (i == C_PF || i == C_DSF) ? 256 : (i == C_DQD ? 128 : 1));
@@ -227,13 +210,11 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int st = i & 1;
         const uint32_t eph = ((i >> 1) & 1) ^ 1;
         mbar_wait(bar(C_QE + st), eph);
-        TRACE(3, i, 0);
         mbar_expect_tx(bar(C_QF + st), kT + 512);
         tma_load_3d(sbase + oQ + st * kT, &tmQ, bar(C_QF + st), 0, w.h, w.tok());
         tma_load_3d(sbase + oQ + st * kT + kH, &tmQ, bar(C_QF + st), 64, w.h, w.tok());
         bulk_load(sbase + oAuxL + st * 512, prm.auxL + w.aux(), 512, bar(C_QF + st));
         if (i > 0) mbar_wait(bar(C_DOE), (i - 1) & 1);   // dV(i-1) has read dO(i-1): the single dO stage is free
-        TRACE(3, i, 1);
         mbar_expect_tx(bar(C_DOF), kT + 512);
         tma_load_3d(sbase + oDO, &tmdO, bar(C_DOF), 0, w.h, w.tok());
         tma_load_3d(sbase + oDO + kH, &tmdO, bar(C_DOF), 64, w.h, w.tok());
@@ -265,14 +246,10 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_fence_after();
       mma_dP(0);
       mma_commit(bar(C_DPF));
-#ifdef CAS_TRACE
-      CTA_TRACE(2, gtime()); CTA_TRACE(5, n);
-#endif
       for (int i = 0; i < n; ++i) {
         const int st = i & 1, st1 = st ^ 1;
         const uint32_t ph1 = ((i + 1) >> 1) & 1;
         mbar_wait(bar(C_PF), i & 1);
-        TRACE(0, i, 0);
         tc_fence_after();
         // dV += P^T dO ; P^T (bf16) of query columns [0,64) sits at tS+[0,32), of [64,128) at tS+64+[0,32)
 #pragma unroll
@@ -286,9 +263,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           mma_S(st1);
           mma_commit(bar(C_SF));
         }
-        TRACE(0, i, 1);
         mbar_wait(bar(C_DSF), i & 1);
-        TRACE(0, i, 2);
         tc_fence_after();
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk)     // dQ = dS K
@@ -298,21 +273,15 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         for (int kk = 0; kk < 8; ++kk)     // dK += dS^T Q
           mma_ss(tdK, kmaj(sbase + oDS, kk), mnmaj(sbase + oQ + st * kT, kk), id_kmn, (i > 0 || kk > 0) ? 1u : 0u);
         mma_commit(bar(C_QE + st));
-        TRACE(0, i, 3);
         if (i + 1 < n) {
           mbar_wait(bar(C_DOF), (i + 1) & 1);
-          TRACE(0, i, 4);
           mbar_wait(bar(C_DQD), i & 1);
-          TRACE(0, i, 5);
           tc_fence_after();
           mma_dP(st1);
           mma_commit(bar(C_DPF));
         }
       }
       mma_commit(bar(C_DONE));
-#ifdef CAS_TRACE
-      CTA_TRACE(3, gtime());
-#endif
     } }
   } else if (warp < 8) {
     // =================================================================== compute: P^T, dS^T
@@ -337,9 +306,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const float4* aL = reinterpret_cast<const float4*>(smem + oAuxL + st * 512 + wg * 256);
       const float4* aD = reinterpret_cast<const float4*>(smem + oAuxD + st * 512 + wg * 256);
       mbar_wait(bar(C_QF + st), ph);
-      if (threadIdx.x == 0) TRACE(1, i, 0);
       mbar_wait(bar(C_SF), i & 1);
-      if (threadIdx.x == 0) TRACE(1, i, 1);
       tc_fence_after();
       float p[64];
       const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2);
@@ -379,11 +346,8 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_wait_st();
       tc_fence_before();
       mbar_arrive(bar(C_PF));
-      if (threadIdx.x == 0) TRACE(1, i, 2);
       mbar_wait(bar(C_DOF), i & 1);
-      if (threadIdx.x == 0) TRACE(1, i, 3);
       mbar_wait(bar(C_DPF), i & 1);
-      if (threadIdx.x == 0) TRACE(1, i, 4);
       tc_fence_after();
 #pragma unroll
       uint32_t dall[64];
@@ -412,12 +376,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
         }
       }
-      if (threadIdx.x == 0) TRACE(1, i, 6);
       tc_fence_before();
       fence_proxy_async();
-      if (threadIdx.x == 0) TRACE(1, i, 7);
       mbar_arrive(bar(C_DSF));
-      if (threadIdx.x == 0) TRACE(1, i, 5);
       w.next();
     }
   } else {
@@ -432,7 +393,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const uint32_t stage = sbase + oStg;           // dedicated staging: two 16 KB quarter-tile buffers
       float* dst = prm.dQacc + ((int64_t)w.h * (prm.aux_stride >> 7) + w.utile()) * 16384;
       mbar_wait(bar(C_DQF), i & 1);
-      if (q == 0) TRACE(2, i, 0);
       tc_fence_after();
       uint32_t d[128];
 #pragma unroll
@@ -440,7 +400,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       tc_wait_ld();
       tc_fence_before();
       mbar_arrive(bar(C_DQD));                       // TMEM is free for dP(i+1)
-      if (q == 0) TRACE(2, i, 1);
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         const uint32_t buf = stage + (c & 1) * kH;
@@ -462,7 +421,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
       }
-      if (q == 0) TRACE(2, i, 2);
       w.next();
     }
     if (q == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -532,9 +490,6 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   }
   tc_fence_before();
   __syncthreads();
-#ifdef CAS_TRACE
-  if (threadIdx.x == 0) CTA_TRACE(4, gtime());
-#endif
   if (warp == 12) tmem_dealloc(tbase, 512);
 }
 
@@ -548,10 +503,10 @@ size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D) {
 
 int tc_attn_bwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
-  static bool attr_set = false;
-  if (!attr_set) {
-    CAS_CUDA(cudaFuncSetAttribute(tc_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBwdSmem));
-    attr_set = true;
+  static SmemAttrOnce attr;
+  {
+    const int rc_attr = attr.set((const void*)tc_bwd_kernel, (int)kBwdSmem);
+    if (rc_attr) return rc_attr;
   }
   const size_t nqt = (size_t)t->qtile_off[t->B];
   const size_t b_acc = up1k((size_t)a.Hq * nqt * 65536), b_aux = up1k((size_t)a.Hq * nqt * 128 * 4);
@@ -594,11 +549,3 @@ int tc_attn_bwd(const AttnArgs& a) {
 
 }  // namespace cas
 
-#ifdef CAS_TRACE
-extern "C" int cas_debug_trace_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, cas::cas_trace_buf, sizeof(cas::cas_trace_buf));
-}
-extern "C" int cas_debug_cta_trace_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, cas::cas_cta_trace, sizeof(cas::cas_cta_trace));
-}
-#endif

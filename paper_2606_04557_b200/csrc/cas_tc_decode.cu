@@ -404,10 +404,10 @@ int tc_decode_fwd(const AttnArgs& a) {
   cas_slot_table* t = const_cast<cas_slot_table*>(a.tab);
   int rc = decode_prepare(t, a.Hq);
   if (rc) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    CAS_CUDA(cudaFuncSetAttribute(tc_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDecSmem));
-    attr_set = true;
+  static SmemAttrOnce attr;
+  {
+    const int rc_attr = attr.set((const void*)tc_decode_kernel, (int)kDecSmem);
+    if (rc_attr) return rc_attr;
   }
   const float scale_log2 = a.scale * 1.4426950408889634f;
   DecParams prm{t->d_dec_items, t->d_dec_seqs, t->d_dec_tiles, t->d_seq_off, (const __nv_bfloat16*)a.Q,

@@ -62,15 +62,6 @@ bool tc_supported(const cas_pool* p, const cas_slot_table*, int) {
 }
 
 // ------------------------------------------------------------------------------- kernel
-#ifdef CAS_TRACE
-__device__ long long cas_fwd_trace_buf[4 * 32 * 8];
-#define FTRACE(role, i, ev)                                                                       \
-  do {                                                                                            \
-    if (blockIdx.x == 300 && (i) < 32) cas_fwd_trace_buf[((role) * 32 + (i)) * 8 + (ev)] = clock64(); \
-  } while (0)
-#else
-#define FTRACE(role, i, ev) do {} while (0)
-#endif
 constexpr int kFwdThreads = 384;   // 3 warpgroups: two softmax groups + (TMA, MMA, 2 idle warps)
 constexpr uint32_t kTile = 32768, kHalf = 16384;
 constexpr uint32_t kOffQ = 0, kOffK = 2 * kTile, kOffV = 4 * kTile, kOffBar = 6 * kTile;
@@ -200,10 +191,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const bool act0 = j < nkv0, act1 = nq == 2;
         const bool nxt0 = j + 1 < nkv0, nxt1 = nq == 2 && j + 1 < n_max;
         mbar_wait(bar(B_VF + s), (j >> 1) & 1);
-        FTRACE(0, j, 0);
         if (act0) {
           mbar_wait(bar(B_PF), j & 1);
-          FTRACE(0, j, 1);
           tc_fence_after();
           issue_pv(0, j);
         }
@@ -215,10 +204,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           issue_qk(0, j + 1);
           mma_commit(bar(B_SF));
         }
-        FTRACE(0, j, 2);
         if (act1) {
           mbar_wait(bar(B_PF + 1), j & 1);
-          FTRACE(0, j, 3);
           tc_fence_after();
           issue_pv(1, j);
         }
@@ -228,7 +215,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           mma_commit(bar(B_SF + 1));
         }
         if (nxt0 || nxt1) mma_commit(bar(B_KE + ((j + 1) & 1)));
-        FTRACE(0, j, 4);
       }
       mma_commit(bar(B_OD));
     }
@@ -253,7 +239,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           limit = min(min(128, lq - k0), row - k0 + 1);
         }
         mbar_wait(bar(B_SF + t), j & 1);
-        if ((threadIdx.x & 127) == 0) FTRACE(1 + t, j, 0);
         tc_fence_after();
         uint32_t s[128];
         tmem_ld32(tS, s);
@@ -261,7 +246,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         tmem_ld32(tS + 64, s + 64);
         tmem_ld32(tS + 96, s + 96);
         tc_wait_ld();
-        if ((threadIdx.x & 127) == 0) FTRACE(1 + t, j, 1);
         if (!__all_sync(0xffffffffu, limit >= 128)) {
 #pragma unroll
           for (int c = 0; c < 128; ++c)
@@ -292,7 +276,6 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
             tmem_st32(tO + c * 32, o);
           }
         }
-        if ((threadIdx.x & 127) == 0) FTRACE(1 + t, j, 2);
         // p = 2^(s*scale_log2 - m): one packed FFMA per two scores, one MUFU each, packed row sum
         const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);
         uint64_t sum2a = pack2(0.f, 0.f), sum2b = sum2a;
@@ -314,13 +297,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           unpack2(add2(sum2a, sum2b), x0, x1);
           l += x0 + x1;
         }
-        if ((threadIdx.x & 127) == 0) FTRACE(1 + t, j, 3);
         tmem_st32(tS, s);
         tmem_st32(tS + 32, s + 32);
         tc_wait_st();
         tc_fence_before();
         mbar_arrive(bar(B_PF + t));
-        if ((threadIdx.x & 127) == 0) FTRACE(1 + t, j, 4);
       }
       // epilogue: O = acc / l, LSE = ln2 * m + ln(l)
       mbar_wait(bar(B_OD), 0);
@@ -355,25 +336,13 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 
 int tc_attn_fwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
-  // Opt-in (CAS_FWD_PAIRS=1): 512-row blocks go to the CTA-pair kernel (cas_tc_fwd2.cu), the rest to this one.
-  // Off by default: the pair kernel is parity-green but slower here (c2 0.90 vs 0.78 ms).
-  static const bool pairs = getenv("CAS_FWD_PAIRS") && getenv("CAS_FWD_PAIRS")[0] == '1';
   const FwdItem* items = t->d_fwd_items;
-  size_t n_items = t->fwd_items.size();
-  if (pairs && !t->fwd2_items.empty()) {
-    const int rc2 = tc_attn_fwd_pairs(a, (int)t->fwd2_items.size());
-    if (rc2) return rc2;
-    items = t->d_fwd_rest_items;
-    n_items = t->fwd_rest_items.size();
-    if (n_items == 0) return CAS_OK;
-  }
-  static bool attr_set = false;
-  if (!attr_set) {
-    CAS_CUDA(cudaFuncSetAttribute(tc_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFwdSmem));
-    attr_set = true;
-  }
+  const size_t n_items = t->fwd_items.size();
+  static SmemAttrOnce attr;
+  int rc = attr.set((const void*)tc_fwd_kernel, (int)kFwdSmem);
+  if (rc) return rc;
   CUtensorMap tmQ, tmKs, tmVs;
-  int rc = make_thd_map(&tmQ, a.Q, t->T, a.Hq, 128);
+  rc = make_thd_map(&tmQ, a.Q, t->T, a.Hq, 128);
   if (rc) return rc;
   if (a.Ks) {
     rc = make_thd_map(&tmKs, a.Ks, t->T, a.Hkv, 128);
@@ -394,8 +363,3 @@ int tc_attn_fwd(const AttnArgs& a) {
 
 }  // namespace cas
 
-#ifdef CAS_TRACE
-extern "C" int cas_debug_fwd_trace_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, cas::cas_fwd_trace_buf, sizeof(cas::cas_fwd_trace_buf));
-}
-#endif

@@ -37,6 +37,13 @@ def err(a, b, dtype):
     return rel_max(a, b) if dtype == "f32" else rel_fro(a, b)
 
 
+def kv_heads_for(seed: int, Hkv: int, n: int = 1):
+    """The KV head group(s) a full-size test compares completely (the oracle cannot afford all
+    Hkv groups at full size): derived from the seed, so no head is privileged by the test source."""
+    first = (seed * 2654435761 >> 7) % Hkv
+    return sorted({(first + i * (Hkv // 2 + 1)) % Hkv for i in range(n)})
+
+
 def oracle_inputs(wl):
     blocks_K = [wl.cart_kv(c)[0] for c in range(wl.cfg.n_carts)]
     blocks_V = [wl.cart_kv(c)[1] for c in range(wl.cfg.n_carts)]
@@ -76,21 +83,22 @@ def check_attention(wl, impl, kv_heads, self_block=True, backward=True, pre_grad
         assert np.isfinite(dQ).all()
         assert res["dQ"] <= tolO, res
         used = sorted(gKo.keys())
-        gk = np.concatenate([sess.read(c, "gK")[:, kv_heads].ravel() for c in used])
-        gv = np.concatenate([sess.read(c, "gV")[:, kv_heads].ravel() for c in used])
-        gko = np.concatenate([gKo[c][:, kv_heads].ravel() for c in used])
-        gvo = np.concatenate([gVo[c][:, kv_heads].ravel() for c in used])
-        res["dK"] = err(gk, gko, cfg.dtype)
-        res["dV"] = err(gv, gvo, cfg.dtype)
-        assert res["dK"] <= tolKV and res["dV"] <= tolKV, res
+        # dK/dV are gated PER SLOT (SURVEY.md A22 "per tensor"): a slot that one short sequence selected has small
+        # gradients and must not hide inside the norm of the big ones
+        res["dK"] = res["dV"] = 0.0
+        for c in used:
+            eK = err(sess.read(c, "gK")[:, kv_heads], gKo[c][:, kv_heads], cfg.dtype)
+            eV = err(sess.read(c, "gV")[:, kv_heads], gVo[c][:, kv_heads], cfg.dtype)
+            assert eK <= tolKV and eV <= tolKV, (c, eK, eV)
+            res["dK"], res["dV"] = max(res["dK"], eK), max(res["dV"], eV)
         if self_block:
             res["dKs"] = err(sess.np(sess.dKs)[:, kv_heads], dKso[:, kv_heads], cfg.dtype)
             res["dVs"] = err(sess.np(sess.dVs)[:, kv_heads], dVso[:, kv_heads], cfg.dtype)
             assert res["dKs"] <= tolKV and res["dVs"] <= tolKV, res
-        # unselected resident cartridges: gradient slots stay bit-zero
+        # unselected resident cartridges: EVERY such gradient slot stays bit-zero
         cnt = cas.cas_pool_counters(sess.pool)
         untouched = [c for c in range(cfg.n_carts) if cnt["slot_of"][c] >= 0 and c not in set(used)]
-        for c in untouched[:8]:
+        for c in untouched:
             assert not sess.read(c, "gK").any() and not sess.read(c, "gV").any()
         # conservation over ALL heads: sum of dV over every visible key = sum_i dO_i per KV head
         tot = np.zeros((cfg.Hkv, cfg.D))

@@ -3,7 +3,7 @@ published SplitMix64 test vectors for the priority hash, and structural properti
 import numpy as np
 import pytest
 
-from oracle.bookkeeping import DIR_IN, DIR_OUT, BookError, PoolBook, mix64
+from oracle.bookkeeping import DIR_IN, DIR_OUT, BookError, PoolBook, mix64, position_offsets
 
 NB = 6 * 16 * 4 * 4          # bytes of one 16-token cartridge home: 6 tensors x 16 x (Hkv*D=4) x 4 B
 
@@ -33,6 +33,7 @@ def test_hand_worked_rotation_trace():
     assert sel_slot == [1, 0, 1]
     assert inv_off == [0, 1, 3, 3] and inv_seq == [0, 0, 1]
     assert P == [32, 16]
+    assert position_offsets(bk, P) == (48, [32, 16])          # 3 resident cartridges x 16 tokens
     assert bk.last_used == [0, 0, -1, -1, -1, -1]
     man = bk.plan_rotation(0, n_in=1, n_out=1, protect=[0, 1], seed=1)
     assert [e.as_tuple() for e in man] == [(2, 2, DIR_OUT, 2 * NB, NB), (4, 2, DIR_IN, 4 * NB, NB)]
@@ -61,6 +62,25 @@ def test_hand_worked_rotation_trace():
     man = bk.plan_rotation(2, n_in=1, n_out=2, protect=[], seed=1)
     assert [e.as_tuple() for e in man] == [(0, 0, DIR_OUT, 0, NB), (2, 1, DIR_OUT, 2 * NB, NB),
                                            (1, 0, DIR_IN, NB, NB)]
+
+
+def test_position_offsets_hand_worked_ragged():
+    """PAPER.md:77 "offset by the total number of active cartridge KV tokens": lengths 16, 48, 32, 80, 64 with
+    the first three resident -> 96 active tokens; a sample that sees cartridges 2 and 0 has a 48-token visible
+    prefix (R7 returns both readings).  After cartridge 1 (48) is swapped for cartridge 4 (64) the
+    active total is 16 + 32 + 64 = 112."""
+    bk = PoolBook([16, 48, 32, 80, 64], n_slots=3, Hkv=1, D=4, tile_tokens=16)
+    _, _, _, P = bk.slot_table([0, 3, 8], [0, 2, 3], [2, 0, 1], step=0)
+    assert position_offsets(bk, P) == (96, [48, 48])
+    bk.adam_slots()
+    man = bk.plan_rotation(1, n_in=1, n_out=1, protect=[0, 2], seed=3)
+    assert [(e.cart, e.dir) for e in man][0] == (1, DIR_OUT)
+    bk.swap_out(man, 1)
+    arrival = [e.cart for e in man if e.dir == DIR_IN]
+    bk.swap_in(man, 1)
+    assert position_offsets(bk, [])[0] == 96                  # residency flips at commit, not before
+    bk.commit()
+    assert position_offsets(bk, [])[0] == 96 - 48 + bk.cart_len[arrival[0]]
 
 
 def test_validation_errors():

@@ -9,7 +9,7 @@ import re
 import numpy as np
 import pytest
 
-from oracle.bookkeeping import BookError, PoolBook
+from oracle.bookkeeping import BookError, PoolBook, position_offsets
 from paper_2606_04557_b200 import _build, cas
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -86,7 +86,7 @@ def run_protocol(N, S, steps, n_in, n_out, seed, rng, lens=None, B=3, nsel=4):
         lq = np.diff(seq_off)
         assert tab.info.pairs_per_head == int(sum(l * p + l * (l + 1) // 2 for l, p in zip(lq, want[3])))
         tot, P = cas.cas_position_offsets(pool, tab)
-        assert tot == sum(lens[c] for c in range(N) if bk.slot_of[c] >= 0) and P.tolist() == want[3]
+        assert (tot, P.tolist()) == position_offsets(bk, want[3])
         man, n = cas.cas_plan_rotation(pool, step, n_in, n_out, sorted(set(sel)), seed)
         wman = bk.plan_rotation(step, n_in, n_out, sorted(set(sel)), seed)
         assert manifest_tuples(man, n) == [e.as_tuple() for e in wman]
