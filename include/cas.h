@@ -74,6 +74,10 @@ typedef struct {
   int32_t tile_tokens;      /* slot capacity granularity; 0 => 128 (the KV tile of the kernels;
                                the paper's own page is 16 tokens) */
   const int32_t* cart_len;  /* host [n_carts], tokens per cartridge, each >= 1 */
+  int32_t n_layers;         /* L of Z in R^{L x p x d x 2}; 0 => 1.  Every layer has the same slot
+                               layout; the device arena holds L carvings back to back, a cartridge's pinned home
+                               L x (pK,pV,mK,mV,vK,vV).  Residency, step counts and rotation are per cartridge
+                               (all layers move together); gradients-dirty is tracked per (layer, slot) */
 } cas_pool_desc;
 
 /* Device-side layout of the pool inside the caller's arena (all pointers are device pointers
@@ -143,6 +147,9 @@ int cas_pool_load(cas_pool* pool, int32_t cart, const float* K, const float* V);
  * 6,7 = grad_K, grad_V (fp32, resident only; zeros for a clean slot); 8,9 = working copy K,V (pool dtype,
  * resident only). */
 int cas_pool_read(cas_pool* pool, int32_t cart, int32_t what, void* out);
+/* The same for one layer of a multi-layer pool (cas_pool_load / cas_pool_read act on layer 0). */
+int cas_pool_load_layer(cas_pool* pool, int32_t layer, int32_t cart, const float* K, const float* V);
+int cas_pool_read_layer(cas_pool* pool, int32_t layer, int32_t cart, int32_t what, void* out);
 /* Export integer state; any pointer may be NULL.  slot_of[n_carts] (-1 = not resident),
  * cart_in[n_slots] (-1 = free), opt_steps[n_carts], last_used[n_carts],
  * in_transit[n_carts] (0 stable, 1 leaving, 2 arriving), grad_dirty[n_slots]. */
@@ -199,6 +206,29 @@ int cas_rope_apply(int32_t dtype, int32_t B, const int32_t* seq_off, const int64
 int cas_prefix_attn_fwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,
                         const void* K_self, const void* V_self, float scale, void* O, float* LSE,
                         void* stream);
+/* Decode step with a growing self cache (sec. 2.5 inference: the selected
+ * cartridges' KV are concatenated before the prompt; :340 App. A "2048 maximum completion tokens").  `table` must
+ * hold ONE query token per sequence (seq_off = 0,1,..,B); Q,O device [B,Hq,D] bf16, LSE device [B,Hq] fp32.  The
+ * keys of sequence b are all tokens of its selected cartridges (read in place from the pool) plus rows
+ * [0, self_len[b]) of ITS OWN cache K_cache/V_cache, device [B, cache_cap, Hkv, D] bf16: the caller appends the
+ * current token's key/value at row self_len[b]-1 before the call, so the query sees itself (causal diagonal) and
+ * every earlier token of the sequence.  self_len is a HOST array [B], 0 <= self_len[b] <= cache_cap.  K_cache and
+ * V_cache may both be NULL (prefix only).  The result is cas_prefix_attn_fwd's for the last row of a sequence of
+ * self_len[b] tokens.  Cache rows at and beyond self_len[b] are loaded with their tile and masked: they must hold
+ * FINITE values (zero-initialise the cache).  bf16 pools with D = 128 only (CAS_ERR_SHAPE otherwise); at most 1024
+ * sequences per call when a cache is given (CAS_ERR_CAPACITY).  One kernel launch: split-KV partials are merged by
+ * the CTA that finishes a row last.  A slot table carries the scratch of ONE decode launch at a time: launches that
+ * share a table must be ordered (same stream).  Asynchronous on `stream`. */
+int cas_decode_attn(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q, const void* K_cache,
+                    const void* V_cache, int32_t cache_cap, const int32_t* self_len, float scale, void* O,
+                    float* LSE, void* stream);
+/* Retrieval-ordered cartridge selection (sec. 3 "Retrieval": "we map each retrieved chunk to a document
+ * id, which in turn is associated with a cartridge.  The final list contains the unique cartridge ids in the order of
+ * their retrieval").  chunk_ids[k]: retrieved chunks, best first; chunk_to_cart[n_chunks]: chunk -> cartridge id.
+ * Writes at most max_carts distinct cartridge ids in order of first appearance.  Host only. */
+int cas_select_retrieved(const int32_t* chunk_ids, int32_t k, const int32_t* chunk_to_cart, int32_t n_chunks,
+                         int32_t max_carts, int32_t* out_carts, int32_t* n_out);
+
 /* Device workspace bytes cas_prefix_attn_bwd needs for this table / Hq. */
 int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* pool, const cas_slot_table* table,
                                         int32_t Hq, size_t* bytes);
@@ -286,13 +316,47 @@ int cas_lr_schedule(const cas_lr_cfg* cfg, int64_t t, double* eta);
 int cas_warmup_scales(const cas_pool* pool, const int32_t* slots, int32_t n, int32_t w_c, int32_t n_b,
                       float* scale);
 
+/* ---- the layer axis and micro-batches -----------------------------------------
+ * a cartridge is Z in R^{L x p x d x 2} -- one K/V block per attention layer; PAPER.md:375-376 (Table 5):
+ * global batch 128 of packed 8,192-token sequences, i.e. several micro-batches per optimizer step.  The *_layer
+ * calls are cas_prefix_attn_fwd / _bwd / cas_decode_attn on layer `layer` of the pool (those act on layer 0); ONE
+ * slot table serves every layer (the selection, and the residency it was built against, are per cartridge).
+ * cas_adam_step updates every layer of the listed slots in one launch sequence, cas_swap_* move every layer. */
+int cas_prefix_attn_fwd_layer(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
+                              const void* K_self, const void* V_self, float scale, void* O, float* LSE, void* stream);
+int cas_prefix_attn_bwd_layer(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
+                              const void* K_self, const void* V_self, const void* O, const float* LSE,
+                              const void* dO, float scale, void* dQ, void* dK_self, void* dV_self, void* workspace,
+                              size_t workspace_bytes, void* stream);
+int cas_decode_attn_layer(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
+                          const void* K_cache, const void* V_cache, int32_t cache_cap, const int32_t* self_len,
+                          float scale, void* O, float* LSE, void* stream);
+/* Device buffers of one (micro-batch, layer): shapes as in cas_prefix_attn_fwd / _bwd. */
+typedef struct {
+  const void *Q, *K_self, *V_self, *dO;
+  void* O;
+  float* LSE;
+  void *dQ, *dK_self, *dV_self;
+} cas_layer_io;
+/* One optimizer step: for every micro-batch m (its own slot table tables[m], all built against the current
+ * residency) the forward pass of layers 0..L-1, then the backward pass of layers L-1..0 -- dK/dV ACCUMULATE into the
+ * gradient slots across micro-batches -- and then ONE cas_adam_step over all stable resident slots (lr_scale as
+ * there, per resident slot in ascending slot order, or NULL).  io[m * L + l].  In a real model each layer's Q and
+ * dO come from the frozen network around the attention call; this driver takes them all up front (synthetic
+ * benchmarks, tests).  workspace: cas_train_step_layers_workspace_bytes().  Asynchronous on `stream`. */
+int cas_train_step_layers_workspace_bytes(const cas_pool* pool, const cas_slot_table* const* tables, int32_t n_micro,
+                                          int32_t Hq, size_t* bytes);
+int cas_train_step_layers(cas_pool* pool, const cas_slot_table* const* tables, int32_t n_micro, int32_t Hq,
+                          const cas_layer_io* io, float scale, const cas_adam_cfg* cfg, const float* lr_scale,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- end-to-end convenience: one training step from HOST buffers --------------------------------
  * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
  * resident slots, D2H of O, LSE, dQ and (when hdK_self/hdV_self are given: both or neither) dK_self, dV_self --
  * every result of the backward pass that does not stay in the pool.  Kernels run on `stream`; the copies run on
  * two internal copy streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and
  * dQ, dK_self, dV_self leave under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
- * cas_train_step_host_scratch_bytes() and belongs to the library between back-to-back calls that reuse it: when
+ * cas_train_step_host_scratch_bytes() (single-layer pools only) and belongs to the library between back-to-back calls that reuse it: when
  * the next call has the SAME scratch layout (same T, Hq, workspace size) its input copies start as soon as the
  * previous backward pass is done; with a different layout (ragged batches) they wait for the previous call's last
  * read-back, because the regions move.  Asynchronous; synchronise `stream` before reading the host results or

@@ -57,7 +57,8 @@ class PoolBook:
     """Integer state of the cartridge pool."""
 
     def __init__(self, cart_len: Sequence[int], n_slots: int, Hkv: int, D: int,
-                 tile_tokens: int = 128):
+                 tile_tokens: int = 128, n_layers: int = 1):
+        self.n_layers = int(n_layers)               # PAPER.md:42: Z in R^{L x p x d x 2}; a home holds all L layers
         self.cart_len = [int(x) for x in cart_len]
         self.n_carts = len(self.cart_len)
         self.n_slots = int(n_slots)
@@ -92,7 +93,7 @@ class PoolBook:
         self.pending: List[Tuple[ManifestEntry, int]] = []   # (entry, plan step)
 
     def home_bytes(self, c: int) -> int:
-        return 6 * self.cart_len[c] * self.row_elems * 4
+        return self.n_layers * 6 * self.cart_len[c] * self.row_elems * 4
 
     # ---- K1 ---------------------------------------------------------------------------------
     def slot_table(self, seq_off: Sequence[int], sel_off: Sequence[int], sel_cart: Sequence[int],
@@ -301,3 +302,22 @@ def warmup_scale(s: int, w_c: int, n_b: int) -> float:
     num = min(s + 1, w_c) * n_b                      # min(1,(s+1)/W_c) * N_b = num / w_c
     level = -(-num // w_c)                           # ceil
     return level / n_b
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: retrieval-ordered cartridge selection
+# ---------------------------------------------------------------------------------------------
+def select_retrieved(chunk_ids: Sequence[int], chunk_to_cart: Sequence[int], max_carts: int) -> List[int]:
+    """PAPER.md:142 (sec. 3, Retrieval): "we map each retrieved chunk to a document id, which in turn is associated
+    with a cartridge.  The final list contains the unique cartridge ids in the order of their retrieval."
+    chunk_ids are ranked best first; at most max_carts cartridges are kept (the k of "top-k cartridges")."""
+    out: List[int] = []
+    for ch in chunk_ids:
+        if len(out) >= max_carts:
+            break
+        if ch < 0 or ch >= len(chunk_to_cart):
+            raise BookError("INVALID_ARG", "chunk id")
+        c = int(chunk_to_cart[ch])
+        if c not in out:
+            out.append(c)
+    return out

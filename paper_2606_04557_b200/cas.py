@@ -32,7 +32,8 @@ class CasError(RuntimeError):
 
 class PoolDesc(C.Structure):
     _fields_ = [("dtype", C.c_int32), ("Hkv", C.c_int32), ("D", C.c_int32), ("n_carts", C.c_int32),
-                ("n_slots", C.c_int32), ("tile_tokens", C.c_int32), ("cart_len", C.POINTER(C.c_int32))]
+                ("n_slots", C.c_int32), ("tile_tokens", C.c_int32), ("cart_len", C.POINTER(C.c_int32)),
+                ("n_layers", C.c_int32)]
 
 
 class PoolLayout(C.Structure):
@@ -120,10 +121,11 @@ class Pool:
     """Owns the torch tensors backing the arenas + the opaque cas_pool handle."""
 
     def __init__(self, dtype: int, Hkv: int, D: int, cart_len: Sequence[int], n_slots: int,
-                 tile_tokens: int = 0, device: Optional[str] = "cuda:0", side_stream=None):
+                 tile_tokens: int = 0, device: Optional[str] = "cuda:0", side_stream=None, n_layers: int = 1):
         self._cart_len = _i32(cart_len)
+        self.n_layers = n_layers
         self.desc = PoolDesc(dtype, Hkv, D, len(self._cart_len), n_slots, tile_tokens,
-                             _p(self._cart_len))
+                             _p(self._cart_len), n_layers)
         self.dtype, self.Hkv, self.D = dtype, Hkv, D
         self.n_carts, self.n_slots = len(self._cart_len), n_slots
         self.dev_bytes, self.host_bytes = cas_pool_query_bytes(self.desc)
@@ -160,23 +162,25 @@ class Pool:
             pass
 
 
-def cas_pool_load(pool: Pool, cart: int, K: np.ndarray, V: np.ndarray):
+def cas_pool_load(pool: Pool, cart: int, K: np.ndarray, V: np.ndarray, layer: int = 0):
     K = np.ascontiguousarray(K, dtype=np.float32)
     V = np.ascontiguousarray(V, dtype=np.float32)
-    _check(lib().cas_pool_load(pool.handle, C.c_int32(cart), _p(K, C.c_float), _p(V, C.c_float)))
+    _check(lib().cas_pool_load_layer(pool.handle, C.c_int32(layer), C.c_int32(cart), _p(K, C.c_float),
+                                     _p(V, C.c_float)))
 
 
 READ_NAMES = {"pK": 0, "pV": 1, "mK": 2, "mV": 3, "vK": 4, "vV": 5, "gK": 6, "gV": 7, "wK": 8, "wV": 9}
 
 
-def cas_pool_read(pool: Pool, cart: int, what) -> np.ndarray:
+def cas_pool_read(pool: Pool, cart: int, what, layer: int = 0) -> np.ndarray:
     w = READ_NAMES[what] if isinstance(what, str) else int(what)
     n = int(pool._cart_len[cart])
     if w < 8 or pool.dtype == CAS_F32:
         out = np.empty((n, pool.Hkv, pool.D), dtype=np.float32)
     else:
         out = np.empty((n, pool.Hkv, pool.D), dtype=np.uint16)       # raw bf16 bits
-    _check(lib().cas_pool_read(pool.handle, C.c_int32(cart), C.c_int32(w), C.c_void_p(out.ctypes.data)))
+    _check(lib().cas_pool_read_layer(pool.handle, C.c_int32(layer), C.c_int32(cart), C.c_int32(w),
+                                     C.c_void_p(out.ctypes.data)))
     return out
 
 
@@ -254,10 +258,27 @@ def cas_rope_apply(dtype: int, seq_off, pos_off, H: int, D: int, base: float, la
 
 
 def cas_prefix_attn_fwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, scale: float, O, LSE,
-                        stream=None):
-    _check(lib().cas_prefix_attn_fwd(pool.handle, tab.handle, C.c_int32(Hq), _dptr(Q), _dptr(K_self),
-                                     _dptr(V_self), C.c_float(scale), _dptr(O), _dptr(LSE),
-                                     _stream(stream)))
+                        stream=None, layer: int = 0):
+    _check(lib().cas_prefix_attn_fwd_layer(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q),
+                                           _dptr(K_self), _dptr(V_self), C.c_float(scale), _dptr(O), _dptr(LSE),
+                                           _stream(stream)))
+
+
+def cas_decode_attn(pool: Pool, tab: SlotTable, Hq: int, Q, K_cache, V_cache, cache_cap: int, self_len, scale: float,
+                    O, LSE, stream=None, layer: int = 0):
+    sl = None if self_len is None else _i32(self_len)
+    _check(lib().cas_decode_attn_layer(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q),
+                                       _dptr(K_cache), _dptr(V_cache), C.c_int32(cache_cap), _p(sl), C.c_float(scale),
+                                       _dptr(O), _dptr(LSE), _stream(stream)))
+
+
+def cas_select_retrieved(chunk_ids, chunk_to_cart, max_carts: int) -> np.ndarray:
+    ch, mp = _i32(chunk_ids), _i32(chunk_to_cart)
+    out = np.empty(max(max_carts, 1), np.int32)
+    n = C.c_int32(0)
+    _check(lib().cas_select_retrieved(_p(ch), C.c_int32(len(ch)), _p(mp), C.c_int32(len(mp)), C.c_int32(max_carts),
+                                      _p(out), C.byref(n)))
+    return out[:n.value].copy()
 
 
 def cas_prefix_attn_bwd_workspace_bytes(pool: Pool, tab: SlotTable, Hq: int) -> int:
@@ -267,12 +288,44 @@ def cas_prefix_attn_bwd_workspace_bytes(pool: Pool, tab: SlotTable, Hq: int) -> 
 
 
 def cas_prefix_attn_bwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, O, LSE, dO, scale: float,
-                        dQ, dK_self, dV_self, workspace, stream=None):
-    _check(lib().cas_prefix_attn_bwd(pool.handle, tab.handle, C.c_int32(Hq), _dptr(Q), _dptr(K_self),
-                                     _dptr(V_self), _dptr(O), _dptr(LSE), _dptr(dO), C.c_float(scale),
-                                     _dptr(dQ), _dptr(dK_self), _dptr(dV_self), _dptr(workspace),
-                                     C.c_size_t(workspace.numel() * workspace.element_size()),
-                                     _stream(stream)))
+                        dQ, dK_self, dV_self, workspace, stream=None, layer: int = 0):
+    _check(lib().cas_prefix_attn_bwd_layer(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q),
+                                           _dptr(K_self), _dptr(V_self), _dptr(O), _dptr(LSE), _dptr(dO),
+                                           C.c_float(scale), _dptr(dQ), _dptr(dK_self), _dptr(dV_self),
+                                           _dptr(workspace),
+                                           C.c_size_t(workspace.numel() * workspace.element_size()),
+                                           _stream(stream)))
+
+
+class LayerIO(C.Structure):
+    _fields_ = [("Q", C.c_void_p), ("K_self", C.c_void_p), ("V_self", C.c_void_p), ("dO", C.c_void_p),
+                ("O", C.c_void_p), ("LSE", C.c_void_p), ("dQ", C.c_void_p), ("dK_self", C.c_void_p),
+                ("dV_self", C.c_void_p)]
+
+
+def cas_train_step_layers(pool: Pool, tabs, Hq: int, io, scale: float, cfg: AdamCfg, lr_scale=None, workspace=None,
+                          stream=None):
+    """io[m][l]: dict of torch tensors Q, K_self, V_self, dO, O, LSE, dQ, dK_self, dV_self (micro-batch m, layer l)."""
+    n_micro, L = len(tabs), pool.n_layers
+    arr = (LayerIO * (n_micro * L))()
+    for m in range(n_micro):
+        for l in range(L):
+            for k, _ in LayerIO._fields_:
+                t = io[m][l].get(k)
+                setattr(arr[m * L + l], k, None if t is None else t.data_ptr())
+    tp = (C.c_void_p * n_micro)(*[t.handle for t in tabs])
+    ls = None if lr_scale is None else np.ascontiguousarray(lr_scale, dtype=np.float32)
+    _check(lib().cas_train_step_layers(pool.handle, tp, C.c_int32(n_micro), C.c_int32(Hq), arr, C.c_float(scale),
+                                       C.byref(cfg), _p(ls, C.c_float), _dptr(workspace),
+                                       C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
+def cas_train_step_layers_workspace_bytes(pool: Pool, tabs, Hq: int) -> int:
+    n = C.c_size_t(0)
+    tp = (C.c_void_p * len(tabs))(*[t.handle for t in tabs])
+    _check(lib().cas_train_step_layers_workspace_bytes(pool.handle, tp, C.c_int32(len(tabs)), C.c_int32(Hq),
+                                                       C.byref(n)))
+    return n.value
 
 
 def cas_adam_step(pool: Pool, cfg: AdamCfg, slots=None, lr_scale=None, stream=None, host_only=False):

@@ -63,6 +63,7 @@ static int check_desc(const cas_pool_desc* d) {
   if (d->Hkv < 1 || d->D < 32 || d->D > 128 || d->D % 32) { set_error("Hkv>=1, D in {32,64,96,128}"); return CAS_ERR_SHAPE; }
   if (d->n_carts < 1 || d->n_slots < 1 || d->n_slots > d->n_carts) { set_error("need 1 <= n_slots <= n_carts"); return CAS_ERR_INVALID_ARG; }
   if (d->n_slots > kMaxSlots) { set_error("at most %d slots", kMaxSlots); return CAS_ERR_CAPACITY; }
+  if (d->n_layers < 0 || d->n_layers > 1024) { set_error("n_layers must be in [0, 1024] (0 = 1)"); return CAS_ERR_INVALID_ARG; }
   if (d->tile_tokens < 0 || (d->tile_tokens && d->tile_tokens % 16)) { set_error("tile_tokens must be a multiple of 16"); return CAS_ERR_INVALID_ARG; }
   for (int i = 0; i < d->n_carts; ++i)
     if (d->cart_len[i] < 1) { set_error("cart_len[%d] < 1", i); return CAS_ERR_INVALID_ARG; }
@@ -122,10 +123,11 @@ int cas_pool_query_bytes(const cas_pool_desc* desc, size_t* dev_bytes, size_t* h
   if (pool_tokens >= (1ll << 31)) { set_error("pool too large for int32 token indices"); return CAS_ERR_CAPACITY; }
   const int64_t row = (int64_t)desc->Hkv * desc->D;
   Carve c = carve(pool_tokens, row, desc->dtype == CAS_BF16 ? 2 : 4);
-  if (dev_bytes) *dev_bytes = (size_t)c.total;
+  const int64_t L = desc->n_layers ? desc->n_layers : 1;
+  if (dev_bytes) *dev_bytes = (size_t)(L * c.total);
   if (host_bytes) {
     int64_t h = 0;
-    for (int i = 0; i < desc->n_carts; ++i) h += 6 * (int64_t)desc->cart_len[i] * row * 4;
+    for (int i = 0; i < desc->n_carts; ++i) h += L * 6 * (int64_t)desc->cart_len[i] * row * 4;
     *host_bytes = (size_t)h;
   }
   return CAS_OK;
@@ -145,6 +147,8 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
   p->cart_len.assign(desc->cart_len, desc->cart_len + desc->n_carts);
   p->desc.cart_len = p->cart_len.data();
   p->tile = desc->tile_tokens ? desc->tile_tokens : 128;
+  p->n_layers = desc->n_layers ? desc->n_layers : 1;
+  p->desc.n_layers = p->n_layers;
   p->row_elems = (int64_t)desc->Hkv * desc->D;
   p->elem_bytes = desc->dtype == CAS_BF16 ? 2 : 4;
   layout_slots(desc, p->slot_base, p->slot_cap, p->pool_tokens);
@@ -155,7 +159,8 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
   p->cart_in.assign(desc->n_slots, -1);
   for (int s = 0; s < desc->n_slots; ++s) { p->slot_of[s] = s; p->cart_in[s] = s; }
   p->in_transit.assign(desc->n_carts, 0);
-  p->grad_dirty.assign(desc->n_slots, 0);
+  p->grad_dirty.assign((size_t)p->n_layers * desc->n_slots, 0);
+  p->layers.assign(p->n_layers, PoolLayer());
   p->opt_steps.assign(desc->n_carts, 0);
   p->last_used.assign(desc->n_carts, -1);
   p->dev = (char*)dev_arena;
@@ -163,12 +168,16 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
   p->side = (cudaStream_t)side_stream;
   if (p->dev) {
     Carve c = carve(p->pool_tokens, p->row_elems, p->elem_bytes);
-    p->pool_K = p->dev + c.off_K;
-    p->pool_V = p->dev + c.off_V;
-    p->grad_K = (float*)(p->dev + c.off_gK);
-    p->grad_V = (float*)(p->dev + c.off_gV);
-    p->state = (float*)(p->dev + c.off_state);
-    cudaError_t e = cudaMemsetAsync(p->dev, 0, (size_t)c.total, p->side);
+    for (int l = 0; l < p->n_layers; ++l) {        // the same carving repeated per layer
+      char* base = p->dev + (int64_t)l * c.total;
+      PoolLayer& L = p->layers[l];
+      L.pool_K = base + c.off_K;
+      L.pool_V = base + c.off_V;
+      L.grad_K = (float*)(base + c.off_gK);
+      L.grad_V = (float*)(base + c.off_gV);
+      L.state = (float*)(base + c.off_state);
+    }
+    cudaError_t e = cudaMemsetAsync(p->dev, 0, (size_t)c.total * p->n_layers, p->side);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->side);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_main, cudaEventDisableTiming);
@@ -224,11 +233,12 @@ int cas_pool_destroy(cas_pool* p) {
 
 int cas_pool_layout_get(const cas_pool* p, cas_pool_layout* out) {
   if (!p || !out) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
-  out->pool_K = p->pool_K;
-  out->pool_V = p->pool_V;
-  out->grad_K = p->grad_K;
-  out->grad_V = p->grad_V;
-  out->state = p->state;
+  const PoolLayer L0 = p->layers.empty() ? PoolLayer() : p->layers[0];
+  out->pool_K = L0.pool_K;
+  out->pool_V = L0.pool_V;
+  out->grad_K = L0.grad_K;
+  out->grad_V = L0.grad_V;
+  out->state = L0.state;
   out->slot_base = p->slot_base.data();
   out->slot_cap = p->slot_cap.data();
   out->pool_tokens = p->pool_tokens;
@@ -241,63 +251,70 @@ static int need_data(const cas_pool* p) {
   return CAS_OK;
 }
 
-int cas_pool_load(cas_pool* p, int32_t cart, const float* K, const float* V) {
+int cas_pool_load_layer(cas_pool* p, int32_t layer, int32_t cart, const float* K, const float* V) {
   int rc = need_data(p);
   if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
   if (cart < 0 || cart >= p->desc.n_carts || !K || !V) { set_error("bad cart / null data"); return CAS_ERR_INVALID_ARG; }
   if (p->in_transit[cart]) { set_error("cartridge %d in transit", cart); return CAS_ERR_BUSY; }
   const int64_t n = (int64_t)p->cart_len[cart] * p->row_elems;
   const int s = p->slot_of[cart];
+  const PoolLayer& L = p->layers[layer];
   if (s >= 0) {
     CAS_CUDA(cudaStreamSynchronize(p->side));
-    CAS_CUDA(cudaMemcpy(p->slot_state(s, 0), K, n * 4, cudaMemcpyHostToDevice));
-    CAS_CUDA(cudaMemcpy(p->slot_state(s, 1), V, n * 4, cudaMemcpyHostToDevice));
-    for (int w = 2; w < 6; ++w) CAS_CUDA(cudaMemsetAsync(p->slot_state(s, w), 0, n * 4, p->side));
+    CAS_CUDA(cudaMemcpy(p->slot_state(layer, s, 0), K, n * 4, cudaMemcpyHostToDevice));
+    CAS_CUDA(cudaMemcpy(p->slot_state(layer, s, 1), V, n * 4, cudaMemcpyHostToDevice));
+    for (int w = 2; w < 6; ++w) CAS_CUDA(cudaMemsetAsync(p->slot_state(layer, s, w), 0, n * 4, p->side));
     const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
-    rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
-                        (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, n,
-                        p->desc.dtype, p->side);
+    rc = launch_refresh(p->slot_state(layer, s, 0), p->slot_state(layer, s, 1), (char*)L.pool_K + o * p->elem_bytes,
+                        (char*)L.pool_V + o * p->elem_bytes, L.grad_K + o, L.grad_V + o, n, p->desc.dtype, p->side);
     if (rc) return rc;
     CAS_CUDA(cudaStreamSynchronize(p->side));
-    p->grad_dirty[s] = 0;
+    p->grad_dirty[(size_t)layer * p->desc.n_slots + s] = 0;
   } else {
     if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
     CAS_CUDA(cudaStreamSynchronize(p->side));
-    memcpy(p->home(cart, 0), K, n * 4);
-    memcpy(p->home(cart, 1), V, n * 4);
-    memset(p->home(cart, 2), 0, 4 * n * 4);
+    memcpy(p->home(cart, layer, 0), K, n * 4);
+    memcpy(p->home(cart, layer, 1), V, n * 4);
+    memset(p->home(cart, layer, 2), 0, 4 * n * 4);
   }
   return CAS_OK;
 }
 
-int cas_pool_read(cas_pool* p, int32_t cart, int32_t what, void* out) {
+int cas_pool_load(cas_pool* p, int32_t cart, const float* K, const float* V) { return cas_pool_load_layer(p, 0, cart, K, V); }
+
+int cas_pool_read_layer(cas_pool* p, int32_t layer, int32_t cart, int32_t what, void* out) {
   int rc = need_data(p);
   if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
   if (cart < 0 || cart >= p->desc.n_carts || what < 0 || what > 9 || !out) { set_error("bad args"); return CAS_ERR_INVALID_ARG; }
   const int64_t n = (int64_t)p->cart_len[cart] * p->row_elems;
   const int s = p->slot_of[cart];
+  const PoolLayer& L = p->layers[layer];
   CAS_CUDA(cudaDeviceSynchronize());
   if (what < 6) {
     if (s >= 0 && p->in_transit[cart] != 2) {
-      CAS_CUDA(cudaMemcpy(out, p->slot_state(s, what), n * 4, cudaMemcpyDeviceToHost));
+      CAS_CUDA(cudaMemcpy(out, p->slot_state(layer, s, what), n * 4, cudaMemcpyDeviceToHost));
     } else {
       if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
-      memcpy(out, p->home(cart, what), n * 4);
+      memcpy(out, p->home(cart, layer, what), n * 4);
     }
     return CAS_OK;
   }
   if (s < 0) { set_error("cartridge %d not resident", cart); return CAS_ERR_NOT_RESIDENT; }
   const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
-  if ((what == 6 || what == 7) && !p->grad_dirty[s]) {   // a clean slot's buffer is undefined: its gradient is zero
-    memset(out, 0, (size_t)n * 4);
+  if ((what == 6 || what == 7) && !p->grad_dirty[(size_t)layer * p->desc.n_slots + s]) {
+    memset(out, 0, (size_t)n * 4);   // a clean slot's buffer is undefined: its gradient is zero
     return CAS_OK;
   }
-  if (what == 6) CAS_CUDA(cudaMemcpy(out, p->grad_K + o, n * 4, cudaMemcpyDeviceToHost));
-  if (what == 7) CAS_CUDA(cudaMemcpy(out, p->grad_V + o, n * 4, cudaMemcpyDeviceToHost));
-  if (what == 8) CAS_CUDA(cudaMemcpy(out, (char*)p->pool_K + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
-  if (what == 9) CAS_CUDA(cudaMemcpy(out, (char*)p->pool_V + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
+  if (what == 6) CAS_CUDA(cudaMemcpy(out, L.grad_K + o, n * 4, cudaMemcpyDeviceToHost));
+  if (what == 7) CAS_CUDA(cudaMemcpy(out, L.grad_V + o, n * 4, cudaMemcpyDeviceToHost));
+  if (what == 8) CAS_CUDA(cudaMemcpy(out, (char*)L.pool_K + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
+  if (what == 9) CAS_CUDA(cudaMemcpy(out, (char*)L.pool_V + o * p->elem_bytes, n * p->elem_bytes, cudaMemcpyDeviceToHost));
   return CAS_OK;
 }
+
+int cas_pool_read(cas_pool* p, int32_t cart, int32_t what, void* out) { return cas_pool_read_layer(p, 0, cart, what, out); }
 
 int cas_pool_counters(const cas_pool* p, int32_t* slot_of, int32_t* cart_in, int64_t* opt_steps,
                       int64_t* last_used, int32_t* in_transit, int32_t* grad_dirty) {
@@ -308,7 +325,7 @@ int cas_pool_counters(const cas_pool* p, int32_t* slot_of, int32_t* cart_in, int
   if (opt_steps) memcpy(opt_steps, p->opt_steps.data(), N * 8);
   if (last_used) memcpy(last_used, p->last_used.data(), N * 8);
   if (in_transit) memcpy(in_transit, p->in_transit.data(), N * 4);
-  if (grad_dirty) memcpy(grad_dirty, p->grad_dirty.data(), S * 4);
+  if (grad_dirty) for (int s2 = 0; s2 < S; ++s2) grad_dirty[s2] = p->any_dirty(s2) ? 1 : 0;   // any layer
   return CAS_OK;
 }
 
@@ -514,8 +531,12 @@ int cas_slot_table_destroy(cas_slot_table* t) {
     else if (t->used) cudaDeviceSynchronize();
     t->pool->tab_free.push_back(t->blob);
   }
-  if (t->d_dec_blob) cudaDeviceSynchronize();
-  if (t->d_dec_blob) cudaFree(t->d_dec_blob);
+  if (t->d_dec_blob) {
+    cudaDeviceSynchronize();
+    cudaFree(t->d_dec_blob);
+    cudaFreeHost(t->h_dec_blob);
+  }
+  if (t->dec_ready) cudaEventDestroy(t->dec_ready);
   delete t;
   return CAS_OK;
 }
@@ -595,10 +616,11 @@ static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) 
   return ok;
 }
 
-int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
-                        const void* Vs, float scale, void* O, float* LSE, void* stream) {
+int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                              const void* Ks, const void* Vs, float scale, void* O, float* LSE, void* stream) {
   int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
   rc = table_on_stream(t, stream);
   if (rc) return rc;
   if (!Q || !O || !LSE) { set_error("null Q/O/LSE"); return CAS_ERR_INVALID_ARG; }
@@ -606,10 +628,71 @@ int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   a.pool = p; a.tab = t; a.Hq = Hq; a.Hkv = p->desc.Hkv; a.D = p->desc.D; a.dtype = p->desc.dtype;
   a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O_out = O; a.LSE_out = LSE; a.scale = scale;
   a.stream = (cudaStream_t)stream;
+  a.layer = layer; a.L = &p->layers[layer];
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
-  if (tc && tc_decode_supported(p, t, Hq)) return tc_decode_fwd(a);
+  if (tc && tc_decode_supported(p, t, Hq)) {
+    // one query token per sequence whose only self key is itself: the decode kernel with a 1-token "cache"
+    const std::vector<int32_t> ones(t->B, 1);
+    return tc_decode_fwd(a, Ks, Vs, 1, ones.data());
+  }
   return tc ? tc_attn_fwd(a) : simt_attn_fwd(a);
+}
+
+int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
+                        const void* Vs, float scale, void* O, float* LSE, void* stream) {
+  return cas_prefix_attn_fwd_layer(p, t, 0, Hq, Q, Ks, Vs, scale, O, LSE, stream);
+}
+
+int cas_decode_attn_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                          const void* K_cache, const void* V_cache, int32_t cache_cap, const int32_t* self_len,
+                          float scale, void* O, float* LSE, void* stream) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
+  if (!t || t->pool != p) { set_error("table does not belong to this pool"); return CAS_ERR_INVALID_ARG; }
+  if (Hq < 1 || Hq % p->desc.Hkv) { set_error("Hq must be a positive multiple of Hkv"); return CAS_ERR_SHAPE; }
+  if (!(scale > 0.f) || !std::isfinite(scale)) { set_error("scale must be positive and finite"); return CAS_ERR_INVALID_ARG; }
+  if (!Q || !O || !LSE) { set_error("null Q/O/LSE"); return CAS_ERR_INVALID_ARG; }
+  if ((K_cache == nullptr) != (V_cache == nullptr)) { set_error("K_cache and V_cache: both or none"); return CAS_ERR_INVALID_ARG; }
+  if (K_cache && (!self_len || cache_cap < 1)) { set_error("a self cache needs self_len and cache_cap >= 1"); return CAS_ERR_INVALID_ARG; }
+  if (t->max_lq != 1) { set_error("cas_decode_attn needs one query token per sequence"); return CAS_ERR_SHAPE; }
+  for (int k = 0; k < t->nsel; ++k) {
+    const int c = t->sel_cart[k];
+    if (p->slot_of[c] != t->sel_slot[k] || p->in_transit[c]) { set_error("stale slot table (cartridge %d moved)", c); return CAS_ERR_NOT_RESIDENT; }
+  }
+  if (!tc_decode_supported(p, t, Hq)) { set_error("cas_decode_attn needs a bf16 pool with D = 128"); return CAS_ERR_SHAPE; }
+  rc = table_on_stream(t, stream);
+  if (rc) return rc;
+  AttnArgs a{};
+  a.pool = p; a.tab = t; a.Hq = Hq; a.Hkv = p->desc.Hkv; a.D = p->desc.D; a.dtype = p->desc.dtype;
+  a.Q = Q; a.O_out = O; a.LSE_out = LSE; a.scale = scale;
+  a.stream = (cudaStream_t)stream;
+  a.layer = layer; a.L = &p->layers[layer];
+  return tc_decode_fwd(a, K_cache, V_cache, cache_cap, self_len);
+}
+
+int cas_decode_attn(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* K_cache,
+                    const void* V_cache, int32_t cache_cap, const int32_t* self_len, float scale, void* O, float* LSE,
+                    void* stream) {
+  return cas_decode_attn_layer(p, t, 0, Hq, Q, K_cache, V_cache, cache_cap, self_len, scale, O, LSE, stream);
+}
+
+// PAPER.md:142 (sec. 3 Retrieval): "we map each retrieved chunk to a document id, which in turn is associated with a
+// cartridge.  The final list contains the unique cartridge ids in the order of their retrieval."
+int cas_select_retrieved(const int32_t* chunk_ids, int32_t k, const int32_t* chunk_to_cart, int32_t n_chunks,
+                         int32_t max_carts, int32_t* out_carts, int32_t* n_out) {
+  if (k < 0 || (k && !chunk_ids) || !chunk_to_cart || n_chunks < 0 || !out_carts || !n_out || max_carts < 0) { set_error("bad args"); return CAS_ERR_INVALID_ARG; }
+  int n = 0;
+  for (int i = 0; i < k && n < max_carts; ++i) {
+    if (chunk_ids[i] < 0 || chunk_ids[i] >= n_chunks) { set_error("chunk id %d out of range", chunk_ids[i]); return CAS_ERR_INVALID_ARG; }
+    const int32_t c = chunk_to_cart[chunk_ids[i]];
+    bool seen = false;
+    for (int j = 0; j < n; ++j) seen |= out_carts[j] == c;
+    if (!seen) out_carts[n++] = c;
+  }
+  *n_out = n;
+  return CAS_OK;
 }
 
 int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* p, const cas_slot_table* t, int32_t Hq, size_t* bytes) {
@@ -618,11 +701,14 @@ int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* p, const cas_slot_table*
   return CAS_OK;
 }
 
-int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
-                        const void* Vs, const void* O, const float* LSE, const void* dO, float scale,
-                        void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes, void* stream) {
+int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                              const void* Ks, const void* Vs, const void* O, const float* LSE, const void* dO,
+                              float scale, void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes,
+                              void* stream) {
   int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
+  int32_t* dirty = p->grad_dirty.data() + (size_t)layer * p->desc.n_slots;
   rc = table_on_stream(t, stream);
   if (rc) return rc;
   if (!Q || !O || !LSE || !dO || !dQ) { set_error("null Q/O/LSE/dO/dQ"); return CAS_ERR_INVALID_ARG; }
@@ -635,21 +721,29 @@ int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O = O; a.LSE_in = LSE; a.dO = dO; a.dQ = dQ; a.dKs = dKs; a.dVs = dVs;
   a.scale = scale; a.workspace = workspace; a.workspace_bytes = workspace_bytes;
   a.stream = (cudaStream_t)stream;
+  a.layer = layer; a.L = &p->layers[layer];
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
   if (!tc) {
     // the CUDA-core path accumulates read-modify-write: give the clean slots it is about to touch real zeros
     for (int sl : t->used_slots)
-      if (!p->grad_dirty[sl]) {
+      if (!dirty[sl]) {
         const int64_t o = (int64_t)p->slot_base[sl] * p->row_elems, nb = (int64_t)p->slot_cap[sl] * p->row_elems * 4;
-        CAS_CUDA(cudaMemsetAsync(p->grad_K + o, 0, nb, (cudaStream_t)stream));
-        CAS_CUDA(cudaMemsetAsync(p->grad_V + o, 0, nb, (cudaStream_t)stream));
+        CAS_CUDA(cudaMemsetAsync(a.L->grad_K + o, 0, nb, (cudaStream_t)stream));
+        CAS_CUDA(cudaMemsetAsync(a.L->grad_V + o, 0, nb, (cudaStream_t)stream));
       }
   }
   rc = tc ? tc_attn_bwd(a) : simt_attn_bwd(a);
   if (rc) return rc;
-  for (int s : t->used_slots) p->grad_dirty[s] = 1;
+  for (int s2 : t->used_slots) dirty[s2] = 1;
   return CAS_OK;
+}
+
+int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
+                        const void* Vs, const void* O, const float* LSE, const void* dO, float scale,
+                        void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes, void* stream) {
+  return cas_prefix_attn_bwd_layer(p, t, 0, Hq, Q, Ks, Vs, O, LSE, dO, scale, dQ, dKs, dVs, workspace, workspace_bytes,
+                                   stream);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -676,32 +770,39 @@ int cas_adam_step(cas_pool* p, const cas_adam_cfg* cfg, const int32_t* slots, in
     if (p->cart_in[s] < 0) { set_error("slot %d is empty", s); return CAS_ERR_NOT_RESIDENT; }
     if (p->in_transit[p->cart_in[s]]) { set_error("slot %d in transit", s); return CAS_ERR_BUSY; }
   }
-  const int cnt = (int)list.size();
+  const int cnt = (int)list.size(), S = p->desc.n_slots;
   if (p->dev && cnt) {
-    std::vector<AdamSlotDesc> h(cnt);
-    for (int i = 0; i < cnt; ++i) {
-      const int s = list[i], c = p->cart_in[s];
-      const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
-      const double t = (double)(p->opt_steps[c] + 1);
-      h[i].state = p->slot_state(s, 0);
-      h[i].wK = (char*)p->pool_K + o * p->elem_bytes;
-      h[i].wV = (char*)p->pool_V + o * p->elem_bytes;
-      h[i].gK = p->grad_K + o;
-      h[i].gV = p->grad_V + o;
-      h[i].cap_elems = (int64_t)p->slot_cap[s] * p->row_elems;
-      h[i].n_elems = (int64_t)p->cart_len[c] * p->row_elems;
-      h[i].frozen_elems = std::min<int64_t>(cfg->n_frozen, p->cart_len[c]) * p->row_elems;
-      h[i].step_size_scale = lr_scale ? lr_scale[i] : 1.0f;
-      h[i].bc1 = (float)(1.0 - pow((double)cfg->beta1, t));
-      h[i].bc2 = (float)(1.0 - pow((double)cfg->beta2, t));
-      h[i].has_grad = p->grad_dirty[s] ? 1 : 0;
+    // every layer of every listed slot in one go (PAPER.md:42: a cartridge is Z in R^{L x p x d x 2}; :85 one step count
+    // and one lr scale per cartridge, not per layer)
+    std::vector<AdamSlotDesc> h((size_t)cnt * p->n_layers);
+    for (int l = 0; l < p->n_layers; ++l) {
+      const PoolLayer& L = p->layers[l];
+      for (int i = 0; i < cnt; ++i) {
+        const int s = list[i], c = p->cart_in[s];
+        const int64_t o = (int64_t)p->slot_base[s] * p->row_elems;
+        const double t = (double)(p->opt_steps[c] + 1);
+        AdamSlotDesc& d = h[(size_t)l * cnt + i];
+        d.state = p->slot_state(l, s, 0);
+        d.wK = (char*)L.pool_K + o * p->elem_bytes;
+        d.wV = (char*)L.pool_V + o * p->elem_bytes;
+        d.gK = L.grad_K + o;
+        d.gV = L.grad_V + o;
+        d.cap_elems = (int64_t)p->slot_cap[s] * p->row_elems;
+        d.n_elems = (int64_t)p->cart_len[c] * p->row_elems;
+        d.frozen_elems = std::min<int64_t>(cfg->n_frozen, p->cart_len[c]) * p->row_elems;
+        d.step_size_scale = lr_scale ? lr_scale[i] : 1.0f;
+        d.bc1 = (float)(1.0 - pow((double)cfg->beta1, t));
+        d.bc2 = (float)(1.0 - pow((double)cfg->beta2, t));
+        d.has_grad = p->grad_dirty[(size_t)l * S + s] ? 1 : 0;
+      }
     }
-    int rc = launch_adam(h.data(), cnt, *cfg, p->desc.dtype, (cudaStream_t)stream);
+    int rc = launch_adam(h.data(), (int)h.size(), *cfg, p->desc.dtype, (cudaStream_t)stream);
     if (rc) return rc;
   }
   for (int s : list) {
     p->opt_steps[p->cart_in[s]] += 1;
-    if (cfg->zero_grad) p->grad_dirty[s] = 0;
+    if (cfg->zero_grad)
+      for (int l = 0; l < p->n_layers; ++l) p->grad_dirty[(size_t)l * S + s] = 0;
   }
   return CAS_OK;
 }
@@ -714,7 +815,7 @@ int cas_grad_zero(cas_pool* p, const int32_t* slots, int32_t n, void* stream) {
   else for (int s = 0; s < p->desc.n_slots; ++s) list.push_back(s);
   for (int s : list) {
     if (s < 0 || s >= p->desc.n_slots) { set_error("bad slot"); return CAS_ERR_INVALID_ARG; }
-    p->grad_dirty[s] = 0;   // clean = zero gradient; the buffer itself is overwritten by the next backward pass
+    for (int l = 0; l < p->n_layers; ++l) p->grad_dirty[(size_t)l * p->desc.n_slots + s] = 0;   // clean = zero gradient
   }
   return CAS_OK;
 }
@@ -779,15 +880,17 @@ int cas_plan_rotation(const cas_pool* p, int64_t step, int32_t n_in, int32_t n_o
 static int copy_cart(cas_pool* p, int c, int s, bool to_host, cudaStream_t st) {
   const int64_t n = (int64_t)p->cart_len[c] * p->row_elems;
   const cudaMemcpyKind kind = to_host ? cudaMemcpyDeviceToHost : cudaMemcpyHostToDevice;
-  if (p->cart_len[c] == p->slot_cap[s]) {   // the six tensors are contiguous on both sides
-    void* d = p->slot_state(s, 0);
-    void* h = p->home(c, 0);
-    CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, 6 * n * 4, kind, st));
-  } else {
-    for (int w = 0; w < 6; ++w) {
-      void* d = p->slot_state(s, w);
-      void* h = p->home(c, w);
-      CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, n * 4, kind, st));
+  for (int l = 0; l < p->n_layers; ++l) {
+    if (p->cart_len[c] == p->slot_cap[s]) {   // the six tensors of a layer are contiguous on both sides
+      void* d = p->slot_state(l, s, 0);
+      void* h = p->home(c, l, 0);
+      CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, 6 * n * 4, kind, st));
+    } else {
+      for (int w = 0; w < 6; ++w) {
+        void* d = p->slot_state(l, s, w);
+        void* h = p->home(c, l, w);
+        CAS_CUDA(cudaMemcpyAsync(to_host ? h : d, to_host ? d : h, n * 4, kind, st));
+      }
     }
   }
   return CAS_OK;
@@ -801,7 +904,7 @@ int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t st
     if (c < 0 || c >= p->desc.n_carts || s < 0 || s >= p->desc.n_slots) { set_error("bad manifest entry"); return CAS_ERR_INVALID_ARG; }
     if (p->slot_of[c] != s) { set_error("cartridge %d is not in slot %d", c, s); return CAS_ERR_NOT_RESIDENT; }
     if (p->in_transit[c]) { set_error("cartridge %d already in transit", c); return CAS_ERR_BUSY; }
-    if (p->grad_dirty[s]) { set_error("slot %d has un-consumed gradients", s); return CAS_ERR_BUSY; }
+    if (p->any_dirty(s)) { set_error("slot %d has un-consumed gradients", s); return CAS_ERR_BUSY; }
     if (e[i].host_off != p->home_off[c] || e[i].nbytes != p->home_bytes(c)) { set_error("manifest bytes mismatch"); return CAS_ERR_INVALID_ARG; }
   }
   if (p->dev) {
@@ -863,10 +966,13 @@ int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t ste
     const int c = e[i].cart, s = e[i].slot;
     if (p->dev) {
       const int64_t o = (int64_t)p->slot_base[s] * p->row_elems, nel = (int64_t)p->cart_len[c] * p->row_elems;
-      int rc = launch_refresh(p->slot_state(s, 0), p->slot_state(s, 1), (char*)p->pool_K + o * p->elem_bytes,
-                              (char*)p->pool_V + o * p->elem_bytes, p->grad_K + o, p->grad_V + o, nel,
-                              p->desc.dtype, p->side_in);
-      if (rc) return rc;
+      for (int l = 0; l < p->n_layers; ++l) {
+        const PoolLayer& L = p->layers[l];
+        int rc = launch_refresh(p->slot_state(l, s, 0), p->slot_state(l, s, 1), (char*)L.pool_K + o * p->elem_bytes,
+                                (char*)L.pool_V + o * p->elem_bytes, L.grad_K + o, L.grad_V + o, nel, p->desc.dtype,
+                                p->side_in);
+        if (rc) return rc;
+      }
     }
     p->in_transit[c] = 2;
     p->pending.push_back({e[i], step});
@@ -929,6 +1035,7 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   int rc = need_data(p);
   if (rc) return rc;
   if (!t || !hQ || !hKs || !hVs || !hdO || !cfg || !hO || !hLSE || !hdQ || !scratch) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  if (p->n_layers != 1) { set_error("cas_train_step_host drives single-layer pools; use cas_train_step_layers"); return CAS_ERR_SHAPE; }
   if ((hdKs == nullptr) != (hdVs == nullptr)) { set_error("hdK_self / hdV_self: both or none"); return CAS_ERR_INVALID_ARG; }
   const StepScratch s = step_scratch(p, t, Hq);
   if (scratch_bytes < s.total) { set_error("scratch too small: need %zu", s.total); return CAS_ERR_CAPACITY; }
@@ -986,6 +1093,49 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   if (rc) return rc;
   CAS_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
   return CAS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// one optimizer step over all layers and several micro-batches (device buffers)
+// ---------------------------------------------------------------------------------------------
+int cas_train_step_layers_workspace_bytes(const cas_pool* p, const cas_slot_table* const* tables, int32_t n_micro,
+                                          int32_t Hq, size_t* bytes) {
+  if (!p || !tables || n_micro < 1 || !bytes) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  size_t mx = 0;
+  for (int m = 0; m < n_micro; ++m) {
+    size_t b = 0;
+    int rc = cas_prefix_attn_bwd_workspace_bytes(p, tables[m], Hq, &b);
+    if (rc) return rc;
+    mx = std::max(mx, b);
+  }
+  *bytes = mx;
+  return CAS_OK;
+}
+
+int cas_train_step_layers(cas_pool* p, const cas_slot_table* const* tables, int32_t n_micro, int32_t Hq,
+                          const cas_layer_io* io, float scale, const cas_adam_cfg* cfg, const float* lr_scale,
+                          void* workspace, size_t workspace_bytes, void* stream) {
+  int rc = need_data(p);
+  if (rc) return rc;
+  if (!tables || n_micro < 1 || !io || !cfg) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  const int L = p->n_layers;
+  for (int m = 0; m < n_micro; ++m) {
+    const cas_slot_table* t = tables[m];
+    // forward through the layer stack, then backward in reverse order: the order a model visits its layers in
+    for (int l = 0; l < L; ++l) {
+      const cas_layer_io& x = io[(size_t)m * L + l];
+      rc = cas_prefix_attn_fwd_layer(p, t, l, Hq, x.Q, x.K_self, x.V_self, scale, x.O, x.LSE, stream);
+      if (rc) return rc;
+    }
+    for (int l = L - 1; l >= 0; --l) {
+      const cas_layer_io& x = io[(size_t)m * L + l];
+      rc = cas_prefix_attn_bwd_layer(p, t, l, Hq, x.Q, x.K_self, x.V_self, x.O, x.LSE, x.dO, scale, x.dQ, x.dK_self,
+                                     x.dV_self, workspace, workspace_bytes, stream);
+      if (rc) return rc;
+    }
+  }
+  // ONE Adam step consumes the gradients every micro-batch has accumulated into the slots of every layer
+  return cas_adam_step(p, cfg, nullptr, 0, lr_scale, stream);
 }
 
 }  // extern "C"

@@ -51,15 +51,17 @@ struct FwdItem {
   int32_t cost;
 };
 
-// Decode work item (cas_tc_decode.cu): one row block (<= 128/G sequences with the same selection
-// group) x one chunk of that group's KV tiles.
-struct DecItem {
-  int32_t seq_off;   // into dec_seqs
-  int32_t n_seqs;
-  int32_t tile_off;  // into dec_tiles
+// Decode segment (cas_tc_decode.cu): one run of KV tiles for one row block (<= 128/G sequences with the same
+// selection group, or ONE sequence's self cache) and one KV head; a persistent CTA walks a list of them.
+struct DecSeg {
+  int32_t kind;      // 0 = pool tiles (dec_tiles[tile_off ..]), 1 = self cache of sequence seq_off, -1 = stop
+  int32_t tile_off;
   int32_t n_tiles;
-  int32_t row_off;   // first partial row of this item, in units of sequences (x G rows per sequence)
-  int32_t pad[3];
+  int32_t g;         // KV head
+  int32_t seq_off;   // into dec_seqs (kind 0) / the sequence id (kind 1)
+  int32_t n_seqs;
+  int32_t part_row;  // first partial row of this segment, in units of sequences (x G rows per sequence)
+  int32_t self_len;  // kind 1: keys in the cache
 };
 
 }  // namespace cas
@@ -73,6 +75,16 @@ struct TabBlob {
   size_t cap = 0;
   cudaEvent_t done = nullptr, ready = nullptr;
   bool has_done = false;
+};
+
+// One layer of the pool (Z in R^{L x p x d x 2} has a layer axis): the same slot layout repeated.
+struct PoolLayer {
+  void* pool_K = nullptr;
+  void* pool_V = nullptr;
+  float* grad_K = nullptr;
+  float* grad_V = nullptr;
+  float* state = nullptr;
+  CUtensorMap tm_K, tm_V;        // [pool_tokens, Hkv, 128] bf16, 128-token boxes (bf16, D == 128 only)
 };
 
 // Layout of cas_train_step_host's device scratch (byte offsets of the staged inputs, outputs and workspace).
@@ -89,18 +101,16 @@ struct cas_pool {
   std::vector<int32_t> slot_base, slot_cap;
   int64_t pool_tokens = 0;
   std::vector<int64_t> home_off;
-  std::vector<int32_t> slot_of, cart_in, in_transit, grad_dirty;
+  std::vector<int32_t> slot_of, cart_in, in_transit;
+  std::vector<int32_t> grad_dirty;   // [n_layers * n_slots], layer-major
   std::vector<int64_t> opt_steps, last_used;
   std::vector<cas::Pending> pending;
   // data (caller-owned arenas)
   char* dev = nullptr;
   char* pinned = nullptr;
   cudaStream_t side = nullptr;
-  void* pool_K = nullptr;
-  void* pool_V = nullptr;
-  float* grad_K = nullptr;
-  float* grad_V = nullptr;
-  float* state = nullptr;
+  int n_layers = 1;
+  std::vector<PoolLayer> layers;
   cudaEvent_t ev_side = nullptr, ev_main = nullptr;
   // arrivals (H2D) run on a second, library-owned stream so that they overlap the evictions (D2H) on
   // the caller's side stream (full-duplex host link); ev_slot[s] orders an arrival after the eviction
@@ -117,16 +127,20 @@ struct cas_pool {
   void* step_prev_scratch = nullptr;     // scratch / stream of the previous cas_train_step_host call
   cudaStream_t step_prev_stream = nullptr;
   StepScratch step_prev_layout{};
-  // TMA descriptors over the working copy (bf16, D==128 only)
-  bool has_tma = false;
-  CUtensorMap tm_K, tm_V;
+  bool has_tma = false;              // TMA descriptors over the working copies exist (bf16, D==128 only)
 
-  float* slot_state(int s, int which) const {  // which: 0..5 = pK,pV,mK,mV,vK,vV
-    return state + 6 * (int64_t)slot_base[s] * row_elems + (int64_t)which * slot_cap[s] * row_elems;
+  float* slot_state(int l, int s, int which) const {  // which: 0..5 = pK,pV,mK,mV,vK,vV
+    return layers[l].state + 6 * (int64_t)slot_base[s] * row_elems + (int64_t)which * slot_cap[s] * row_elems;
   }
-  int64_t home_bytes(int c) const { return 6 * (int64_t)cart_len[c] * row_elems * 4; }
-  float* home(int c, int which) const {
-    return (float*)(pinned + home_off[c]) + (int64_t)which * cart_len[c] * row_elems;
+  // pinned home of cartridge c: n_layers x six fp32 tensors of cart_len*Hkv*D elements, layer-major
+  int64_t home_layer_bytes(int c) const { return 6 * (int64_t)cart_len[c] * row_elems * 4; }
+  int64_t home_bytes(int c) const { return n_layers * home_layer_bytes(c); }
+  float* home(int c, int l, int which) const {
+    return (float*)(pinned + home_off[c] + l * home_layer_bytes(c)) + (int64_t)which * cart_len[c] * row_elems;
+  }
+  bool any_dirty(int s) const {
+    for (int l = 0; l < n_layers; ++l) if (grad_dirty[(size_t)l * desc.n_slots + s]) return true;
+    return false;
   }
 };
 
@@ -156,13 +170,17 @@ struct cas_slot_table {
   cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
   cas::BwdItem* d_bwd_items = nullptr;
   int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
-  // decode-shaped batches: split-KV work items, built lazily for a given Hq by cas_tc_decode.cu
+  // decode-shaped batches: segments of the persistent split-KV kernel, built lazily for a given Hq by cas_tc_decode.cu
   int32_t dec_Hq = 0;
-  int64_t dec_rows = 0;                       // partial rows per KV head = dec_seq_rows * G
-  std::vector<cas::DecItem> dec_items;
+  int64_t dec_rows = 0;                       // partial rows per KV head (prefix segments + one self row per sequence) x G
+  int32_t dec_grid = 0, dec_self_row_base = 0, dec_n_segs = 0;
+  std::vector<int32_t> dec_comb_off;          // [B+1] prefix partials per sequence
   char* d_dec_blob = nullptr;
-  cas::DecItem* d_dec_items = nullptr;
-  int32_t *d_dec_seqs = nullptr, *d_comb_off = nullptr, *d_comb_row = nullptr;
+  char* h_dec_blob = nullptr;                 // pinned mirror of the lists (asynchronous upload)
+  cudaEvent_t dec_ready = nullptr;
+  cas::DecSeg* d_dec_segs = nullptr;
+  int32_t *d_dec_cta_off = nullptr, *d_dec_seqs = nullptr, *d_comb_off = nullptr, *d_comb_row = nullptr,
+          *d_dec_cnt = nullptr, *d_dec_ticket = nullptr;
   cas::KvTile* d_dec_tiles = nullptr;
   float* d_dec_part = nullptr;
 };
@@ -179,6 +197,8 @@ struct SlotMask {
 
 struct AttnArgs {
   const cas_pool* pool;
+  const PoolLayer* L;            // the layer this call works on
+  int layer;
   const cas_slot_table* tab;
   int Hq, Hkv, D, dtype;
   const void *Q, *Ks, *Vs, *O, *dO;
@@ -201,7 +221,7 @@ int tc_attn_bwd(const AttnArgs& a);
 size_t tc_bwd_workspace(const cas_slot_table* t, int Hq, int D);
 int tc_make_pool_maps(cas_pool* p);
 bool tc_decode_supported(const cas_pool* p, const cas_slot_table* t, int Hq);
-int tc_decode_fwd(const AttnArgs& a);
+int tc_decode_fwd(const AttnArgs& a, const void* Kc, const void* Vc, int cache_cap, const int32_t* self_len);
 
 // Adam / refresh / zero
 struct AdamSlotDesc {

@@ -287,7 +287,7 @@ static int run_fwd(const AttnArgs& a) {
               t->d_simt_items, t->d_bwd_items};
   dim3 grid((unsigned)t->simt_items.size(), (unsigned)a.Hq);
   simt_rowwise_kernel<T, D, 0><<<grid, 128, 0, a.stream>>>(
-      tab, (const T*)a.Q, (const T*)a.pool->pool_K, (const T*)a.pool->pool_V, (const T*)a.Ks, (const T*)a.Vs,
+      tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
       nullptr, nullptr, nullptr, (T*)a.O_out, a.LSE_out, a.Hq, a.Hkv, a.scale);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "simt fwd launch");
@@ -303,12 +303,12 @@ static int run_bwd(const AttnArgs& a) {
   delta_kernel<T><<<(unsigned)((rows * 32 + 255) / 256), 256, 0, a.stream>>>((const T*)a.O, (const T*)a.dO, delta, rows, D);
   dim3 grid((unsigned)t->simt_items.size(), (unsigned)a.Hq);
   simt_rowwise_kernel<T, D, 1><<<grid, 128, 0, a.stream>>>(
-      tab, (const T*)a.Q, (const T*)a.pool->pool_K, (const T*)a.pool->pool_V, (const T*)a.Ks, (const T*)a.Vs,
+      tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
       (const T*)a.dO, a.LSE_in, delta, (T*)a.dQ, nullptr, a.Hq, a.Hkv, a.scale);
   dim3 grid2((unsigned)(4 * t->bwd_items.size()), (unsigned)a.Hkv);
   simt_dkdv_kernel<T, D><<<grid2, 128, 0, a.stream>>>(
-      tab, (const T*)a.Q, (const T*)a.pool->pool_K, (const T*)a.pool->pool_V, (const T*)a.Ks, (const T*)a.Vs,
-      (const T*)a.dO, a.LSE_in, delta, a.pool->grad_K, a.pool->grad_V, (T*)a.dKs, (T*)a.dVs, a.Hq, a.Hkv, a.scale);
+      tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
+      (const T*)a.dO, a.LSE_in, delta, a.L->grad_K, a.L->grad_V, (T*)a.dKs, (T*)a.dVs, a.Hq, a.Hkv, a.scale);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "simt bwd launch");
 }

@@ -530,17 +530,18 @@ int tc_attn_bwd(const AttnArgs& a) {
     rc = make_thd_map(&tmVs, a.Vs, t->T, a.Hkv, 128);
     if (rc) return rc;
   } else {
-    tmKs = a.pool->tm_K;
-    tmVs = a.pool->tm_V;
+    tmKs = a.L->tm_K;
+    tmVs = a.L->tm_V;
   }
   BwdParams prm{t->d_seq_off, t->d_inv_off, t->d_inv_seq, t->d_qtile_off, t->d_bwd_items, auxL, auxD, dQacc,
-                a.pool->grad_K, a.pool->grad_V, (__nv_bfloat16*)a.dKs, (__nv_bfloat16*)a.dVs, (int64_t)nqt * 128,
+                a.L->grad_K, a.L->grad_V, (__nv_bfloat16*)a.dKs, (__nv_bfloat16*)a.dVs, (int64_t)nqt * 128,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale, a.scale * kLog2e};
   const unsigned grid = (unsigned)(t->bwd_items.size() * a.Hkv);
   SlotMask dirty{};
+  const int32_t* gd = a.pool->grad_dirty.data() + (size_t)a.layer * a.pool->desc.n_slots;   // this layer's flags
   for (int sl = 0; sl < a.pool->desc.n_slots; ++sl)
-    if (a.pool->grad_dirty[sl]) dirty.w[sl >> 5] |= 1u << (sl & 31);
-  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm, dirty);
+    if (gd[sl]) dirty.w[sl >> 5] |= 1u << (sl & 31);
+  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.L->tm_K, a.L->tm_V, tmKs, tmVs, prm, dirty);
   dq_convert_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
       dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows);
   cudaError_t e = cudaGetLastError();

@@ -1,21 +1,29 @@
-// Prefix-attention FORWARD for decode-shaped batches (every sequence has exactly ONE query token;
-// BASELINE.json configs[4], PAPER.md:111 inference over all loaded cartridges, :142 retrieval-selected
-// variant), bf16, head_dim 128, tcgen05 + TMEM + TMA.
+// Prefix-attention FORWARD for decode-shaped batches: every sequence has exactly ONE query token whose keys are
+// the selected cartridges (read in place from the pool) plus the sequence's own cache of self keys -- the tokens
+// generated so far ("2048 maximum completion tokens"; BASELINE.json configs[4]; PAPER.md:111 inference
+// over all loaded cartridges, :142 retrieval-selected variant).  bf16, head_dim 128, tcgen05 + TMEM + TMA.
 //
-// The work is HBM-bound (each K/V byte is used by G query heads of a few sequences), so the kernel
-// is organised to read every selected K/V tile from HBM as few times as possible and to keep every
-// SM streaming:
-//  * KV-stationary batching through the INVERTED slot table: slots with the same set of selecting
-//    sequences form a group; the rows of an MMA tile are (sequence, head-of-group) pairs -- up to
-//    128/G sequences x G heads -- so one pass over a K/V tile serves all of them (c5 "all loaded":
-//    64 sequences x 4 heads = two 128-row blocks share each tile; the second read hits L2).
-//  * split-KV: a group's tile list is cut into chunks so that the grid has a few CTAs per SM; each
-//    CTA writes an un-normalised partial (O, m, l) per row and decode_combine_kernel merges the
-//    partials of a (sequence, head) and adds the query's own key/value (the 1-token causal block).
-// CTA: warps 0-3 softmax (thread = row = TMEM lane), 4 TMA producer, 5 MMA issuer.
-// SMEM: Q tile 32 KB (gathered rows, written by the softmax warps) + 3-stage K/V ring 192 KB.
-// TMEM: S0 | S1 | O (fp32, 128 columns each); QK(j+1) is issued before PV(j) into the other S buffer.
+// The work is HBM-bound (each K/V byte is used by G query heads of a few sequences), so the kernel reads every
+// selected K/V tile from HBM as few times as possible and keeps every SM streaming:
+//  * KV-stationary batching through the INVERTED slot table: slots with the same set of selecting sequences form a
+//    group; the rows of an MMA tile are (sequence, head-of-group) pairs -- up to 128/G sequences x G heads -- so one
+//    pass over a K/V tile serves all of them.
+//  * PERSISTENT CTAs, one per SM.  The host cuts every (group, row block, KV head) tile list into segments of about
+//    total/#SM tiles and deals them to the CTAs in order (the row blocks that share a chunk of tiles run at the same
+//    time, so the second read of a tile hits L2); a CTA then draws the self-cache units -- one per (sequence, KV
+//    head), whose length is only known at launch -- from a device ticket counter, which also evens out the tail.
+//  * One segment = one (row block, KV head, run of tiles).  Two softmax warpgroups take alternate tiles (even tiles:
+//    S0/O0, odd tiles: S1/O1 in TMEM), each with its own running max and sum, so the exp work of tile j+1 overlaps
+//    the MMAs of tiles j and j+2; at the end of the segment the two accumulators are merged and written as ONE
+//    un-normalised partial (O, m, l) per row.
+//  * FUSED MERGE: every row (sequence, head) has a counter; the CTA that writes the row's last partial merges all of
+//    them (plus the few self keys of a young cache, dotted on the CUDA cores), normalises and writes O and LSE.
+//    No second launch.
+// Warps: 0-3 / 4-7 softmax warpgroups (thread = row = TMEM lane), 8 scheduler + TMA producer, 9 MMA issuer,
+// 10-11 query gather (the rows of the next segment while the current one drains).
+// SMEM: Q tile 32 KB + 3-stage K/V ring 192 KB.  TMEM (512 cols): S0 | S1 | O0 | O1.
 #include <algorithm>
+#include <cstring>
 #include <map>
 
 #include "cas_sm100.cuh"
@@ -24,44 +32,230 @@
 namespace cas {
 using namespace sm100;
 
-constexpr int kDecThreads = 192;
+constexpr int kDecThreads = 384;
 constexpr int kDecStages = 3;
+constexpr int kDescRing = 4;
+constexpr int kInlineSelf = 4;     // caches up to this length are dotted on the CUDA cores inside the merge
+constexpr int kMaxDecB = 1024;     // sequences per decode call with a self cache (their lengths travel as kernel parameters)
 constexpr uint32_t dT = 32768, dH = 16384;
 constexpr uint32_t dOffQ = 0, dOffKV = dT, dOffBar = dT + kDecStages * 2 * dT;
-constexpr uint32_t kDecSmem = dOffBar + 256;
-enum { D_KF = 0, D_KE = 3, D_VF = 6, D_VE = 9, D_SF = 12, D_PF = 14, D_QR = 16, D_OV = 17, D_OD = 18, D_N = 19 };
+enum { D_KF = 0, D_KE = 3, D_VF = 6, D_VE = 9, D_SF = 12, D_PF = 14, D_OV = 16, D_QF = 18, D_QE = 19, D_DF = 20, D_DE = 24, D_N = 28 };
+constexpr uint32_t dOffDesc = dOffBar + D_N * 8 + 32;                       // after the barriers and the TMEM slot
+constexpr uint32_t dOffML = dOffDesc + kDescRing * 32;                      // (m, l) of both warpgroups: 2 x 128 x 8 B
+constexpr uint32_t dOffFlag = dOffML + 2048;                                // "this row is complete": 128 x 4 B
+constexpr uint32_t kDecSmem = dOffFlag + 512;
+static_assert(kDecSmem <= 232448, "decode kernel shared memory");
+static_assert(sizeof(DecSeg) == 32, "descriptor ring entry");
 constexpr int kPartStride = 132;   // 128 O + m + l + pad (16-byte aligned rows)
 
+struct SelfLens {
+  int32_t v[kMaxDecB];
+};
+
 struct DecParams {
-  const DecItem* items;
+  const DecSeg* segs;
+  const int32_t* cta_seg_off;   // [grid + 1]
   const int32_t* seqs;          // row-block sequence lists
   const KvTile* tiles;
-  const int32_t* seq_off;
+  const int32_t* seq_off;       // packed token index of every sequence (one token each)
+  const int32_t* comb_off;      // [B + 1] partial rows (in units of sequences) of the prefix segments covering sequence b
+  const int32_t* comb_row;
   const __nv_bfloat16* Q;
+  const __nv_bfloat16 *Kc, *Vc; // self cache [B, cache_cap, Hkv, 128] or null
+  __nv_bfloat16* O;
+  float* LSE;
   float* part;
+  int32_t* cnt;                 // [Hkv * B * G] partials written per row so far (self-resetting)
+  int32_t* ticket;              // [2]: next self unit, CTAs done (self-resetting)
   int64_t rows_total;           // partial rows per KV head
-  int Hq, Hkv;
+  int32_t self_row_base;        // first partial row (in units of sequences) of the self units
+  int32_t cache_cap;
+  int B, Hq, Hkv;
   float scale_log2;
 };
 
+// A sequence's cache gets its own tensor-core segment when it is longer than the merge can dot inline, or when it is
+// the sequence's only source of keys (someone has to trigger the merge).
+__host__ __device__ __forceinline__ bool has_self_unit(int len, int n_prefix_partials) {
+  return len > kInlineSelf || (len > 0 && n_prefix_partials == 0);
+}
+
+// End of a segment (both softmax warpgroups, 256 threads): merge the two TMEM accumulators, write ONE partial per row,
+// count it, and -- for the rows whose last partial this was -- merge all partials of the row, normalise, write O / LSE.
+__device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const SelfLens& slen, const DecSeg d, const int w,
+                                                  const int r, const uint32_t tbase, const uint32_t lane_base,
+                                                  const float m, const float l, const int c0, const int c1,
+                                                  const uint32_t bar_ov, float2* ml, int32_t* flag) {
+  const int G = prm.Hq / prm.Hkv;
+  const int n = d.n_tiles;
+  // ---- segment epilogue: merge the two accumulators, write ONE partial per row
+  const int n0 = (n + 1) >> 1, n1 = n >> 1;
+  ml[w * 128 + r] = make_float2(m, l);
+  asm volatile("bar.sync 2, 256;" ::: "memory");                 // both warpgroups are past their last tile ...
+  if (n0) mbar_wait(bar_ov, (c0 - 1) & 1);                    // ... so these waits are at most one phase behind
+  if (n1) mbar_wait(bar_ov + 8, (c1 - 1) & 1);
+  tc_fence_after();
+  const float2 a = ml[r], b = ml[128 + r];
+  const float M = n1 ? fmaxf(a.x, b.x) : a.x;
+  const float f0 = ex2_approx(a.x - M), f1 = n1 ? ex2_approx(b.x - M) : 0.f;
+  const float L = f0 * a.y + f1 * b.y;
+  const int n_rows = d.n_seqs * G;
+  const int sj = r / G, hh = r % G;
+  const int seq = r < n_rows ? (d.kind == 0 ? prm.seqs[d.seq_off + sj] : d.seq_off) : 0;
+  float* prow = prm.part + ((int64_t)d.g * prm.rows_total + (int64_t)(d.part_row + sj) * G + hh) * kPartStride;
+  const uint32_t tO0 = tbase + 256 + lane_base + w * 64, tO1 = tO0 + 128;       // this thread: columns [64w, 64w + 64)
+#pragma unroll
+  for (int cc = 0; cc < 2; ++cc) {
+    uint32_t o0[32], o1[32];
+    tmem_ld32(tO0 + cc * 32, o0);
+    if (n1) tmem_ld32(tO1 + cc * 32, o1);
+    tc_wait_ld();
+    if (r < n_rows) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        float4 v;
+        v.x = f0 * __uint_as_float(o0[4 * i]); v.y = f0 * __uint_as_float(o0[4 * i + 1]);
+        v.z = f0 * __uint_as_float(o0[4 * i + 2]); v.w = f0 * __uint_as_float(o0[4 * i + 3]);
+        if (n1) {
+          v.x += f1 * __uint_as_float(o1[4 * i]); v.y += f1 * __uint_as_float(o1[4 * i + 1]);
+          v.z += f1 * __uint_as_float(o1[4 * i + 2]); v.w += f1 * __uint_as_float(o1[4 * i + 3]);
+        }
+        __stcg(reinterpret_cast<float4*>(prow + w * 64 + cc * 32 + 4 * i), v);
+      }
+    }
+  }
+  if (w == 0 && r < n_rows) __stcg(reinterpret_cast<float2*>(prow + 128), make_float2(M, L));
+  tc_fence_before();
+  __threadfence();
+  asm volatile("bar.sync 2, 256;" ::: "memory");
+  if (w == 0) {
+    int last = 0;
+    if (r < n_rows) {
+      const int len = prm.Kc ? slen.v[seq] : 0;
+      const int npre = prm.comb_off[seq + 1] - prm.comb_off[seq];
+      const int expected = npre + (has_self_unit(len, npre) ? 1 : 0);
+      last = atomicAdd(prm.cnt + ((int64_t)d.g * prm.B + seq) * G + hh, 1) == expected - 1;
+    }
+    flag[r] = last;
+  }
+  asm volatile("bar.sync 2, 256;" ::: "memory");
+  if (flag[r]) {
+    // ---- fused merge: this row's last partial has just been written
+    __threadfence();
+    const int h = d.g * G + hh;
+    const int e0 = prm.comb_off[seq], e1 = prm.comb_off[seq + 1];
+    const int len = prm.Kc ? slen.v[seq] : 0;
+    const bool self_unit = has_self_unit(len, e1 - e0);
+    const int n_inline = self_unit ? 0 : len;
+    const int64_t pbase = (int64_t)d.g * prm.rows_total * kPartStride;
+    auto part_row = [&](int e) {
+      const int pr = e < e1 ? prm.comb_row[e] : prm.self_row_base + seq;
+      return prm.part + pbase + ((int64_t)pr * G + hh) * kPartStride;
+    };
+    const int e_end = e1 + (self_unit ? 1 : 0);
+    const int64_t tq = prm.seq_off[seq];
+    float s_in[kInlineSelf];
+    float Mx = -INFINITY;
+    for (int e = e0; e < e_end; ++e) Mx = fmaxf(Mx, __ldcg(part_row(e) + 128));
+#pragma unroll
+    for (int i = 0; i < kInlineSelf; ++i) {
+      s_in[i] = -INFINITY;
+      if (i < n_inline) {
+        const uint4* qp = reinterpret_cast<const uint4*>(prm.Q + (tq * prm.Hq + h) * 128);
+        const uint4* kp = reinterpret_cast<const uint4*>(prm.Kc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + d.g) * 128);
+        float dot = 0.f;
+#pragma unroll 4
+        for (int x = 0; x < 16; ++x) {
+          const uint4 qa = qp[x], ka = kp[x];
+          const uint32_t qq[4] = {qa.x, qa.y, qa.z, qa.w}, kq[4] = {ka.x, ka.y, ka.z, ka.w};
+#pragma unroll
+          for (int y = 0; y < 4; ++y) {
+            const float2 qf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qq[y]));
+            const float2 kf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&kq[y]));
+            dot = fmaf(qf.x, kf.x, dot);
+            dot = fmaf(qf.y, kf.y, dot);
+          }
+        }
+        s_in[i] = dot * prm.scale_log2;
+        Mx = fmaxf(Mx, s_in[i]);
+      }
+    }
+    float acc[64];
+#pragma unroll
+    for (int i = 0; i < 64; ++i) acc[i] = 0.f;
+    float Ls = 0.f;
+    for (int e = e0; e < e_end; ++e) {
+      const float* p = part_row(e);
+      const float2 mlp = __ldcg(reinterpret_cast<const float2*>(p + 128));
+      const float f = ex2_approx(mlp.x - Mx);
+      Ls += f * mlp.y;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        const float4 v = __ldcg(reinterpret_cast<const float4*>(p + w * 64 + 4 * i));
+        acc[4 * i] += f * v.x; acc[4 * i + 1] += f * v.y; acc[4 * i + 2] += f * v.z; acc[4 * i + 3] += f * v.w;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < kInlineSelf; ++i) {
+      if (i < n_inline) {
+        const float f = ex2_approx(s_in[i] - Mx);
+        Ls += f;
+        const uint4* vp = reinterpret_cast<const uint4*>(prm.Vc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + d.g) * 128 + w * 64);
+#pragma unroll
+        for (int x = 0; x < 8; ++x) {
+          const uint4 va = vp[x];
+          const uint32_t vq[4] = {va.x, va.y, va.z, va.w};
+#pragma unroll
+          for (int y = 0; y < 4; ++y) {
+            const float2 vf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&vq[y]));
+            acc[8 * x + 2 * y] += f * vf.x;
+            acc[8 * x + 2 * y + 1] += f * vf.y;
+          }
+        }
+      }
+    }
+    const float inv = 1.f / Ls;
+    __nv_bfloat16* orow = prm.O + (tq * prm.Hq + h) * 128 + w * 64;
+#pragma unroll
+    for (int x = 0; x < 8; ++x) {
+      uint4 u;
+      u.x = pack_bf16(acc[8 * x] * inv, acc[8 * x + 1] * inv);
+      u.y = pack_bf16(acc[8 * x + 2] * inv, acc[8 * x + 3] * inv);
+      u.z = pack_bf16(acc[8 * x + 4] * inv, acc[8 * x + 5] * inv);
+      u.w = pack_bf16(acc[8 * x + 6] * inv, acc[8 * x + 7] * inv);
+      *reinterpret_cast<uint4*>(orow + 8 * x) = u;
+    }
+    if (w == 0) {
+      prm.LSE[tq * prm.Hq + h] = Mx * 0.6931471805599453f + logf(Ls);
+      prm.cnt[((int64_t)d.g * prm.B + seq) * G + hh] = 0;       // re-arm for the next launch on this table
+    }
+  }
+}
+
 __global__ void __launch_bounds__(kDecThreads, 1)
-tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV, const DecParams prm) {
+tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
+                 const __grid_constant__ CUtensorMap tmKc, const __grid_constant__ CUtensorMap tmVc,
+                 const __grid_constant__ DecParams prm, const __grid_constant__ SelfLens slen) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + dOffBar + D_N * 8);
   auto bar = [&](int i) { return sbase + dOffBar + 8u * i; };
-  const int warp = warp_id_uniform(), lane = threadIdx.x & 31;
-  const int g = blockIdx.x % prm.Hkv, G = prm.Hq / prm.Hkv;
-  const DecItem it = prm.items[blockIdx.x / prm.Hkv];
-  const KvTile* tiles = prm.tiles + it.tile_off;
-  const int n = it.n_tiles;
+  const DecSeg* dring = reinterpret_cast<const DecSeg*>(smem + dOffDesc);
+  const int warp = warp_id_uniform();
+  const int G = prm.Hq / prm.Hkv;
 
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();
-    for (int i = 0; i < D_N; ++i) mbar_init(bar(i), (i == D_PF || i == D_PF + 1 || i == D_QR) ? 128 : 1);
+    for (int i = 0; i < D_N; ++i) {
+      uint32_t c = 1;
+      if (i == D_PF || i == D_PF + 1) c = 128;
+      if (i == D_QF) c = 64;
+      if (i >= D_DE) c = 2;
+      mbar_init(bar(i), c);
+    }
     fence_mbar_init();
   }
-  if (warp == 4) {
+  if (warp == 8) {
     tmem_alloc(smem_u32(tmem_slot), 512);
     tmem_relinquish();
   }
@@ -69,257 +263,285 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
   __syncthreads();
   tc_fence_after();
   const uint32_t tbase = *tmem_slot;
-  const uint32_t tO = tbase + 256;
 
-  if (warp == 4) {
-    // ===================================================================== TMA producer
-    if (elect_one()) {
-      tma_prefetch_desc(&tmK);
-      tma_prefetch_desc(&tmV);
-      for (int j = 0; j < n; ++j) {
-        const int s = j % kDecStages;
-        const uint32_t ph = (j / kDecStages) & 1;
-        const uint32_t kb = sbase + dOffKV + s * 2 * dT, vb = kb + dT;
-        const int tok = tiles[j].tok;
-        mbar_wait(bar(D_KE + s), ph ^ 1);
-        mbar_expect_tx(bar(D_KF + s), dT);
-        tma_load_3d(kb, &tmK, bar(D_KF + s), 0, g, tok);
-        tma_load_3d(kb + dH, &tmK, bar(D_KF + s), 64, g, tok);
-        mbar_wait(bar(D_VE + s), ph ^ 1);
-        mbar_expect_tx(bar(D_VF + s), dT);
-        tma_load_3d(vb, &tmV, bar(D_VF + s), 0, g, tok);
-        tma_load_3d(vb + dH, &tmV, bar(D_VF + s), 64, g, tok);
-      }
-    }
-  } else if (warp == 5) {
-    // ===================================================================== MMA issuer
-    if (elect_one()) {
-      constexpr uint32_t idesc_qk = make_idesc(128, 128, 0, 0);
-      constexpr uint32_t idesc_pv = make_idesc(128, 128, 0, 1);
-      auto issue_qk = [&](int j) {
-        const uint32_t qa = sbase + dOffQ, ka = sbase + dOffKV + (j % kDecStages) * 2 * dT;
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-          const uint32_t o = (kk >> 2) * dH + (kk & 3) * 32;
-          mma_ss(tbase + (j & 1) * 128, desc_kmajor(qa + o), desc_kmajor(ka + o), idesc_qk, kk > 0);
+  if (warp >= 8) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
+    if (warp == 8) {
+      // ===================================================================== scheduler + TMA producer
+      if (elect_one()) {
+        tma_prefetch_desc(&tmK);
+        tma_prefetch_desc(&tmV);
+        DecSeg* wring = reinterpret_cast<DecSeg*>(smem + dOffDesc);
+        int nseg = 0, t = 0;
+        auto push = [&](const DecSeg& d) {
+          const int k = nseg & (kDescRing - 1);
+          mbar_wait(bar(D_DE + k), ((nseg / kDescRing) & 1) ^ 1);
+          wring[k] = d;
+          mbar_arrive(bar(D_DF + k));
+          ++nseg;
+          const CUtensorMap* mk = d.kind == 0 ? &tmK : &tmKc;
+          const CUtensorMap* mv = d.kind == 0 ? &tmV : &tmVc;
+          for (int j = 0; j < d.n_tiles; ++j, ++t) {
+            const int s = t % kDecStages;
+            const uint32_t ph = (t / kDecStages) & 1;
+            const uint32_t kb = sbase + dOffKV + s * 2 * dT, vb = kb + dT;
+            const int tok = d.kind == 0 ? prm.tiles[d.tile_off + j].tok : d.seq_off * prm.cache_cap + 128 * j;
+            mbar_wait(bar(D_KE + s), ph ^ 1);
+            mbar_expect_tx(bar(D_KF + s), dT);
+            tma_load_3d(kb, mk, bar(D_KF + s), 0, d.g, tok);
+            tma_load_3d(kb + dH, mk, bar(D_KF + s), 64, d.g, tok);
+            mbar_wait(bar(D_VE + s), ph ^ 1);
+            mbar_expect_tx(bar(D_VF + s), dT);
+            tma_load_3d(vb, mv, bar(D_VF + s), 0, d.g, tok);
+            tma_load_3d(vb + dH, mv, bar(D_VF + s), 64, d.g, tok);
+          }
+        };
+        for (int s = prm.cta_seg_off[blockIdx.x]; s < prm.cta_seg_off[blockIdx.x + 1]; ++s) push(prm.segs[s]);
+        if (prm.Kc != nullptr) {
+          // self-cache units, one per (sequence, KV head), drawn from the ticket counter
+          const int n_units = prm.B * prm.Hkv;
+          for (;;) {
+            const int u = atomicAdd(prm.ticket, 1);
+            if (u >= n_units) break;
+            const int b = u / prm.Hkv, g = u % prm.Hkv;
+            const int len = slen.v[b];
+            if (!has_self_unit(len, prm.comb_off[b + 1] - prm.comb_off[b])) continue;
+            push(DecSeg{1, 0, (len + 127) >> 7, g, b, 1, prm.self_row_base + b, len});
+          }
+          __threadfence();
+          if (atomicAdd(prm.ticket + 1, 1) == (int)gridDim.x - 1) {   // every CTA has left its ticket loop: re-arm
+            prm.ticket[0] = 0;
+            prm.ticket[1] = 0;
+          }
         }
-      };
-      mbar_wait(bar(D_QR), 0);
-      mbar_wait(bar(D_KF), 0);
-      tc_fence_after();
-      issue_qk(0);
-      mma_commit(bar(D_SF));
-      mma_commit(bar(D_KE));
-      for (int j = 0; j < n; ++j) {
-        if (j + 1 < n) {
-          const int s1 = (j + 1) % kDecStages;
-          mbar_wait(bar(D_KF + s1), ((j + 1) / kDecStages) & 1);
+        push(DecSeg{-1, 0, 0, 0, 0, 0, 0, 0});
+      }
+    } else if (warp == 9) {
+      // ===================================================================== MMA issuer
+      if (elect_one()) {
+        constexpr uint32_t idesc_qk = make_idesc(128, 128, 0, 0);
+        constexpr uint32_t idesc_pv = make_idesc(128, 128, 0, 1);
+        int t = 0, c0 = 0, c1 = 0;
+        auto issue_qk = [&](int tt, int w) {
+          const int s = tt % kDecStages;
+          mbar_wait(bar(D_KF + s), (tt / kDecStages) & 1);
           tc_fence_after();
-          issue_qk(j + 1);
-          mma_commit(bar(D_SF + ((j + 1) & 1)));
-          mma_commit(bar(D_KE + s1));
-        }
-        const int s = j % kDecStages;
-        mbar_wait(bar(D_PF + (j & 1)), (j >> 1) & 1);
-        mbar_wait(bar(D_VF + s), (j / kDecStages) & 1);
-        tc_fence_after();
-        const uint32_t va = sbase + dOffKV + s * 2 * dT + dT;
+          const uint32_t qa = sbase + dOffQ, ka = sbase + dOffKV + s * 2 * dT;
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
-          mma_ts(tO, tbase + (j & 1) * 128 + kk * 8, desc_mnmajor(va + kk * 2048, dH), idesc_pv, (j > 0 || kk > 0) ? 1u : 0u);
-        mma_commit(bar(D_VE + s));
-        mma_commit(bar(D_OV));
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint32_t o = (kk >> 2) * dH + (kk & 3) * 32;
+            mma_ss(tbase + w * 128, desc_kmajor(qa + o), desc_kmajor(ka + o), idesc_qk, kk > 0);
+          }
+          mma_commit(bar(D_SF + w));
+          mma_commit(bar(D_KE + s));
+        };
+        for (int nseg = 0;; ++nseg) {
+          const int k = nseg & (kDescRing - 1);
+          mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
+          const int n = dring[k].n_tiles;
+          if (dring[k].kind < 0) break;
+          mbar_wait(bar(D_QF), nseg & 1);
+          tc_fence_after();
+          issue_qk(t, 0);
+          if (n > 1) issue_qk(t + 1, 1);
+          if (n <= 2) mma_commit(bar(D_QE));
+          for (int j = 0; j < n; ++j) {
+            const int w = j & 1, s = (t + j) % kDecStages;
+            const int cw = w ? c1 : c0;
+            mbar_wait(bar(D_PF + w), cw & 1);
+            if (w) ++c1; else ++c0;
+            mbar_wait(bar(D_VF + s), ((t + j) / kDecStages) & 1);
+            tc_fence_after();
+            const uint32_t va = sbase + dOffKV + s * 2 * dT + dT;
+#pragma unroll
+            for (int kk = 0; kk < 8; ++kk)
+              mma_ts(tbase + 256 + w * 128, tbase + w * 128 + kk * 8, desc_mnmajor(va + kk * 2048, dH), idesc_pv,
+                     (j >= 2 || kk > 0) ? 1u : 0u);
+            mma_commit(bar(D_VE + s));
+            mma_commit(bar(D_OV + w));
+            if (j + 2 < n) {
+              issue_qk(t + j + 2, w);
+              if (j + 2 == n - 1) mma_commit(bar(D_QE));
+            }
+          }
+          t += n;
+        }
       }
-      mma_commit(bar(D_OD));
+    } else {
+      // ===================================================================== query gather (warps 10, 11)
+      const int i = threadIdx.x - 320;                               // 0..63: rows i and i + 64
+      for (int nseg = 0;; ++nseg) {
+        const int k = nseg & (kDescRing - 1);
+        mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
+        const DecSeg d = dring[k];
+        if (d.kind < 0) break;
+        mbar_wait(bar(D_QE), (nseg & 1) ^ 1);                        // the previous segment's last QK has read the tile
+        const int n_rows = d.n_seqs * G;
+#pragma unroll
+        for (int rr = 0; rr < 2; ++rr) {
+          const int r = i + 64 * rr;
+          const uint4* src = nullptr;
+          if (r < n_rows) {
+            const int seq = d.kind == 0 ? prm.seqs[d.seq_off + r / G] : d.seq_off, h = d.g * G + r % G;
+            src = reinterpret_cast<const uint4*>(prm.Q + ((int64_t)prm.seq_off[seq] * prm.Hq + h) * 128);
+          }
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            uint4 q[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) q[c] = src ? src[half * 8 + c] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+              const uint32_t addr = sbase + dOffQ + half * dH + r * 128 + ((uint32_t)(c ^ (r & 7)) << 4);
+              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(q[c].x), "r"(q[c].y), "r"(q[c].z), "r"(q[c].w) : "memory");
+            }
+          }
+        }
+        fence_proxy_async();
+        mbar_arrive(bar(D_QF));
+      }
     }
   } else {
-    // ===================================================================== softmax + partial write
-    const int r = threadIdx.x;                                   // row = TMEM lane
-    const int n_rows = it.n_seqs * G;
-    const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-    {
-      // gather this row's query: (sequence j, head g*G + h') -> 256 bytes into the swizzled K-major tile
-      uint4 q[16];
-      if (r < n_rows) {
-        const int seq = prm.seqs[it.seq_off + r / G], h = g * G + r % G;
-        const uint4* src = reinterpret_cast<const uint4*>(prm.Q + ((int64_t)prm.seq_off[seq] * prm.Hq + h) * 128);
-#pragma unroll
-        for (int c = 0; c < 16; ++c) q[c] = src[c];
-      } else {
-#pragma unroll
-        for (int c = 0; c < 16; ++c) q[c] = make_uint4(0, 0, 0, 0);
-      }
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        const uint32_t addr = sbase + dOffQ + (c >> 3) * dH + r * 128 + ((uint32_t)((c & 7) ^ (r & 7)) << 4);
-        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(q[c].x), "r"(q[c].y), "r"(q[c].z), "r"(q[c].w) : "memory");
-      }
-      fence_proxy_async();
-      mbar_arrive(bar(D_QR));
-    }
-    float m = -INFINITY, l = 0.f;
-    for (int j = 0; j < n; ++j) {
-      const uint32_t tS = tbase + (j & 1) * 128 + lane_base;
-      const int limit = tiles[j].len;
-      mbar_wait(bar(D_SF + (j & 1)), (j >> 1) & 1);
-      tc_fence_after();
-      uint32_t s[128];
-      tmem_ld32(tS, s);
-      tmem_ld32(tS + 32, s + 32);
-      tmem_ld32(tS + 64, s + 64);
-      tmem_ld32(tS + 96, s + 96);
-      tc_wait_ld();
-      if (limit < 128) {
-#pragma unroll
-        for (int c = 0; c < 128; ++c)
-          if (c >= limit) s[c] = 0xff800000u;
-      }
-      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;   // four independent chains
-#pragma unroll
-      for (int c = 0; c < 128; c += 8) {
-        mx0 = max3(mx0, __uint_as_float(s[c]), __uint_as_float(s[c + 1]));
-        mx1 = max3(mx1, __uint_as_float(s[c + 2]), __uint_as_float(s[c + 3]));
-        mx2 = max3(mx2, __uint_as_float(s[c + 4]), __uint_as_float(s[c + 5]));
-        mx3 = max3(mx3, __uint_as_float(s[c + 6]), __uint_as_float(s[c + 7]));
-      }
-      const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * prm.scale_log2);
-      if (j == 0) {
-        m = m_new;
-      } else if (__any_sync(0xffffffffu, m_new > m + 8.f)) {
-        mbar_wait(bar(D_OV), (j - 1) & 1);                       // PV(j-1) has finished updating O
+    // ======================================================================= softmax warpgroups + merge
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    const int w = warp >> 2;                                         // warpgroup: tiles j = w, w + 2, ...
+    const int r = threadIdx.x & 127;                                 // row = TMEM lane
+    const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t tS = tbase + w * 128 + lane_base, tOw = tbase + 256 + w * 128 + lane_base;
+    float2* ml = reinterpret_cast<float2*>(smem + dOffML);           // [2][128]
+    int32_t* flag = reinterpret_cast<int32_t*>(smem + dOffFlag);
+    int cme = 0, cother = 0;                                         // tiles this / the other warpgroup has handled
+    for (int nseg = 0;; ++nseg) {
+      const int k = nseg & (kDescRing - 1);
+      mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
+      const DecSeg d = dring[k];
+      if (d.kind < 0) break;
+      const int n = d.n_tiles;
+      float m = -INFINITY, l = 0.f;
+      for (int j = w; j < n; j += 2) {
+        const int limit = d.kind == 0 ? prm.tiles[d.tile_off + j].len : min(128, d.self_len - 128 * j);
+        const bool ragged = limit < 128;
+        mbar_wait(bar(D_SF + w), cme & 1);
         tc_fence_after();
-        const float f = ex2_approx(m - m_new);
-        m = m_new;
-        l *= f;
+        // two passes over the 128 scores, 64 at a time (row max, then exp): TMEM reads are cheap and half the
+        // registers leave room for the merge code below
+        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;   // four independent chains
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t o[32];
-          tmem_ld32(tO + lane_base + c * 32, o);
+        for (int hf = 0; hf < 2; ++hf) {
+          uint32_t s[64];
+          tmem_ld32(tS + hf * 64, s);
+          tmem_ld32(tS + hf * 64 + 32, s + 32);
+          tc_wait_ld();
+          if (ragged) {
+#pragma unroll
+            for (int cc = 0; cc < 64; ++cc)
+              if (hf * 64 + cc >= limit) s[cc] = 0xff800000u;
+          }
+#pragma unroll
+          for (int cc = 0; cc < 64; cc += 8) {
+            mx0 = max3(mx0, __uint_as_float(s[cc]), __uint_as_float(s[cc + 1]));
+            mx1 = max3(mx1, __uint_as_float(s[cc + 2]), __uint_as_float(s[cc + 3]));
+            mx2 = max3(mx2, __uint_as_float(s[cc + 4]), __uint_as_float(s[cc + 5]));
+            mx3 = max3(mx3, __uint_as_float(s[cc + 6]), __uint_as_float(s[cc + 7]));
+          }
+        }
+        const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * prm.scale_log2);
+        if (j < 2) {
+          m = m_new;
+        } else if (__any_sync(0xffffffffu, m_new > m + 8.f)) {
+          mbar_wait(bar(D_OV + w), (cme - 1) & 1);                   // this warpgroup's previous PV has updated O
+          tc_fence_after();
+          const float f = ex2_approx(m - m_new);
+          m = m_new;
+          l *= f;
+#pragma unroll
+          for (int cc = 0; cc < 4; ++cc) {
+            uint32_t o[32];
+            tmem_ld32(tOw + cc * 32, o);
+            tc_wait_ld();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
+            tmem_st32(tOw + cc * 32, o);
+          }
+        }
+        const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);
+        uint64_t sum2a = pack2(0.f, 0.f), sum2b = sum2a;
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          uint32_t s[64];
+          tmem_ld32(tS + hf * 64, s);
+          tmem_ld32(tS + hf * 64 + 32, s + 32);
           tc_wait_ld();
 #pragma unroll
-          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
-          tmem_st32(tO + lane_base + c * 32, o);
+          for (int i = 0; i < 32; i += 2) {
+            float a0, a1, b0, b1;
+            unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
+            unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
+            a0 = ex2_approx(a0); a1 = ex2_approx(a1);
+            if ((i & 6) != 6) exp2_poly2(b0, b1, b0, b1);    // 3 of every 8 scores on the FMA pipe
+            else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
+            if (ragged) {
+              // a masked key weighs EXACTLY 0 (its raw score may be anything; its V row may be a stale cache row)
+              const int c0 = hf * 64 + 2 * i;
+              a0 = c0 < limit ? a0 : 0.f;
+              a1 = c0 + 1 < limit ? a1 : 0.f;
+              b0 = c0 + 2 < limit ? b0 : 0.f;
+              b1 = c0 + 3 < limit ? b1 : 0.f;
+            }
+            sum2a = add2(sum2a, pack2(a0, a1));
+            sum2b = add2(sum2b, pack2(b0, b1));
+            s[i] = pack_bf16(a0, a1);
+            s[i + 1] = pack_bf16(b0, b1);
+          }
+          tmem_st32(tS + hf * 32, s);
         }
+        {
+          float x0, x1;
+          unpack2(add2(sum2a, sum2b), x0, x1);
+          l += x0 + x1;
+        }
+        tc_wait_st();
+        tc_fence_before();
+        mbar_arrive(bar(D_PF + w));
+        ++cme;
       }
-      const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);
-      uint64_t sum2a = pack2(0.f, 0.f), sum2b = sum2a;
-#pragma unroll
-      for (int i = 0; i < 64; i += 2) {
-        float a0, a1, b0, b1;
-        unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
-        unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
-        a0 = ex2_approx(a0); a1 = ex2_approx(a1);
-        if ((i & 6) != 6) exp2_poly2(b0, b1, b0, b1);    // 3 of every 8 scores on the FMA pipe
-        else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
-        sum2a = add2(sum2a, pack2(a0, a1));
-        sum2b = add2(sum2b, pack2(b0, b1));
-        s[i] = pack_bf16(a0, a1);
-        s[i + 1] = pack_bf16(b0, b1);
-      }
-      {
-        float x0, x1;
-        unpack2(add2(sum2a, sum2b), x0, x1);
-        l += x0 + x1;
-      }
-      tmem_st32(tS, s);
-      tmem_st32(tS + 32, s + 32);
-      tc_wait_st();
-      tc_fence_before();
-      mbar_arrive(bar(D_PF + (j & 1)));
+      cother += (n - (w ^ 1) + 1) >> 1;                             // the other warpgroup's tiles of this segment
+      dec_segment_epilogue(prm, slen, d, w, r, tbase, lane_base, m, l, w ? cother : cme, w ? cme : cother,
+                           bar(D_OV), ml, flag);
+      if ((threadIdx.x & 127) == 0) mbar_arrive(bar(D_DE + k));
     }
-    mbar_wait(bar(D_OD), 0);
-    tc_fence_after();
-    float* prow = prm.part + ((int64_t)g * prm.rows_total + (int64_t)it.row_off * G + r) * kPartStride;
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      uint32_t o[32];
-      tmem_ld32(tO + lane_base + c * 32, o);
-      tc_wait_ld();
-      if (r < n_rows) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-          *reinterpret_cast<float4*>(prow + c * 32 + 4 * i) =
-              make_float4(__uint_as_float(o[4 * i]), __uint_as_float(o[4 * i + 1]), __uint_as_float(o[4 * i + 2]),
-                          __uint_as_float(o[4 * i + 3]));
-      }
-    }
-    if (r < n_rows) *reinterpret_cast<float2*>(prow + 128) = make_float2(m, l);
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 4) tmem_dealloc(tbase, 512);
-}
-
-// Merges the split-KV partials of one (sequence, head) and adds the query's own key/value (the
-// causal self block of a 1-token sequence).  One warp per (sequence, head); lane = 4 columns.
-__global__ void __launch_bounds__(256)
-decode_combine_kernel(const float* __restrict__ part, const int32_t* __restrict__ comb_off,
-                      const int32_t* __restrict__ comb_row, const int32_t* __restrict__ seq_off,
-                      const __nv_bfloat16* __restrict__ Q, const __nv_bfloat16* __restrict__ Ks,
-                      const __nv_bfloat16* __restrict__ Vs, __nv_bfloat16* __restrict__ O, float* __restrict__ LSE,
-                      int64_t rows_total, int B, int Hq, int Hkv, float scale_log2) {
-  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (w >= B * Hq) return;
-  const int b = w / Hq, h = w % Hq, G = Hq / Hkv, g = h / G;
-  const int64_t t = seq_off[b];
-  const int e0 = comb_off[b], e1 = comb_off[b + 1];
-  float M = -INFINITY, s_self = -INFINITY;
-  if (Ks != nullptr) {
-    const uint2 qa = *reinterpret_cast<const uint2*>(Q + (t * Hq + h) * 128 + lane * 4);
-    const uint2 ka = *reinterpret_cast<const uint2*>(Ks + (t * Hkv + g) * 128 + lane * 4);
-    const float2 q0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qa.x));
-    const float2 q1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qa.y));
-    const float2 k0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ka.x));
-    const float2 k1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ka.y));
-    float d = q0.x * k0.x + q0.y * k0.y + q1.x * k1.x + q1.y * k1.y;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) d += __shfl_xor_sync(0xffffffffu, d, o);
-    s_self = d * scale_log2;
-    M = s_self;
-  }
-  for (int e = e0; e < e1; ++e)
-    M = fmaxf(M, part[((int64_t)g * rows_total + (int64_t)comb_row[e] * G + h % G) * kPartStride + 128]);
-  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  float L = 0.f;
-  for (int e = e0; e < e1; ++e) {
-    const float* p = part + ((int64_t)g * rows_total + (int64_t)comb_row[e] * G + h % G) * kPartStride;
-    const float f = ex2_approx(p[128] - M);
-    const float4 v = *reinterpret_cast<const float4*>(p + lane * 4);
-    acc.x += f * v.x; acc.y += f * v.y; acc.z += f * v.z; acc.w += f * v.w;
-    L += f * p[129];
-  }
-  if (Ks != nullptr) {
-    const float f = ex2_approx(s_self - M);
-    const uint2 va = *reinterpret_cast<const uint2*>(Vs + (t * Hkv + g) * 128 + lane * 4);
-    const float2 v0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&va.x));
-    const float2 v1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&va.y));
-    acc.x += f * v0.x; acc.y += f * v0.y; acc.z += f * v1.x; acc.w += f * v1.y;
-    L += f;
-  }
-  const float inv = 1.f / L;
-  uint2 o;
-  o.x = pack_bf16(acc.x * inv, acc.y * inv);
-  o.y = pack_bf16(acc.z * inv, acc.w * inv);
-  *reinterpret_cast<uint2*>(O + (t * Hq + h) * 128 + lane * 4) = o;
-  if (lane == 0) LSE[t * Hq + h] = M * 0.6931471805599453f + logf(L);
+  if (warp == 8) tmem_dealloc(tbase, 512);
 }
 
 // ------------------------------------------------------------------------------- host side
 bool tc_decode_supported(const cas_pool* p, const cas_slot_table* t, int Hq) {
   if (!(p->desc.dtype == CAS_BF16 && p->desc.D == 128 && p->has_tma)) return false;
-  if (t->max_lq != 1 || t->nsel == 0) return false;
+  if (t->max_lq != 1) return false;
   const int G = Hq / p->desc.Hkv;
   return G >= 1 && G <= 128;
 }
 
-// Groups the used slots by their set of selecting sequences, cuts every group into row blocks of
-// 128/G sequences and chunks of KV tiles, and uploads the item / sequence / tile / combine lists plus
-// the partial-result scratch (library-owned, part of the slot table, freed with it).
+// Groups the used slots by their set of selecting sequences, cuts every (group, row block, KV head) tile list into
+// chunks of about total/#SM tiles, deals the resulting segments to the persistent CTAs and uploads the lists
+// (asynchronously, through a pinned mirror) together with the partial-result scratch, the row counters and the
+// ticket -- all library-owned, part of the slot table, freed with it.
 static int decode_prepare(cas_slot_table* t, int Hq) {
   if (t->dec_Hq == Hq && t->d_dec_blob) return CAS_OK;
-  if (t->d_dec_blob) { cudaDeviceSynchronize(); cudaFree(t->d_dec_blob); t->d_dec_blob = nullptr; }
+  if (t->d_dec_blob) {
+    cudaDeviceSynchronize();
+    cudaFree(t->d_dec_blob);
+    cudaFreeHost(t->h_dec_blob);
+    t->d_dec_blob = nullptr;
+    t->h_dec_blob = nullptr;
+  }
   const cas_pool* p = t->pool;
   const int Hkv = p->desc.Hkv, G = Hq / Hkv, R = 128 / G;
+  int dev = 0, n_sm = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   std::map<std::vector<int32_t>, std::vector<int32_t>> groups;   // sequence set -> slots (ascending)
   for (int s : t->used_slots)
     groups[std::vector<int32_t>(t->inv_seq.begin() + t->inv_off[s], t->inv_seq.begin() + t->inv_off[s + 1])].push_back(s);
@@ -331,12 +553,11 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
       const int len = p->cart_len[p->cart_in[s]];
       for (int j = 0; j < len; j += 128) tl.push_back({p->slot_base[s] + j, std::min(128, len - j)});
     }
-    units += (int64_t)((kv.first.size() + R - 1) / R) * (int64_t)tl.size();
+    units += (int64_t)((kv.first.size() + R - 1) / R) * (int64_t)tl.size() * Hkv;
     gtiles.push_back(std::move(tl));
   }
-  const int64_t target = std::max<int64_t>(1, (148 * 4) / Hkv);          // CTAs per KV head: ~4 per SM in total
-  const int64_t C = std::max<int64_t>(4, (units + target - 1) / target);  // tiles per chunk
-  std::vector<DecItem> items;
+  const int64_t quota = std::max<int64_t>(1, (units + n_sm - 1) / n_sm);   // tiles per CTA
+  std::vector<DecSeg> segs;
   std::vector<int32_t> seqs;
   std::vector<KvTile> tiles;
   std::vector<std::vector<int32_t>> comb(t->B);
@@ -345,80 +566,127 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   for (auto& kv : groups) {
     const std::vector<KvTile>& tl = gtiles[gi++];
     const int nt = (int)tl.size();
-    const int nchunk = (int)((nt + C - 1) / C);
-    // chunk-major: the row blocks that share a chunk of tiles get adjacent block indices, so they run in the
-    // same wave and the second read of a K/V tile hits L2 instead of HBM
+    // whole chunks of about `quota` tiles: the row blocks of one chunk land on CTAs that start together and walk the
+    // same tiles at the same time, so a tile that several row blocks need is fetched from HBM once
+    const int nchunk = (int)std::max<int64_t>(1, (nt + quota / 2) / quota);
     std::vector<int> seq_offs;
     for (size_t r0 = 0; r0 < kv.first.size(); r0 += R) {
       const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
       seq_offs.push_back((int)seqs.size());
       seqs.insert(seqs.end(), kv.first.begin() + r0, kv.first.begin() + r0 + ns);
     }
+    const int to = (int)tiles.size();
+    tiles.insert(tiles.end(), tl.begin(), tl.end());
     for (int c = 0; c < nchunk; ++c) {
       const int a = (int)((int64_t)nt * c / nchunk), b = (int)((int64_t)nt * (c + 1) / nchunk);
-      const int to = (int)tiles.size();
-      tiles.insert(tiles.end(), tl.begin() + a, tl.begin() + b);
       for (size_t rb = 0; rb < seq_offs.size(); ++rb) {
         const size_t r0 = rb * R;
         const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
-        items.push_back({seq_offs[rb], ns, to, b - a, row_off, {0, 0, 0}});
+        for (int g = 0; g < Hkv; ++g) segs.push_back(DecSeg{0, to + a, b - a, g, seq_offs[rb], ns, row_off, 0});
         for (int j = 0; j < ns; ++j) comb[kv.first[r0 + j]].push_back(row_off + j);
         row_off += ns;
       }
     }
   }
-  std::stable_sort(items.begin(), items.end(), [](const DecItem& a, const DecItem& b) { return a.n_tiles > b.n_tiles; });
+  // deal the segments to the CTAs in order: a CTA is closed once it holds its share of what is left
+  const int grid = n_sm;
+  std::vector<int32_t> cta_seg_off(grid + 1, 0);
+  {
+    int64_t load = 0, done = 0;
+    int cta = 0;
+    for (size_t i = 0; i < segs.size(); ++i) {
+      const int64_t share = (units - done + (grid - cta) - 1) / std::max(1, grid - cta);
+      if (load > 0 && load + segs[i].n_tiles / 2 >= share && cta < grid - 1) {
+        cta_seg_off[++cta] = (int32_t)i;
+        done += load;
+        load = 0;
+      }
+      load += segs[i].n_tiles;
+    }
+    for (int c = cta + 1; c <= grid; ++c) cta_seg_off[c] = (int32_t)segs.size();
+  }
   std::vector<int32_t> comb_off(t->B + 1, 0), comb_row;
   for (int b = 0; b < t->B; ++b) {
     comb_row.insert(comb_row.end(), comb[b].begin(), comb[b].end());
     comb_off[b + 1] = (int32_t)comb_row.size();
   }
   auto up = [](size_t x) { return (x + 255) / 256 * 256; };
-  const size_t o_it = 0, o_sq = up(items.size() * sizeof(DecItem)), o_tl = o_sq + up(seqs.size() * 4),
-               o_co = o_tl + up(tiles.size() * sizeof(KvTile)), o_cr = o_co + up(comb_off.size() * 4),
-               o_pt = o_cr + up(comb_row.size() * 4 + 4);
-  const size_t part_bytes = (size_t)Hkv * row_off * G * kPartStride * 4;
-  std::vector<char> h(o_pt, 0);
-  memcpy(h.data() + o_it, items.data(), items.size() * sizeof(DecItem));
-  memcpy(h.data() + o_sq, seqs.data(), seqs.size() * 4);
-  memcpy(h.data() + o_tl, tiles.data(), tiles.size() * sizeof(KvTile));
-  memcpy(h.data() + o_co, comb_off.data(), comb_off.size() * 4);
-  if (!comb_row.empty()) memcpy(h.data() + o_cr, comb_row.data(), comb_row.size() * 4);
+  const size_t o_sg = 0, o_cs = up(segs.size() * sizeof(DecSeg) + 32), o_sq = o_cs + up(cta_seg_off.size() * 4),
+               o_tl = o_sq + up(seqs.size() * 4 + 4), o_co = o_tl + up(tiles.size() * sizeof(KvTile) + 8),
+               o_cr = o_co + up(comb_off.size() * 4), o_cn = o_cr + up(comb_row.size() * 4 + 4),
+               o_tk = o_cn + up((size_t)t->B * Hq * 4), o_pt = o_tk + 256;
+  const int64_t part_rows = (int64_t)row_off + t->B;               // prefix partial rows + one self row per sequence
+  const size_t part_bytes = (size_t)Hkv * part_rows * G * kPartStride * 4;
   cudaError_t e = cudaMalloc((void**)&t->d_dec_blob, o_pt + part_bytes + 256);
-  if (e == cudaSuccess) e = cudaMemcpy(t->d_dec_blob, h.data(), o_pt, cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) { if (t->d_dec_blob) cudaFree(t->d_dec_blob); t->d_dec_blob = nullptr; return cuda_fail(e, "decode table upload"); }
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&t->h_dec_blob, o_pt, cudaHostAllocDefault);
+  if (e == cudaSuccess && !t->dec_ready) e = cudaEventCreateWithFlags(&t->dec_ready, cudaEventDisableTiming);
+  if (e != cudaSuccess) {
+    if (t->d_dec_blob) cudaFree(t->d_dec_blob);
+    if (t->h_dec_blob) cudaFreeHost(t->h_dec_blob);
+    t->d_dec_blob = nullptr;
+    t->h_dec_blob = nullptr;
+    return cuda_fail(e, "decode table allocation");
+  }
+  char* h = t->h_dec_blob;
+  memset(h, 0, o_pt);                                              // row counters and ticket start at zero
+  if (!segs.empty()) memcpy(h + o_sg, segs.data(), segs.size() * sizeof(DecSeg));
+  memcpy(h + o_cs, cta_seg_off.data(), cta_seg_off.size() * 4);
+  if (!seqs.empty()) memcpy(h + o_sq, seqs.data(), seqs.size() * 4);
+  if (!tiles.empty()) memcpy(h + o_tl, tiles.data(), tiles.size() * sizeof(KvTile));
+  memcpy(h + o_co, comb_off.data(), comb_off.size() * 4);
+  if (!comb_row.empty()) memcpy(h + o_cr, comb_row.data(), comb_row.size() * 4);
+  cudaStream_t up_st = t->pool->st_upload;
+  e = cudaMemcpyAsync(t->d_dec_blob, h, o_pt, cudaMemcpyHostToDevice, up_st);
+  if (e == cudaSuccess) e = cudaEventRecord(t->dec_ready, up_st);
+  if (e != cudaSuccess) return cuda_fail(e, "decode table upload");
   char* d = t->d_dec_blob;
-  t->d_dec_items = (DecItem*)(d + o_it);
+  t->d_dec_segs = (DecSeg*)(d + o_sg);
+  t->d_dec_cta_off = (int32_t*)(d + o_cs);
   t->d_dec_seqs = (int32_t*)(d + o_sq);
   t->d_dec_tiles = (KvTile*)(d + o_tl);
   t->d_comb_off = (int32_t*)(d + o_co);
   t->d_comb_row = (int32_t*)(d + o_cr);
+  t->d_dec_cnt = (int32_t*)(d + o_cn);
+  t->d_dec_ticket = (int32_t*)(d + o_tk);
   t->d_dec_part = (float*)(d + o_pt);
-  t->dec_items = std::move(items);
-  t->dec_rows = (int64_t)row_off * G;
+  t->dec_comb_off = comb_off;
+  t->dec_grid = grid;
+  t->dec_rows = part_rows * G;
+  t->dec_self_row_base = row_off;
+  t->dec_n_segs = (int32_t)segs.size();
   t->dec_Hq = Hq;
   return CAS_OK;
 }
 
-int tc_decode_fwd(const AttnArgs& a) {
+int tc_decode_fwd(const AttnArgs& a, const void* Kc, const void* Vc, int cache_cap, const int32_t* self_len) {
   cas_slot_table* t = const_cast<cas_slot_table*>(a.tab);
+  if (Kc && t->B > kMaxDecB) { set_error("decode with a self cache takes at most %d sequences per call", kMaxDecB); return CAS_ERR_CAPACITY; }
   int rc = decode_prepare(t, a.Hq);
   if (rc) return rc;
+  SelfLens sl;
+  for (int b = 0; b < t->B; ++b) {
+    const int len = Kc ? self_len[b] : 0;
+    if (len < 0 || len > cache_cap) { set_error("self_len[%d] = %d outside [0, cache_cap]", b, len); return CAS_ERR_INVALID_ARG; }
+    if (len == 0 && t->dec_comb_off[b + 1] == t->dec_comb_off[b]) { set_error("sequence %d sees no key at all", b); return CAS_ERR_SHAPE; }
+    if (b < kMaxDecB) sl.v[b] = len;
+  }
   static SmemAttrOnce attr;
-  {
-    const int rc_attr = attr.set((const void*)tc_decode_kernel, (int)kDecSmem);
-    if (rc_attr) return rc_attr;
+  rc = attr.set((const void*)tc_decode_kernel, (int)kDecSmem);
+  if (rc) return rc;
+  CAS_CUDA(cudaStreamWaitEvent(a.stream, t->dec_ready, 0));
+  CUtensorMap tmKc = a.L->tm_K, tmVc = a.L->tm_V;
+  if (Kc) {
+    rc = make_thd_map(&tmKc, Kc, (int64_t)t->B * cache_cap, a.Hkv, 128);
+    if (rc) return rc;
+    rc = make_thd_map(&tmVc, Vc, (int64_t)t->B * cache_cap, a.Hkv, 128);
+    if (rc) return rc;
   }
   const float scale_log2 = a.scale * 1.4426950408889634f;
-  DecParams prm{t->d_dec_items, t->d_dec_seqs, t->d_dec_tiles, t->d_seq_off, (const __nv_bfloat16*)a.Q,
-                t->d_dec_part, t->dec_rows, a.Hq, a.Hkv, scale_log2};
-  const unsigned grid = (unsigned)(t->dec_items.size() * a.Hkv);
-  tc_decode_kernel<<<grid, kDecThreads, kDecSmem, a.stream>>>(a.pool->tm_K, a.pool->tm_V, prm);
-  const int n_w = t->B * a.Hq;
-  decode_combine_kernel<<<(n_w * 32 + 255) / 256, 256, 0, a.stream>>>(
-      t->d_dec_part, t->d_comb_off, t->d_comb_row, t->d_seq_off, (const __nv_bfloat16*)a.Q,
-      (const __nv_bfloat16*)a.Ks, (const __nv_bfloat16*)a.Vs, (__nv_bfloat16*)a.O_out, a.LSE_out, t->dec_rows, t->B,
-      a.Hq, a.Hkv, scale_log2);
+  DecParams prm{t->d_dec_segs, t->d_dec_cta_off, t->d_dec_seqs, t->d_dec_tiles, t->d_seq_off, t->d_comb_off,
+                t->d_comb_row, (const __nv_bfloat16*)a.Q, (const __nv_bfloat16*)Kc, (const __nv_bfloat16*)Vc,
+                (__nv_bfloat16*)a.O_out, a.LSE_out, t->d_dec_part, t->d_dec_cnt, t->d_dec_ticket, t->dec_rows,
+                t->dec_self_row_base, cache_cap, t->B, a.Hq, a.Hkv, scale_log2};
+  tc_decode_kernel<<<(unsigned)t->dec_grid, kDecThreads, kDecSmem, a.stream>>>(a.L->tm_K, a.L->tm_V, tmKc, tmVc, prm, sl);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc decode launch");
 }

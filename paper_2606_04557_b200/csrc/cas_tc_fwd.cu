@@ -49,10 +49,12 @@ int make_thd_map(CUtensorMap* out, const void* base, int64_t tokens, int heads, 
 }
 
 int tc_make_pool_maps(cas_pool* p) {
-  int rc = make_thd_map(&p->tm_K, p->pool_K, p->pool_tokens, p->desc.Hkv, 128);
-  if (rc) return rc;
-  rc = make_thd_map(&p->tm_V, p->pool_V, p->pool_tokens, p->desc.Hkv, 128);
-  if (rc) return rc;
+  for (PoolLayer& L : p->layers) {
+    int rc = make_thd_map(&L.tm_K, L.pool_K, p->pool_tokens, p->desc.Hkv, 128);
+    if (rc) return rc;
+    rc = make_thd_map(&L.tm_V, L.pool_V, p->pool_tokens, p->desc.Hkv, 128);
+    if (rc) return rc;
+  }
   p->has_tma = true;
   return CAS_OK;
 }
@@ -350,13 +352,13 @@ int tc_attn_fwd(const AttnArgs& a) {
     rc = make_thd_map(&tmVs, a.Vs, t->T, a.Hkv, 128);
     if (rc) return rc;
   } else {
-    tmKs = a.pool->tm_K;
-    tmVs = a.pool->tm_V;
+    tmKs = a.L->tm_K;
+    tmVs = a.L->tm_V;
   }
   FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale * 1.4426950408889634f};
   const unsigned grid = (unsigned)(n_items * a.Hq);
-  tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.pool->tm_K, a.pool->tm_V, tmKs, tmVs, prm);
+  tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.L->tm_K, a.L->tm_V, tmKs, tmVs, prm);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc fwd launch");
 }

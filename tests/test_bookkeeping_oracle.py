@@ -206,3 +206,21 @@ def test_lr_schedule_table5_values():
     assert all(warmup_scale(s, 20, 4) >= min(1.0, (s + 1) / 20) for s in range(60))
     assert len({warmup_scale(s, 20, 4) for s in range(100)}) == 4             # "at most N_b param groups"
     assert warmup_scale(0, 1, 4) == 1.0
+
+
+def test_select_retrieved_hand_worked_and_order_preserving():
+    """chunk -> document -> cartridge, unique ids in retrieval order.  Hand-worked: the ranked chunks
+    7, 2, 9, 3, 2 belong to documents 3, 1, 3, 0, 1 -> cartridges [3, 1, 0]; with room for two -> [3, 1]."""
+    from oracle.bookkeeping import select_retrieved
+    chunk_to_cart = [5, 5, 1, 0, 4, 4, 2, 3, 2, 3]
+    assert select_retrieved([7, 2, 9, 3, 2], chunk_to_cart, 10) == [3, 1, 0]
+    assert select_retrieved([7, 2, 9, 3, 2], chunk_to_cart, 2) == [3, 1]
+    assert select_retrieved([], chunk_to_cart, 4) == []
+    # against Python's own order-preserving de-duplication on random rankings (Table 9's setting: 10 chunks)
+    rng = np.random.default_rng(9)
+    for _ in range(200):
+        mp = rng.integers(0, 12, size=40).tolist()
+        ranked = rng.permutation(40)[:10].tolist()
+        assert select_retrieved(ranked, mp, 99) == list(dict.fromkeys(mp[c] for c in ranked))
+    with pytest.raises(BookError):
+        select_retrieved([40], [0] * 40, 3)

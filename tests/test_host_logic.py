@@ -49,6 +49,20 @@ def counters_equal(pool, bk):
     assert c["grad_dirty"].tolist() == bk.grad_dirty
 
 
+def test_layer_axis_layout_and_manifest_bytes():
+    """a cartridge has a layer axis; its pinned home (and a manifest entry's nbytes) covers all L layers,
+    the device arena holds L carvings."""
+    lens = [48, 16, 80, 32, 64]
+    one = cas.Pool(cas.CAS_BF16, 2, 32, lens, 3, tile_tokens=16, device=None)
+    pool = cas.Pool(cas.CAS_BF16, 2, 32, lens, 3, tile_tokens=16, device=None, n_layers=4)
+    bk = PoolBook(lens, 3, 2, 32, tile_tokens=16, n_layers=4)
+    assert pool.dev_bytes == 4 * one.dev_bytes and pool.host_bytes == 4 * one.host_bytes
+    assert pool.host_bytes == sum(bk.home_bytes(c) for c in range(5))
+    man, n = cas.cas_plan_rotation(pool, 0, 2, 2, [0], 5)
+    assert manifest_tuples(man, n) == [e.as_tuple() for e in bk.plan_rotation(0, 2, 2, [0], 5)]
+    assert man[0].nbytes == 4 * 6 * lens[man[0].cart] * 64 * 4
+
+
 def test_layout_matches_oracle():
     rng = np.random.default_rng(0)
     lens = rng.integers(1, 700, size=17).tolist()
@@ -202,3 +216,18 @@ def test_lr_schedule_and_warmup_scales_against_oracle():
     assert cas.cas_warmup_scales(pool, [3, 0], 7, 3).tolist() == [np.float32(warmup_scale(5, 7, 3)),
                                                                   np.float32(warmup_scale(0, 7, 3))]
     pool.close()
+
+
+def test_select_retrieved_bit_exact_against_oracle():
+    from oracle.bookkeeping import select_retrieved
+    rng = np.random.default_rng(17)
+    for _ in range(300):
+        n_chunks = int(rng.integers(1, 60))
+        mp = rng.integers(0, 15, size=n_chunks).tolist()
+        k = int(rng.integers(0, 12))
+        ranked = rng.integers(0, n_chunks, size=k).tolist()          # repeats allowed: a chunk may be returned twice
+        cap = int(rng.integers(0, 9))
+        assert cas.cas_select_retrieved(ranked, mp, cap).tolist() == select_retrieved(ranked, mp, cap)
+    with pytest.raises(cas.CasError) as e:
+        cas.cas_select_retrieved([3], [0, 1], 2)
+    assert e.value.name == "CAS_ERR_INVALID_ARG"
