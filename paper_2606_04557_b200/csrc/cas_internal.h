@@ -174,6 +174,7 @@ struct cas_slot_table {
   int32_t dec_Hq = 0;
   int64_t dec_rows = 0;                       // partial rows per KV head (prefix segments + one self row per sequence) x G
   int32_t dec_grid = 0, dec_self_row_base = 0, dec_n_segs = 0;
+  int32_t dec_fused = 1;                     // 1: every row block has <= 32 rows: partials are merged inside the decode launch
   std::vector<int32_t> dec_comb_off;          // [B+1] prefix partials per sequence
   char* d_dec_blob = nullptr;
   char* h_dec_blob = nullptr;                 // pinned mirror of the lists (asynchronous upload)

@@ -39,17 +39,18 @@ constexpr int kInlineSelf = 4;     // caches up to this length are dotted on the
 constexpr int kMaxDecB = 1024;     // sequences per decode call with a self cache (their lengths travel as kernel parameters)
 constexpr uint32_t dT = 32768, dH = 16384;
 constexpr uint32_t dOffQ = 0, dOffKV = dT, dOffBar = dT + kDecStages * 2 * dT;
-enum { D_KF = 0, D_KE = 3, D_VF = 6, D_VE = 9, D_SF = 12, D_PF = 14, D_OV = 16, D_QF = 18, D_QE = 19, D_DF = 20, D_DE = 24, D_N = 28 };
+enum { D_KF = 0, D_KE = 3, D_VF = 6, D_VE = 9, D_SF = 12, D_PF = 14, D_OV = 16, D_QF = 18, D_QE = 19, D_DF = 20, D_DE = 24, D_PW = 28, D_N = 32 };
 constexpr uint32_t dOffDesc = dOffBar + D_N * 8 + 32;                       // after the barriers and the TMEM slot
 constexpr uint32_t dOffML = dOffDesc + kDescRing * 32;                      // (m, l) of both warpgroups: 2 x 128 x 8 B
-constexpr uint32_t dOffFlag = dOffML + 2048;                                // "this row is complete": 128 x 4 B
-constexpr uint32_t kDecSmem = dOffFlag + 512;
+constexpr uint32_t kDecSmem = dOffML + 2048;
 static_assert(kDecSmem <= 232448, "decode kernel shared memory");
 static_assert(sizeof(DecSeg) == 32, "descriptor ring entry");
 constexpr int kPartStride = 132;   // 128 O + m + l + pad (16-byte aligned rows)
 
 struct SelfLens {
-  int32_t v[kMaxDecB];
+  int32_t v[kMaxDecB];       // cached tokens per sequence
+  int32_t useq[kMaxDecB];    // the sequences whose cache gets a tensor-core segment (has_self_unit)
+  int32_t n_useq;
 };
 
 struct DecParams {
@@ -71,6 +72,7 @@ struct DecParams {
   int32_t self_row_base;        // first partial row (in units of sequences) of the self units
   int32_t cache_cap;
   int B, Hq, Hkv;
+  int fused;                    // 1: warp 11 counts and merges in this launch; 0: decode_combine_kernel follows
   float scale_log2;
 };
 
@@ -80,19 +82,18 @@ __host__ __device__ __forceinline__ bool has_self_unit(int len, int n_prefix_par
   return len > kInlineSelf || (len > 0 && n_prefix_partials == 0);
 }
 
-// End of a segment (both softmax warpgroups, 256 threads): merge the two TMEM accumulators, write ONE partial per row,
-// count it, and -- for the rows whose last partial this was -- merge all partials of the row, normalise, write O / LSE.
-__device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const SelfLens& slen, const DecSeg d, const int w,
-                                                  const int r, const uint32_t tbase, const uint32_t lane_base,
-                                                  const float m, const float l, const int c0, const int c1,
-                                                  const uint32_t bar_ov, float2* ml, int32_t* flag) {
+// End of a segment (both softmax warpgroups, 256 threads): merge the two TMEM accumulators and write ONE partial per
+// row; thread (w, r) writes columns [64w, 64w + 64) of row r.  The partials are counted and merged by warps 10-11.
+__device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const DecSeg d, const int w, const int r,
+                                                     const uint32_t tbase, const uint32_t lane_base, const float m,
+                                                     const float l, const int c0, const int c1, const uint32_t bar_ov,
+                                                     float2* ml) {
   const int G = prm.Hq / prm.Hkv;
   const int n = d.n_tiles;
-  // ---- segment epilogue: merge the two accumulators, write ONE partial per row
-  const int n0 = (n + 1) >> 1, n1 = n >> 1;
+  const int n1 = n >> 1;                                           // tiles of warpgroup 1 (warpgroup 0 has >= 1)
   ml[w * 128 + r] = make_float2(m, l);
-  asm volatile("bar.sync 2, 256;" ::: "memory");                 // both warpgroups are past their last tile ...
-  if (n0) mbar_wait(bar_ov, (c0 - 1) & 1);                    // ... so these waits are at most one phase behind
+  asm volatile("bar.sync 2, 256;" ::: "memory");                   // both warpgroups are past their last tile ...
+  mbar_wait(bar_ov, (c0 - 1) & 1);                                 // ... so these waits are at most one phase behind
   if (n1) mbar_wait(bar_ov + 8, (c1 - 1) & 1);
   tc_fence_after();
   const float2 a = ml[r], b = ml[128 + r];
@@ -100,10 +101,8 @@ __device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const
   const float f0 = ex2_approx(a.x - M), f1 = n1 ? ex2_approx(b.x - M) : 0.f;
   const float L = f0 * a.y + f1 * b.y;
   const int n_rows = d.n_seqs * G;
-  const int sj = r / G, hh = r % G;
-  const int seq = r < n_rows ? (d.kind == 0 ? prm.seqs[d.seq_off + sj] : d.seq_off) : 0;
-  float* prow = prm.part + ((int64_t)d.g * prm.rows_total + (int64_t)(d.part_row + sj) * G + hh) * kPartStride;
-  const uint32_t tO0 = tbase + 256 + lane_base + w * 64, tO1 = tO0 + 128;       // this thread: columns [64w, 64w + 64)
+  float* prow = prm.part + ((int64_t)d.g * prm.rows_total + (int64_t)d.part_row * G + r) * kPartStride;
+  const uint32_t tO0 = tbase + 256 + lane_base + w * 64, tO1 = tO0 + 128;
 #pragma unroll
   for (int cc = 0; cc < 2; ++cc) {
     uint32_t o0[32], o1[32];
@@ -125,111 +124,161 @@ __device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const
     }
   }
   if (w == 0 && r < n_rows) __stcg(reinterpret_cast<float2*>(prow + 128), make_float2(M, L));
+  // BOTH warpgroups have read O0 and O1 (each its column half) before either goes on: the next segment's first PV
+  // overwrites an accumulator as soon as ONE warpgroup has posted its next P tile
   tc_fence_before();
-  __threadfence();
   asm volatile("bar.sync 2, 256;" ::: "memory");
-  if (w == 0) {
-    int last = 0;
-    if (r < n_rows) {
-      const int len = prm.Kc ? slen.v[seq] : 0;
-      const int npre = prm.comb_off[seq + 1] - prm.comb_off[seq];
-      const int expected = npre + (has_self_unit(len, npre) ? 1 : 0);
-      last = atomicAdd(prm.cnt + ((int64_t)d.g * prm.B + seq) * G + hh, 1) == expected - 1;
+  // no fence here: the partial is published by the thread that counts it (warp 11 fences after its barrier wait;
+  // a wide table is merged by the next launch)
+}
+
+// Merge of ONE output row (sequence seq, query head g*G + hh): all split-KV partials of the row -- the prefix segments
+// that cover the sequence (comb lists), its self-cache segment if it has one -- plus the few self keys of a young cache
+// dotted here, normalised, written as O (bf16) and LSE.  LPR lanes cooperate on a row (lane `sub` owns 128/LPR
+// columns); the caller guarantees that the LPR lanes of a row are converged and that every partial is visible.
+// One pass with a running maximum; the partials are fetched four at a time (their loads are independent, so a
+// row costs about two L2 round trips per four partials instead of two per partial).
+template <int LPR>
+__device__ __forceinline__ void dec_merge_row(const DecParams& prm, const SelfLens& slen, const int g, const int seq,
+                                              const int hh, const int sub, const bool valid) {
+  constexpr int NC = 128 / LPR;                                    // columns per lane
+  const int G = prm.Hq / prm.Hkv;
+  const int h = g * G + hh;
+  const int e0 = valid ? prm.comb_off[seq] : 0, e1 = valid ? prm.comb_off[seq + 1] : 0;
+  const int len = (valid && prm.Kc) ? slen.v[seq] : 0;
+  const bool self_unit = has_self_unit(len, e1 - e0);
+  const int n_inline = self_unit ? 0 : len;
+  const int e_end = e1 + (self_unit ? 1 : 0);
+  const int64_t pbase = (int64_t)g * prm.rows_total * kPartStride;
+  const int64_t tq = valid ? prm.seq_off[seq] : 0;
+  float Mx = -INFINITY, Ls = 0.f;
+  float acc[NC];
+#pragma unroll
+  for (int i = 0; i < NC; ++i) acc[i] = 0.f;
+  auto fold = [&](float m_p, float l_p, const float* v) {          // (acc, Ls, Mx) += one partial
+    const float Mn = fmaxf(Mx, m_p);
+    const float sc = ex2_approx(Mx - Mn), f = ex2_approx(m_p - Mn);
+    Mx = Mn;
+    Ls = Ls * sc + f * l_p;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) acc[i] = acc[i] * sc + f * v[i];
+  };
+  for (int e = e0; e < e_end; e += 4) {
+    const float* p[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int ee = e + u;
+      p[u] = nullptr;
+      if (ee < e_end) {
+        const int pr = ee < e1 ? prm.comb_row[ee] : prm.self_row_base + seq;
+        p[u] = prm.part + pbase + ((int64_t)pr * G + hh) * kPartStride;
+      }
     }
-    flag[r] = last;
+    float2 mlp[4];
+    float v[4][NC];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      mlp[u] = make_float2(-INFINITY, 0.f);
+      if (p[u]) {
+        mlp[u] = __ldcg(reinterpret_cast<const float2*>(p[u] + 128));
+#pragma unroll
+        for (int i = 0; i < NC; i += 4) {
+          const float4 x = __ldcg(reinterpret_cast<const float4*>(p[u] + sub * NC + i));
+          v[u][i] = x.x; v[u][i + 1] = x.y; v[u][i + 2] = x.z; v[u][i + 3] = x.w;
+        }
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (p[u]) fold(mlp[u].x, mlp[u].y, v[u]);
   }
-  asm volatile("bar.sync 2, 256;" ::: "memory");
-  if (flag[r]) {
-    // ---- fused merge: this row's last partial has just been written
-    __threadfence();
-    const int h = d.g * G + hh;
-    const int e0 = prm.comb_off[seq], e1 = prm.comb_off[seq + 1];
+#pragma unroll
+  for (int i = 0; i < kInlineSelf; ++i) {
+    // the shuffles run with the full mask on every lane, whatever its row's n_inline
+    float dot = 0.f;
+    float vv[NC];
+    if (i < n_inline) {
+      const __nv_bfloat16* qp = prm.Q + (tq * prm.Hq + h) * 128 + sub * NC;
+      const __nv_bfloat16* kp = prm.Kc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + g) * 128 + sub * NC;
+      const __nv_bfloat16* vp = prm.Vc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + g) * 128 + sub * NC;
+#pragma unroll
+      for (int x = 0; x < NC; x += 4) {
+        const uint2 qa = *reinterpret_cast<const uint2*>(qp + x), ka = *reinterpret_cast<const uint2*>(kp + x);
+        const uint2 va = *reinterpret_cast<const uint2*>(vp + x);
+        const float2 q0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qa.x));
+        const float2 q1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qa.y));
+        const float2 k0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ka.x));
+        const float2 k1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ka.y));
+        const float2 v0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&va.x));
+        const float2 v1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&va.y));
+        dot += q0.x * k0.x + q0.y * k0.y + q1.x * k1.x + q1.y * k1.y;
+        vv[x] = v0.x; vv[x + 1] = v0.y; vv[x + 2] = v1.x; vv[x + 3] = v1.y;
+      }
+    }
+#pragma unroll
+    for (int o = LPR / 2; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
+    if (i < n_inline) fold(dot * prm.scale_log2, 1.f, vv);
+  }
+  if (!valid) return;
+  const float inv = 1.f / Ls;
+  __nv_bfloat16* orow = prm.O + (tq * prm.Hq + h) * 128 + sub * NC;
+#pragma unroll
+  for (int x = 0; x < NC; x += 4) {
+    uint2 o;
+    o.x = pack_bf16(acc[x] * inv, acc[x + 1] * inv);
+    o.y = pack_bf16(acc[x + 2] * inv, acc[x + 3] * inv);
+    *reinterpret_cast<uint2*>(orow + x) = o;
+  }
+  if (sub == 0) prm.LSE[tq * prm.Hq + h] = Mx * 0.6931471805599453f + logf(Ls);
+}
+
+// Fused merge (small batches only -- a few sequences generating: at most kFusedOut output rows in all and row blocks of
+// at most 32 rows): warp 11, after a segment's partials are written, counts them per row and merges the rows whose
+// LAST partial this was, four rows at a time (eight lanes per row).  It saves the second launch of a latency-bound
+// step.  Measured on the full-size top-8 config (2048 rows, 3-9 partials each) the same scheme is 2x SLOWER than a
+// separate launch: one warp per CTA walks ~3 dependent L2 round trips per row, and the descriptor ring makes the
+// whole pipeline wait for it -- so bigger batches use decode_combine_kernel (one warp per row, 2048 warps at once).
+constexpr int kFusedRows = 32;
+constexpr int kFusedOut = 256;
+__device__ __forceinline__ void dec_count_and_merge(const DecParams& prm, const SelfLens& slen, const DecSeg d, const int lane) {
+  const int G = prm.Hq / prm.Hkv;
+  const int n_rows = d.n_seqs * G;
+  __threadfence();     // after the barrier wait: covers the partial rows the softmax warpgroups have written
+  int last = 0, seq = 0;
+  if (lane < n_rows) {
+    seq = d.kind == 0 ? prm.seqs[d.seq_off + lane / G] : d.seq_off;
     const int len = prm.Kc ? slen.v[seq] : 0;
-    const bool self_unit = has_self_unit(len, e1 - e0);
-    const int n_inline = self_unit ? 0 : len;
-    const int64_t pbase = (int64_t)d.g * prm.rows_total * kPartStride;
-    auto part_row = [&](int e) {
-      const int pr = e < e1 ? prm.comb_row[e] : prm.self_row_base + seq;
-      return prm.part + pbase + ((int64_t)pr * G + hh) * kPartStride;
-    };
-    const int e_end = e1 + (self_unit ? 1 : 0);
-    const int64_t tq = prm.seq_off[seq];
-    float s_in[kInlineSelf];
-    float Mx = -INFINITY;
-    for (int e = e0; e < e_end; ++e) Mx = fmaxf(Mx, __ldcg(part_row(e) + 128));
-#pragma unroll
-    for (int i = 0; i < kInlineSelf; ++i) {
-      s_in[i] = -INFINITY;
-      if (i < n_inline) {
-        const uint4* qp = reinterpret_cast<const uint4*>(prm.Q + (tq * prm.Hq + h) * 128);
-        const uint4* kp = reinterpret_cast<const uint4*>(prm.Kc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + d.g) * 128);
-        float dot = 0.f;
-#pragma unroll 4
-        for (int x = 0; x < 16; ++x) {
-          const uint4 qa = qp[x], ka = kp[x];
-          const uint32_t qq[4] = {qa.x, qa.y, qa.z, qa.w}, kq[4] = {ka.x, ka.y, ka.z, ka.w};
-#pragma unroll
-          for (int y = 0; y < 4; ++y) {
-            const float2 qf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qq[y]));
-            const float2 kf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&kq[y]));
-            dot = fmaf(qf.x, kf.x, dot);
-            dot = fmaf(qf.y, kf.y, dot);
-          }
-        }
-        s_in[i] = dot * prm.scale_log2;
-        Mx = fmaxf(Mx, s_in[i]);
-      }
-    }
-    float acc[64];
-#pragma unroll
-    for (int i = 0; i < 64; ++i) acc[i] = 0.f;
-    float Ls = 0.f;
-    for (int e = e0; e < e_end; ++e) {
-      const float* p = part_row(e);
-      const float2 mlp = __ldcg(reinterpret_cast<const float2*>(p + 128));
-      const float f = ex2_approx(mlp.x - Mx);
-      Ls += f * mlp.y;
-#pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        const float4 v = __ldcg(reinterpret_cast<const float4*>(p + w * 64 + 4 * i));
-        acc[4 * i] += f * v.x; acc[4 * i + 1] += f * v.y; acc[4 * i + 2] += f * v.z; acc[4 * i + 3] += f * v.w;
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < kInlineSelf; ++i) {
-      if (i < n_inline) {
-        const float f = ex2_approx(s_in[i] - Mx);
-        Ls += f;
-        const uint4* vp = reinterpret_cast<const uint4*>(prm.Vc + (((int64_t)seq * prm.cache_cap + i) * prm.Hkv + d.g) * 128 + w * 64);
-#pragma unroll
-        for (int x = 0; x < 8; ++x) {
-          const uint4 va = vp[x];
-          const uint32_t vq[4] = {va.x, va.y, va.z, va.w};
-#pragma unroll
-          for (int y = 0; y < 4; ++y) {
-            const float2 vf = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&vq[y]));
-            acc[8 * x + 2 * y] += f * vf.x;
-            acc[8 * x + 2 * y + 1] += f * vf.y;
-          }
-        }
-      }
-    }
-    const float inv = 1.f / Ls;
-    __nv_bfloat16* orow = prm.O + (tq * prm.Hq + h) * 128 + w * 64;
-#pragma unroll
-    for (int x = 0; x < 8; ++x) {
-      uint4 u;
-      u.x = pack_bf16(acc[8 * x] * inv, acc[8 * x + 1] * inv);
-      u.y = pack_bf16(acc[8 * x + 2] * inv, acc[8 * x + 3] * inv);
-      u.z = pack_bf16(acc[8 * x + 4] * inv, acc[8 * x + 5] * inv);
-      u.w = pack_bf16(acc[8 * x + 6] * inv, acc[8 * x + 7] * inv);
-      *reinterpret_cast<uint4*>(orow + 8 * x) = u;
-    }
-    if (w == 0) {
-      prm.LSE[tq * prm.Hq + h] = Mx * 0.6931471805599453f + logf(Ls);
-      prm.cnt[((int64_t)d.g * prm.B + seq) * G + hh] = 0;       // re-arm for the next launch on this table
-    }
+    const int npre = prm.comb_off[seq + 1] - prm.comb_off[seq];
+    const int expected = npre + (has_self_unit(len, npre) ? 1 : 0);
+    last = atomicAdd(prm.cnt + ((int64_t)d.g * prm.B + seq) * G + lane % G, 1) == expected - 1;
+    if (last) prm.cnt[((int64_t)d.g * prm.B + seq) * G + lane % G] = 0;      // re-arm for the next launch on this table
   }
+  uint32_t todo = __ballot_sync(0xffffffffu, last);
+  if (todo) __threadfence();
+  while (todo) {
+    // the (lane / 8)-th pending row goes to this group of eight lanes
+    uint32_t t = todo;
+    int mine = -1;
+    for (int q = 0; q < 4 && t; ++q) {
+      const int bit = __ffs(t) - 1;
+      if (q == (lane >> 3)) mine = bit;
+      t &= t - 1;
+    }
+    todo = t;
+    const int rseq = __shfl_sync(0xffffffffu, seq, mine < 0 ? 0 : mine);
+    dec_merge_row<8>(prm, slen, d.g, rseq, (mine < 0 ? 0 : mine) % G, lane & 7, mine >= 0);
+  }
+}
+
+// Tables with wider row blocks (c5 "all loaded": 128 rows with a dozen partials each, all finishing together) are
+// merged by a second, massively parallel launch instead: one warp per output row.
+__global__ void __launch_bounds__(256)
+decode_combine_kernel(const __grid_constant__ DecParams prm, const __grid_constant__ SelfLens slen) {
+  const int wrow = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (wrow >= prm.B * prm.Hq) return;
+  const int G = prm.Hq / prm.Hkv;
+  const int b = wrow / prm.Hq, h = wrow % prm.Hq;
+  dec_merge_row<32>(prm, slen, h / G, b, h % G, lane, true);
 }
 
 __global__ void __launch_bounds__(kDecThreads, 1)
@@ -249,8 +298,9 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
     for (int i = 0; i < D_N; ++i) {
       uint32_t c = 1;
       if (i == D_PF || i == D_PF + 1) c = 128;
-      if (i == D_QF) c = 64;
-      if (i >= D_DE) c = 2;
+      if (i == D_QF) c = 32;
+      if (i >= D_DE) c = 3;
+      if (i >= D_PW) c = 256;
       mbar_init(bar(i), c);
     }
     fence_mbar_init();
@@ -265,7 +315,6 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
   const uint32_t tbase = *tmem_slot;
 
   if (warp >= 8) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;");
     if (warp == 8) {
       // ===================================================================== scheduler + TMA producer
       if (elect_one()) {
@@ -273,12 +322,16 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         tma_prefetch_desc(&tmV);
         DecSeg* wring = reinterpret_cast<DecSeg*>(smem + dOffDesc);
         int nseg = 0, t = 0;
-        auto push = [&](const DecSeg& d) {
+        // descriptors are published ONE SEGMENT AHEAD of the tile loads, so that warp 10 gathers the next segment's
+        // query rows while the current segment still computes
+        auto publish = [&](const DecSeg& d) {
           const int k = nseg & (kDescRing - 1);
           mbar_wait(bar(D_DE + k), ((nseg / kDescRing) & 1) ^ 1);
           wring[k] = d;
           mbar_arrive(bar(D_DF + k));
           ++nseg;
+        };
+        auto load_tiles = [&](const DecSeg& d) {
           const CUtensorMap* mk = d.kind == 0 ? &tmK : &tmKc;
           const CUtensorMap* mv = d.kind == 0 ? &tmV : &tmVc;
           for (int j = 0; j < d.n_tiles; ++j, ++t) {
@@ -296,25 +349,41 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             tma_load_3d(vb + dH, mv, bar(D_VF + s), 64, d.g, tok);
           }
         };
-        for (int s = prm.cta_seg_off[blockIdx.x]; s < prm.cta_seg_off[blockIdx.x + 1]; ++s) push(prm.segs[s]);
-        if (prm.Kc != nullptr) {
-          // self-cache units, one per (sequence, KV head), drawn from the ticket counter
-          const int n_units = prm.B * prm.Hkv;
-          for (;;) {
+        // source of segments: this CTA's static list, then self-cache units (one per (sequence with a long cache, KV
+        // head)) drawn from the ticket counter
+        int sidx = prm.cta_seg_off[blockIdx.x];
+        const int send = prm.cta_seg_off[blockIdx.x + 1];
+        const int n_units = slen.n_useq * prm.Hkv;
+        bool tickets_open = n_units > 0;
+        auto next = [&](DecSeg& out) -> bool {
+          if (sidx < send) { out = prm.segs[sidx++]; return true; }
+          if (tickets_open) {
             const int u = atomicAdd(prm.ticket, 1);
-            if (u >= n_units) break;
-            const int b = u / prm.Hkv, g = u % prm.Hkv;
-            const int len = slen.v[b];
-            if (!has_self_unit(len, prm.comb_off[b + 1] - prm.comb_off[b])) continue;
-            push(DecSeg{1, 0, (len + 127) >> 7, g, b, 1, prm.self_row_base + b, len});
+            if (u < n_units) {
+              const int b = slen.useq[u / prm.Hkv], len = slen.v[b];
+              out = DecSeg{1, 0, (len + 127) >> 7, u % prm.Hkv, b, 1, prm.self_row_base + b, len};
+              return true;
+            }
+            tickets_open = false;
+            __threadfence();
+            if (atomicAdd(prm.ticket + 1, 1) == (int)gridDim.x - 1) {   // every CTA has left the queue: re-arm
+              prm.ticket[0] = 0;
+              prm.ticket[1] = 0;
+            }
           }
-          __threadfence();
-          if (atomicAdd(prm.ticket + 1, 1) == (int)gridDim.x - 1) {   // every CTA has left its ticket loop: re-arm
-            prm.ticket[0] = 0;
-            prm.ticket[1] = 0;
-          }
+          return false;
+        };
+        const DecSeg stop{-1, 0, 0, 0, 0, 0, 0, 0};
+        DecSeg cur, nxt;
+        bool has_cur = next(cur);
+        publish(has_cur ? cur : stop);
+        while (has_cur) {
+          const bool has_nxt = next(nxt);
+          publish(has_nxt ? nxt : stop);
+          load_tiles(cur);
+          cur = nxt;
+          has_cur = has_nxt;
         }
-        push(DecSeg{-1, 0, 0, 0, 0, 0, 0, 0});
       }
     } else if (warp == 9) {
       // ===================================================================== MMA issuer
@@ -368,48 +437,61 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         }
       }
     } else {
-      // ===================================================================== query gather (warps 10, 11)
-      const int i = threadIdx.x - 320;                               // 0..63: rows i and i + 64
-      for (int nseg = 0;; ++nseg) {
-        const int k = nseg & (kDescRing - 1);
-        mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
-        const DecSeg d = dring[k];
-        if (d.kind < 0) break;
-        mbar_wait(bar(D_QE), (nseg & 1) ^ 1);                        // the previous segment's last QK has read the tile
-        const int n_rows = d.n_seqs * G;
+      // ===================================================================== query gather + partial merge (warps 10, 11)
+      const int lane = threadIdx.x & 31;
+      if (warp == 10) {
+        // ------------------------------------------------------------------- query gather: rows lane + 32 rr
+        for (int nseg = 0;; ++nseg) {
+          const int k = nseg & (kDescRing - 1);
+          mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
+          const DecSeg d = dring[k];
+          if (d.kind < 0) break;
+          mbar_wait(bar(D_QE), (nseg & 1) ^ 1);                      // the previous segment's last QK has read the tile
+          const int n_rows = d.n_seqs * G;
+#pragma unroll 1
+          for (int rr = 0; rr < 4; ++rr) {
+            const int r = lane + 32 * rr;
+            const uint4* src = nullptr;
+            if (r < n_rows) {
+              const int seq = d.kind == 0 ? prm.seqs[d.seq_off + r / G] : d.seq_off, h = d.g * G + r % G;
+              src = reinterpret_cast<const uint4*>(prm.Q + ((int64_t)prm.seq_off[seq] * prm.Hq + h) * 128);
+            }
 #pragma unroll
-        for (int rr = 0; rr < 2; ++rr) {
-          const int r = i + 64 * rr;
-          const uint4* src = nullptr;
-          if (r < n_rows) {
-            const int seq = d.kind == 0 ? prm.seqs[d.seq_off + r / G] : d.seq_off, h = d.g * G + r % G;
-            src = reinterpret_cast<const uint4*>(prm.Q + ((int64_t)prm.seq_off[seq] * prm.Hq + h) * 128);
-          }
+            for (int half = 0; half < 2; ++half) {
+              uint4 q[8];
 #pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            uint4 q[8];
+              for (int c = 0; c < 8; ++c) q[c] = src ? src[half * 8 + c] : make_uint4(0, 0, 0, 0);
 #pragma unroll
-            for (int c = 0; c < 8; ++c) q[c] = src ? src[half * 8 + c] : make_uint4(0, 0, 0, 0);
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-              const uint32_t addr = sbase + dOffQ + half * dH + r * 128 + ((uint32_t)(c ^ (r & 7)) << 4);
-              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(q[c].x), "r"(q[c].y), "r"(q[c].z), "r"(q[c].w) : "memory");
+              for (int c = 0; c < 8; ++c) {
+                const uint32_t addr = sbase + dOffQ + half * dH + r * 128 + ((uint32_t)(c ^ (r & 7)) << 4);
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(q[c].x), "r"(q[c].y), "r"(q[c].z), "r"(q[c].w) : "memory");
+              }
             }
           }
+          fence_proxy_async();
+          mbar_arrive(bar(D_QF));
         }
-        fence_proxy_async();
-        mbar_arrive(bar(D_QF));
+      } else {
+        // ------------------------------------------------------------------- warp 11: count + merge (fused tables)
+        for (int nseg = 0;; ++nseg) {
+          const int k = nseg & (kDescRing - 1);
+          mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
+          const DecSeg d = dring[k];
+          if (d.kind < 0) break;
+          // one barrier per descriptor-ring slot: the writers cannot lap this wait (the slot is released below)
+          mbar_wait(bar(D_PW + k), (nseg / kDescRing) & 1);
+          if (prm.fused) dec_count_and_merge(prm, slen, d, lane);
+          if (lane == 0) mbar_arrive(bar(D_DE + k));                 // last reader of the descriptor
+        }
       }
     }
   } else {
-    // ======================================================================= softmax warpgroups + merge
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;");
+    // ======================================================================= softmax warpgroups
     const int w = warp >> 2;                                         // warpgroup: tiles j = w, w + 2, ...
     const int r = threadIdx.x & 127;                                 // row = TMEM lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tS = tbase + w * 128 + lane_base, tOw = tbase + 256 + w * 128 + lane_base;
     float2* ml = reinterpret_cast<float2*>(smem + dOffML);           // [2][128]
-    int32_t* flag = reinterpret_cast<int32_t*>(smem + dOffFlag);
     int cme = 0, cother = 0;                                         // tiles this / the other warpgroup has handled
     for (int nseg = 0;; ++nseg) {
       const int k = nseg & (kDescRing - 1);
@@ -423,22 +505,23 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         const bool ragged = limit < 128;
         mbar_wait(bar(D_SF + w), cme & 1);
         tc_fence_after();
-        // two passes over the 128 scores, 64 at a time (row max, then exp): TMEM reads are cheap and half the
-        // registers leave room for the merge code below
+        // Two passes over the 128 scores (row max, then exp) in 32-column chunks with the NEXT chunk's TMEM load in
+        // flight while the current one is processed: 64 live registers instead of 128, no exposed TMEM latency.
+        uint32_t buf[2][32];
         float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;   // four independent chains
+        tmem_ld32(tS, buf[0]);
 #pragma unroll
-        for (int hf = 0; hf < 2; ++hf) {
-          uint32_t s[64];
-          tmem_ld32(tS + hf * 64, s);
-          tmem_ld32(tS + hf * 64 + 32, s + 32);
+        for (int c = 0; c < 4; ++c) {
           tc_wait_ld();
+          if (c < 3) tmem_ld32(tS + 32 * (c + 1), buf[(c + 1) & 1]);
+          uint32_t* s = buf[c & 1];
           if (ragged) {
 #pragma unroll
-            for (int cc = 0; cc < 64; ++cc)
-              if (hf * 64 + cc >= limit) s[cc] = 0xff800000u;
+            for (int cc = 0; cc < 32; ++cc)
+              if (32 * c + cc >= limit) s[cc] = 0xff800000u;
           }
 #pragma unroll
-          for (int cc = 0; cc < 64; cc += 8) {
+          for (int cc = 0; cc < 32; cc += 8) {
             mx0 = max3(mx0, __uint_as_float(s[cc]), __uint_as_float(s[cc + 1]));
             mx1 = max3(mx1, __uint_as_float(s[cc + 2]), __uint_as_float(s[cc + 3]));
             mx2 = max3(mx2, __uint_as_float(s[cc + 4]), __uint_as_float(s[cc + 5]));
@@ -466,14 +549,14 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         }
         const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);
         uint64_t sum2a = pack2(0.f, 0.f), sum2b = sum2a;
+        tmem_ld32(tS, buf[0]);
 #pragma unroll
-        for (int hf = 0; hf < 2; ++hf) {
-          uint32_t s[64];
-          tmem_ld32(tS + hf * 64, s);
-          tmem_ld32(tS + hf * 64 + 32, s + 32);
+        for (int c = 0; c < 4; ++c) {
           tc_wait_ld();
+          if (c < 3) tmem_ld32(tS + 32 * (c + 1), buf[(c + 1) & 1]);
+          uint32_t* s = buf[c & 1];
 #pragma unroll
-          for (int i = 0; i < 32; i += 2) {
+          for (int i = 0; i < 16; i += 2) {
             float a0, a1, b0, b1;
             unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
             unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
@@ -482,7 +565,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
             if (ragged) {
               // a masked key weighs EXACTLY 0 (its raw score may be anything; its V row may be a stale cache row)
-              const int c0 = hf * 64 + 2 * i;
+              const int c0 = 32 * c + 2 * i;
               a0 = c0 < limit ? a0 : 0.f;
               a1 = c0 + 1 < limit ? a1 : 0.f;
               b0 = c0 + 2 < limit ? b0 : 0.f;
@@ -493,7 +576,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             s[i] = pack_bf16(a0, a1);
             s[i + 1] = pack_bf16(b0, b1);
           }
-          tmem_st32(tS + hf * 32, s);
+          tmem_st16(tS + 16 * c, s);                         // P of keys [32c, 32c+32) -> columns [16c, 16c+16)
         }
         {
           float x0, x1;
@@ -506,8 +589,8 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         ++cme;
       }
       cother += (n - (w ^ 1) + 1) >> 1;                             // the other warpgroup's tiles of this segment
-      dec_segment_epilogue(prm, slen, d, w, r, tbase, lane_base, m, l, w ? cother : cme, w ? cme : cother,
-                           bar(D_OV), ml, flag);
+      dec_segment_epilogue(prm, d, w, r, tbase, lane_base, m, l, w ? cother : cme, w ? cme : cother, bar(D_OV), ml);
+      mbar_arrive(bar(D_PW + k));                                    // warp 11 counts and merges (fused tables)
       if ((threadIdx.x & 127) == 0) mbar_arrive(bar(D_DE + k));
     }
   }
@@ -588,20 +671,25 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
       }
     }
   }
-  // deal the segments to the CTAs in order: a CTA is closed once it holds its share of what is left
+  // deal the segments to the CTAs in order: a CTA is closed once it holds its share of what is left.  A segment
+  // costs its tiles plus a fixed part (pipeline fill and drain, query gather, partial write: about three tile times)
   const int grid = n_sm;
+  constexpr int64_t kSegCost = 3;
   std::vector<int32_t> cta_seg_off(grid + 1, 0);
   {
+    int64_t total = 0;
+    for (const DecSeg& sg : segs) total += sg.n_tiles + kSegCost;
     int64_t load = 0, done = 0;
     int cta = 0;
     for (size_t i = 0; i < segs.size(); ++i) {
-      const int64_t share = (units - done + (grid - cta) - 1) / std::max(1, grid - cta);
-      if (load > 0 && load + segs[i].n_tiles / 2 >= share && cta < grid - 1) {
+      const int64_t c = segs[i].n_tiles + kSegCost;
+      const int64_t share = (total - done + (grid - cta) - 1) / std::max(1, grid - cta);
+      if (load > 0 && load + c / 2 >= share && cta < grid - 1) {
         cta_seg_off[++cta] = (int32_t)i;
         done += load;
         load = 0;
       }
-      load += segs[i].n_tiles;
+      load += c;
     }
     for (int c = cta + 1; c <= grid; ++c) cta_seg_off[c] = (int32_t)segs.size();
   }
@@ -654,6 +742,9 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   t->dec_rows = part_rows * G;
   t->dec_self_row_base = row_off;
   t->dec_n_segs = (int32_t)segs.size();
+  t->dec_fused = t->B * Hq <= kFusedOut ? 1 : 0;
+  for (const DecSeg& sg : segs)
+    if (sg.n_seqs * G > kFusedRows) t->dec_fused = 0;
   t->dec_Hq = Hq;
   return CAS_OK;
 }
@@ -664,11 +755,16 @@ int tc_decode_fwd(const AttnArgs& a, const void* Kc, const void* Vc, int cache_c
   int rc = decode_prepare(t, a.Hq);
   if (rc) return rc;
   SelfLens sl;
+  sl.n_useq = 0;
   for (int b = 0; b < t->B; ++b) {
     const int len = Kc ? self_len[b] : 0;
+    const int npre = t->dec_comb_off[b + 1] - t->dec_comb_off[b];
     if (len < 0 || len > cache_cap) { set_error("self_len[%d] = %d outside [0, cache_cap]", b, len); return CAS_ERR_INVALID_ARG; }
-    if (len == 0 && t->dec_comb_off[b + 1] == t->dec_comb_off[b]) { set_error("sequence %d sees no key at all", b); return CAS_ERR_SHAPE; }
-    if (b < kMaxDecB) sl.v[b] = len;
+    if (len == 0 && npre == 0) { set_error("sequence %d sees no key at all", b); return CAS_ERR_SHAPE; }
+    if (b < kMaxDecB) {
+      sl.v[b] = len;
+      if (has_self_unit(len, npre)) sl.useq[sl.n_useq++] = b;
+    }
   }
   static SmemAttrOnce attr;
   rc = attr.set((const void*)tc_decode_kernel, (int)kDecSmem);
@@ -685,8 +781,12 @@ int tc_decode_fwd(const AttnArgs& a, const void* Kc, const void* Vc, int cache_c
   DecParams prm{t->d_dec_segs, t->d_dec_cta_off, t->d_dec_seqs, t->d_dec_tiles, t->d_seq_off, t->d_comb_off,
                 t->d_comb_row, (const __nv_bfloat16*)a.Q, (const __nv_bfloat16*)Kc, (const __nv_bfloat16*)Vc,
                 (__nv_bfloat16*)a.O_out, a.LSE_out, t->d_dec_part, t->d_dec_cnt, t->d_dec_ticket, t->dec_rows,
-                t->dec_self_row_base, cache_cap, t->B, a.Hq, a.Hkv, scale_log2};
+                t->dec_self_row_base, cache_cap, t->B, a.Hq, a.Hkv, t->dec_fused, scale_log2};
   tc_decode_kernel<<<(unsigned)t->dec_grid, kDecThreads, kDecSmem, a.stream>>>(a.L->tm_K, a.L->tm_V, tmKc, tmVc, prm, sl);
+  if (!t->dec_fused) {
+    const int n_w = t->B * a.Hq;
+    decode_combine_kernel<<<(n_w * 32 + 255) / 256, 256, 0, a.stream>>>(prm, sl);
+  }
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc decode launch");
 }
