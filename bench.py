@@ -197,60 +197,56 @@ def run_reference(args, wl):
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="c2")
-    ap.add_argument("--kernels", default="auto", choices=["auto", "simt", "tc"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-swap", action="store_true", help="c3: the same steps without rotation (overlap baseline)")
-    ap.add_argument("--ref-budget", type=float, default=8.0)
-    ap.add_argument("--ref-units", type=int, default=64)
-    args = ap.parse_args()
+def measure_host_link(torch, dev):
+    """Pinned-copy peak of the host link (not in MEASURED_PEAKS.json, so measured in the same run):
+    256 MiB copies, each direction alone and both at once, best of 4."""
+    hbuf = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+    hbuf2 = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
+    dbuf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    dbuf2 = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    s2 = torch.cuda.Stream()
+    best = {}
+    for name in ("h2d", "d2h", "both"):
+        ts = []
+        for _ in range(4):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            if name in ("h2d", "both"):
+                dbuf.copy_(hbuf, non_blocking=True)
+            if name in ("d2h", "both"):
+                with torch.cuda.stream(s2):
+                    hbuf2.copy_(dbuf2, non_blocking=True)
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+        best[name] = (256 << 20) / min(ts) / 1e9
+    return best
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
-    from workloads import BASE_SEED, CONFIGS, make_workload
-
-    cfg = CONFIGS[args.config]
-    if args.impl == "reference":
-        if rank == 0:
-            run_reference(args, make_workload(cfg, BASE_SEED))
-        return
-
+def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, do_cpu, no_swap=False, sustain_s=0.0):
+    """One workload: W warm-up steps, K timed steps (CUDA events on the launching stream, barrier + synchronize on
+    both sides, clocks sampled through NVML during the timed region).  Returns (line, ms_step_max) on every rank;
+    `line` is the JSON record on rank 0, None elsewhere."""
     import torch
 
-    from paper_2606_04557_b200 import _build, cas
+    from paper_2606_04557_b200 import cas
     from paper_2606_04557_b200.harness import Session
+    from workloads import BASE_SEED, CONFIGS, make_workload
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    _build.build()
-    torch.cuda.set_device(local_rank)
+    cfg = CONFIGS[cfg_name]
     dev = f"cuda:{local_rank}"
     if world > 1:
         import torch.distributed as dist
-
-        dist.init_process_group("nccl", device_id=torch.device(dev))
-    cas.cas_set_impl({"auto": 0, "simt": 1, "tc": 2}[args.kernels])
     wl = make_workload(cfg, BASE_SEED + rank)          # every rank: its own batch, its own pool
     sess = Session(wl, device=dev)
     stream = torch.cuda.current_stream()
     fwd_fl, bwd_fl = attn_flops(wl)
     # resident K+V elements the Adam call updates (with rotation: slots in transit this step are skipped, K4)
-    n_upd = cfg.n_slots - ((cfg.rotate_in + cfg.rotate_out) if (cfg.rotate_in > 0 and not args.no_swap) else 0)
-    n_el = 2 * int(sum(int(wl.cart_len[c]) for c in range(n_upd))) * cfg.Hkv * cfg.D
+    n_upd = cfg.n_slots - ((cfg.rotate_in + cfg.rotate_out) if (cfg.rotate_in > 0 and not no_swap) else 0)
     # algorithmic bytes (DESIGN.md section 5): 30 B per element of a slot that holds gradients this step (read g,p,m,v,
     # write p,m,v + bf16 copy), 26 B per element of a clean slot (g = 0 is not read).  Counted per step in prepare().
     adam_acc = {"bytes": 0, "steps": 0}
 
-    rotate = cfg.rotate_in > 0 and not args.no_swap
+    rotate = cfg.rotate_in > 0 and not no_swap
     rot = {"step": 0, "rng": np.random.Generator(np.random.PCG64(BASE_SEED + 1000 + rank)), "bytes": 0}
     if cfg.rotate_in > 0:
         from workloads.generate import draw_batch_selection
@@ -265,6 +261,7 @@ def main():
             c = cas.cas_pool_counters(sess.pool)
             stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
             sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
+        rot["sel"] = (sel_off, sel_cart)
         if cfg.backward:
             used = set(int(x) for x in sel_cart)
             el = lambda c: 2 * int(wl.cart_len[c]) * cfg.Hkv * cfg.D
@@ -277,10 +274,8 @@ def main():
         if cfg.backward or tau == 0:
             # training: a new batch and a new slot table every step.  Decode (c5): the selection is fixed while
             # a request generates, so the table (and its split-KV work list) is built once and reused per token.
-            t_host = time.perf_counter()
             sess.tab.close()
             sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, sel_off, sel_cart, tau)
-            rot["table_ms"] = (time.perf_counter() - t_host) * 1e3
         if rotate:
             prot = sorted(set(int(x) for x in sel_cart))
             man, n = cas.cas_plan_rotation(sess.pool, tau, cfg.rotate_in, cfg.rotate_out, prot, 260604)
@@ -315,25 +310,52 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    def timed(n_steps):
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(n_steps)]
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(local_rank)
+        barrier()
+        sampler.start()
+        e0.record(stream)
+        for i in range(n_steps):
+            step(evs[i])
+        e1.record(stream)
+        barrier()
+        sampler.stop_flag = True
+        sampler.join(timeout=1.0)
+        return e0.elapsed_time(e1), evs, sampler.summary()
+
+    for _ in range(max(warmup, 3)):
         step()
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local_rank)
-    barrier()
-    sampler.start()
-    e0.record(stream)
-    for i in range(args.steps):
-        step(evs[i])
-    e1.record(stream)
-    barrier()
-    sampler.stop_flag = True
-    total_ms = e0.elapsed_time(e1)
+    total_ms, evs, clocks = timed(steps)
     adam_bytes = adam_acc["bytes"] / max(adam_acc["steps"], 1)
     t_fwd = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     t_bwd = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     t_adam = float(np.mean([e[2].elapsed_time(e[3]) for e in evs]))
-    ms_step = total_ms / args.steps
+    ms_step = total_ms / steps
+
+    # ---- the same steps back to back for >= sustain_s seconds: the clocks settle under the power cap
+    sustained = None
+    if sustain_s > 0:
+        n_sus = max(steps, int(sustain_s * 1e3 / ms_step) + 1)
+        s_ms, s_evs, s_clk = timed(n_sus)
+        sustained = {"seconds": s_ms * 1e-3, "steps": n_sus, "ms_per_step": s_ms / n_sus,
+                     "fwd_ms": float(np.mean([e[0].elapsed_time(e[1]) for e in s_evs])),
+                     "bwd_ms": float(np.mean([e[1].elapsed_time(e[2]) for e in s_evs])),
+                     "adam_ms": float(np.mean([e[2].elapsed_time(e[3]) for e in s_evs])), "clocks": s_clk}
+
+    # ---- host time of one slot-table build on an IDLE blob ring (nothing in flight): median of 9
+    table_ms = None
+    if rank == 0:
+        torch.cuda.synchronize()
+        ts = []
+        for i in range(9):
+            t0 = time.perf_counter()
+            tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, rot["sel"][0], rot["sel"][1], rot["step"] - 1)
+            ts.append((time.perf_counter() - t0) * 1e3)
+            tab.close()
+            torch.cuda.synchronize()
+        table_ms = float(np.median(ts))
 
     # ---- c3: the swap alone (no compute on the main stream) and the host link's own pinned-copy peak
     swap_only = None
@@ -350,34 +372,15 @@ def main():
         barrier()
         swap_ms = a.elapsed_time(b) / 4
         per_dir = (rot["bytes"] - b0) / 4 / 2
-        hbuf = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
-        hbuf2 = torch.empty(256 << 20, dtype=torch.uint8).pin_memory()
-        dbuf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-        dbuf2 = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-        s2 = torch.cuda.Stream()
-        best = {}
-        for name in ("h2d", "d2h", "both"):
-            ts = []
-            for _ in range(4):
-                torch.cuda.synchronize()
-                t0 = time.perf_counter()
-                if name in ("h2d", "both"):
-                    dbuf.copy_(hbuf, non_blocking=True)
-                if name in ("d2h", "both"):
-                    with torch.cuda.stream(s2):
-                        hbuf2.copy_(dbuf2, non_blocking=True)
-                torch.cuda.synchronize()
-                ts.append(time.perf_counter() - t0)
-            best[name] = (256 << 20) / min(ts) / 1e9
+        best = measure_host_link(torch, dev)
         swap_only = {"ms": swap_ms, "gbs_per_direction": per_dir / (swap_ms * 1e-3) / 1e9,
                      "host_link_h2d_gbs": best["h2d"], "host_link_d2h_gbs": best["d2h"],
                      "host_link_bidir_gbs_per_direction": best["both"],
                      "frac_of_host_link": per_dir / (swap_ms * 1e-3) / 1e9 / best["both"]}
-        del hbuf, hbuf2, dbuf, dbuf2
 
     # ---- e2e: host buffers through cas_train_step_host
     e2e = None
-    if cfg.backward and not args.no_e2e:
+    if cfg.backward and do_e2e:
         tdt = sess.tdt
         pin = lambda a: torch.from_numpy(a).to(tdt).pin_memory()
         hQ, hKs, hVs, hdO = pin(wl.Q), pin(wl.K_self), pin(wl.V_self), pin(wl.dO)
@@ -400,28 +403,33 @@ def main():
         barrier()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
-        for _ in range(args.steps):
+        for _ in range(steps):
             e2e_step()
         b.record(stream)
         barrier()
-        e2e_ms = a.elapsed_time(b) / args.steps
+        e2e_ms = a.elapsed_time(b) / steps
         h2d = sum(t.numel() * t.element_size() for t in (hQ, hKs, hVs, hdO))
         d2h = sum(t.numel() * t.element_size() for t in (hO, hdQ, hLSE, hdKs, hdVs))
         e2e = (e2e_ms, h2d, d2h)
 
     ms_step_max, e2e_ms_max, total_flops = reduce_over_ranks(ms_step, e2e[0] if e2e else 0.0, fwd_fl + bwd_fl,
                                                              world, dev)
-
+    line = None
     if rank == 0:
         peaks = load_peaks()
         tc = bool(cfg.dtype == "bf16" and cfg.D == 128 and args.kernels != "simt")
         dom_fl, dom_ms, dom_name = (bwd_fl, t_bwd, "attn_bwd") if cfg.backward else (fwd_fl, t_fwd, "attn_fwd")
         achieved = dom_fl / (dom_ms * 1e-3) / 1e12
-        traffic = load_traffic().get(args.config, {}).get(dom_name)
-        roof = {"kernel": dom_name, "bound": "tensor", "achieved": achieved, "peak": peaks["bf16_sust"],
-                "unit": "TFLOP/s", "frac": achieved / peaks["bf16_sust"], "traffic": traffic,
-                "peak_source": peaks["src"] + " bf16_tflops_sustained (kernel timed inside the step)",
-                "frac_of_burst_peak": achieved / peaks["bf16"]}
+        traffic = load_traffic().get(cfg_name, {}).get(dom_name)
+        # denominator: the BURST bf16 peak when the timed region is short (the clocks have not settled under the power
+        # cap -- what MEASURED_PEAKS' burst figure was taken at), the sustained one for a seconds-long region
+        burst = total_ms < 1000.0
+        pk = peaks["bf16"] if burst else peaks["bf16_sust"]
+        roof = {"kernel": dom_name, "bound": "tensor", "achieved": achieved, "peak": pk,
+                "unit": "TFLOP/s", "frac": achieved / pk, "traffic": traffic,
+                "peak_source": peaks["src"] + (" bf16_tflops (burst: timed region %.0f ms)" % total_ms if burst else
+                                               " bf16_tflops_sustained (timed region %.1f s)" % (total_ms * 1e-3)),
+                "frac_of_burst_peak": achieved / peaks["bf16"], "frac_of_sustained_peak": achieved / peaks["bf16_sust"]}
         if not cfg.backward:
             # decode (c5): HBM-bound; algorithmic bytes = unique selected K+V bytes + Q + O
             uniq = sorted(set(int(x) for x in wl.sel_cart))
@@ -431,9 +439,10 @@ def main():
             roof = {"kernel": "attn_fwd", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
                     "frac": gbs / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " hbm_gbs",
                     "algorithmic_bytes": kv_bytes + io_bytes, "tflops": achieved}
+        n_launch = 5 if cfg.backward else (1 if sess.tab.B * cfg.Hq <= 256 else 2)
         line = {
             "metric": METRIC, "value": total_flops / (ms_step_max * 1e-3) / 1e12, "unit": UNIT,
-            "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step_max,
+            "n_gpus": world, "steps": steps, "warmup": max(warmup, 3), "ms_per_step": ms_step_max,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16" if cfg.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": cfg.name, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_carts": cfg.n_carts,
@@ -442,20 +451,30 @@ def main():
                        "l2": "inputs larger than L2 (pool + optimizer state > 1 GB per step)",
                        "slot_table": ("rebuilt every step (inside the timed region)" if cfg.backward else
                                       "built once before the timed region (selection fixed during generation)"),
-                       "slot_table_build_host_ms": rot.get("table_ms"),
+                       "slot_table_build_host_ms": table_ms,
+                       "slot_table_build_note": "median of 9 builds on an idle blob ring (host time only)",
                        "parallelism": "replicas" if world > 1 else "single"},
             "breakdown": {"fwd_ms": t_fwd, "bwd_ms": t_bwd, "adam_ms": t_adam,
                           "fwd_tflops": fwd_fl / (t_fwd * 1e-3) / 1e12,
                           "bwd_tflops": (bwd_fl / (t_bwd * 1e-3) / 1e12) if cfg.backward else None,
                           "fwd_bwd_tflops": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12,
-                          "fwd_bwd_frac_of_bf16_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16_sust"],
+                          "fwd_bwd_frac_of_bf16_sustained_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16_sust"],
                           "fwd_bwd_frac_of_bf16_burst_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16"],
                           "adam_gbs": (adam_bytes / (t_adam * 1e-3) / 1e9) if cfg.backward else None,
-                          "adam_frac_of_hbm_peak": (adam_bytes / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if cfg.backward else None},
+                          "adam_frac_of_hbm_peak": (adam_bytes / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if cfg.backward else None,
+                          "adam_note": ("algorithmic 30/26 B per element; a fraction above 1 means part of it is served by "
+                                        "L2 (gradient rows the backward pass has just written): see roofline traffic in "
+                                        "profiles/") if cfg.backward else None},
             "roofline": roof,
-            "gpu_launches": args.steps * ((5 if cfg.backward else 1) + (cfg.rotate_in if rotate else 0)),
-            "clocks": sampler.summary(),
+            "gpu_launches": steps * (n_launch + (cfg.rotate_in if rotate else 0)),
+            "clocks": clocks,
         }
+        if sustained:
+            s_fb = (fwd_fl + bwd_fl) / ((sustained["fwd_ms"] + sustained["bwd_ms"]) * 1e-3) / 1e12
+            sustained.update({"value": (fwd_fl + bwd_fl) / (sustained["ms_per_step"] * 1e-3) / 1e12,
+                              "fwd_bwd_tflops": s_fb, "fwd_bwd_frac_of_bf16_sustained_peak": s_fb / peaks["bf16_sust"],
+                              "bwd_tflops": bwd_fl / (sustained["bwd_ms"] * 1e-3) / 1e12 if cfg.backward else None})
+            line["sustained"] = sustained
         if cfg.rotate_in > 0:
             per_step = rot["bytes"] / max(rot["step"], 1)
             line["swap"] = {"enabled": rotate, "bytes_per_step_both_directions": per_step,
@@ -465,12 +484,93 @@ def main():
         if e2e:
             line["e2e"] = {"value": total_flops / (e2e_ms_max * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms_max,
                            "h2d_bytes_per_step": e2e[1], "d2h_bytes_per_step": e2e[2]}
-        if not args.no_cpu_baseline and world == 1:
+        if do_cpu and world == 1:
             tf, desc, secs, threads = oracle_sample(wl, budget_s=12.0)
             line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
-                                    "seconds": secs}
-        print(json.dumps(line))
+                                    "seconds": secs, "note": "numpy float64 oracle as it stands, not tuned"}
     sess.close()
+    del sess, wl
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    return line
+
+
+def compact(line):
+    """The part of a config's record that goes into the headline line's `extra` block."""
+    b, r = line["breakdown"], line["roofline"]
+    out = {"ms_per_step": line["ms_per_step"], "fwd_ms": b["fwd_ms"], "steps": line["steps"], "clocks": line["clocks"],
+           "T": line["config"]["T"], "pairs_per_head": line["config"]["pairs_per_head"]}
+    if b["bwd_tflops"] is not None:
+        out.update({"bwd_ms": b["bwd_ms"], "adam_ms": b["adam_ms"], "fwd_tflops": b["fwd_tflops"],
+                    "bwd_tflops": b["bwd_tflops"], "fwd_bwd_tflops": b["fwd_bwd_tflops"],
+                    "fwd_bwd_frac_of_bf16_burst_peak": b["fwd_bwd_frac_of_bf16_burst_peak"],
+                    "fwd_bwd_frac_of_bf16_sustained_peak": b["fwd_bwd_frac_of_bf16_sustained_peak"],
+                    "adam_gbs": b["adam_gbs"], "adam_frac_of_hbm_peak": b["adam_frac_of_hbm_peak"]})
+    else:
+        out.update({"hbm_gbs_unique_kv": r["achieved"], "frac_of_hbm_peak": r["frac"], "tflops": r["tflops"]})
+    if "swap" in line:
+        out["swap"] = line["swap"]
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c2")
+    ap.add_argument("--kernels", default="auto", choices=["auto", "simt", "tc"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-swap", action="store_true", help="c3: the same steps without rotation (overlap baseline)")
+    ap.add_argument("--no-extra", action="store_true", help="headline config only (no c3/c4/c5 records, no sustained loop)")
+    ap.add_argument("--ref-budget", type=float, default=8.0)
+    ap.add_argument("--ref-units", type=int, default=64)
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from workloads import BASE_SEED, CONFIGS, make_workload
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, make_workload(CONFIGS[args.config], BASE_SEED))
+        return
+
+    import torch
+
+    from paper_2606_04557_b200 import _build, cas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    _build.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    cas.cas_set_impl({"auto": 0, "simt": 1, "tc": 2}[args.kernels])
+    headline = args.config == "c2" and not args.no_extra and world == 1
+    line = run_config(args, args.config, args.steps, args.warmup, rank, world, local_rank, do_e2e=not args.no_e2e,
+                      do_cpu=not args.no_cpu_baseline, no_swap=args.no_swap, sustain_s=3.0 if headline else 0.0)
+    if headline:
+        # BASELINE.json's metric spans five configs: one compact record each for the others (fewer steps; the
+        # headline stays c2).  c3 twice: with rotation overlapped, and the same steps without it.
+        extra = {}
+        for name, kw in (("c3", {}), ("c3_no_swap", {"no_swap": True}), ("c4", {}), ("c5_all", {}), ("c5_top8", {})):
+            cname = "c3" if name.startswith("c3") else name
+            st = {"c3": 8, "c4": 4}.get(cname, 30)
+            rec = run_config(args, cname, st, 3, rank, world, local_rank, do_e2e=False, do_cpu=False, **kw)
+            extra[name] = compact(rec)
+        if "c3" in extra and "c3_no_swap" in extra:
+            extra["c3"]["overlap_efficiency"] = extra["c3_no_swap"]["ms_per_step"] / extra["c3"]["ms_per_step"]
+        line["extra"] = extra
+    if rank == 0:
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

@@ -78,6 +78,15 @@ typedef struct {
                                layout; the device arena holds L carvings back to back, a cartridge's pinned home
                                L x (pK,pV,mK,mV,vK,vV).  Residency, step counts and rotation are per cartridge
                                (all layers move together); gradients-dirty is tracked per (layer, slot) */
+  int64_t pool_tokens_budget; /* 0: static slots (above).  > 0: PAGED pool (PAPER.md:442-446:
+                               cartridge sizes are multiples of the 16-token page of the paged KV cache, "enabling
+                               efficient memory allocation and deallocation during ... pool rotation").  The pool holds
+                               pool_tokens_budget tokens (a multiple of tile_tokens, which must then be given) = that many
+                               pages of tile_tokens tokens; a resident cartridge owns a CONTIGUOUS run of
+                               ceil(len/tile_tokens) pages chosen first-fit (lowest base) when it arrives and freed when
+                               it leaves; the n_slots slots are handles (the most cartridges resident at once) whose
+                               base and capacity follow their occupant.  Cartridges 0..n_slots-1 are placed first-fit
+                               in order at creation (CAS_ERR_CAPACITY if they do not fit). */
 } cas_pool_desc;
 
 /* Device-side layout of the pool inside the caller's arena (all pointers are device pointers
@@ -91,7 +100,8 @@ typedef struct {
   float* grad_V;
   float* state;             /* per slot s at state + 6*slot_base[s]*Hkv*D: six fp32 tensors of
                                slot_cap[s]*Hkv*D elements each: pK, pV, mK, mV, vK, vV */
-  const int32_t* slot_base; /* host [n_slots] first pool token of slot s */
+  const int32_t* slot_base; /* host [n_slots] first pool token of slot s (paged pool: of its current occupant;
+                               valid until the next cas_swap_in) */
   const int32_t* slot_cap;  /* host [n_slots] capacity in tokens (multiple of tile_tokens) */
   int64_t pool_tokens;
 } cas_pool_layout;
@@ -100,7 +110,8 @@ typedef struct {
   int32_t cart;
   int32_t slot;
   int32_t dir;              /* CAS_DIR_OUT | CAS_DIR_IN */
-  int32_t reserved;
+  int32_t base_tok;         /* first pool token of the cartridge's extent: where it sits (OUT) / where it goes (IN).
+                               Static slots: slot_base[slot]; paged pool: the first-fit run the planner chose */
   int64_t host_off;         /* byte offset of the cartridge's home in the pinned arena */
   int64_t nbytes;           /* 6 * cart_len * Hkv * D * 4 (params + both Adam moments, K and V) */
 } cas_manifest_entry;
@@ -267,7 +278,10 @@ int cas_grad_zero(cas_pool* pool, const int32_t* slots, int32_t n, void* stream)
  * cartridges with the fewest opt_steps (ties: smaller mix64(seed,step,cart), then smaller id),
  * paired in that order with the free slots (free now or freed by the evictees) in ascending slot
  * order.  Writes all OUT entries (ascending slot) then all IN entries.  CAS_ERR_CAPACITY if
- * `capacity` entries do not suffice. */
+ * `capacity` entries do not suffice.  Paged pool: an arrival takes the lowest unused slot handle and the
+ * first-fit run of pages that are free now or freed by this round's evictees and not taken by an earlier arrival of
+ * the plan (entry.base_tok); a cartridge for which no run is long enough is skipped (fragmentation -- the paper's
+ * own implementation empties its allocator cache every 5 rotations for the same reason). */
 int cas_plan_rotation(const cas_pool* pool, int64_t step, int32_t n_in, int32_t n_out,
                       const int32_t* protect_carts, int32_t n_protect, uint64_t seed,
                       cas_manifest_entry* entries, int32_t capacity, int32_t* n_entries);

@@ -48,16 +48,17 @@ class ManifestEntry:
     dir: int
     host_off: int
     nbytes: int
+    base_tok: int = 0        # first pool token of the cartridge's extent (OUT: where it sits, IN: where it goes)
 
     def as_tuple(self):
-        return (self.cart, self.slot, self.dir, self.host_off, self.nbytes)
+        return (self.cart, self.slot, self.dir, self.base_tok, self.host_off, self.nbytes)
 
 
 class PoolBook:
     """Integer state of the cartridge pool."""
 
     def __init__(self, cart_len: Sequence[int], n_slots: int, Hkv: int, D: int,
-                 tile_tokens: int = 128, n_layers: int = 1):
+                 tile_tokens: int = 128, n_layers: int = 1, budget_tokens: int = 0):
         self.n_layers = int(n_layers)               # PAPER.md:42: Z in R^{L x p x d x 2}; a home holds all L layers
         self.cart_len = [int(x) for x in cart_len]
         self.n_carts = len(self.cart_len)
@@ -65,17 +66,40 @@ class PoolBook:
         self.row_elems = Hkv * D
         self.tile = tile_tokens
         up = lambda x: (x + tile_tokens - 1) // tile_tokens * tile_tokens
-        # slot capacities: everything resident -> slot s is sized for cartridge s;
-        # otherwise uniform slots sized for the longest cartridge.
-        if self.n_slots == self.n_carts:
-            self.slot_cap = [up(l) for l in self.cart_len]
+        # PAGED pool (budget_tokens > 0; cartridge sizes are multiples of the 16-token page of the
+        # paged KV cache, "enabling efficient memory allocation and deallocation during ... pool rotation"): the pool
+        # is budget_tokens/tile pages; a resident cartridge owns a contiguous run of ceil(len/tile) pages chosen
+        # first-fit (lowest base); slots are mere handles whose base/capacity change with their occupant.
+        self.budget = int(budget_tokens)
+        self.paged = self.budget > 0
+        if self.paged:
+            assert self.budget % tile_tokens == 0
+            self.n_pages = self.budget // tile_tokens
+            self.page_owner = [-1] * self.n_pages       # committed owner (cartridge id) of every page
+            self.page_claim = [-1] * self.n_pages       # arrival in flight that will own the page at commit
+            self.slot_cap = [0] * self.n_slots
+            self.slot_base = [0] * self.n_slots
+            for c in range(min(self.n_slots, self.n_carts)):
+                n = up(self.cart_len[c]) // tile_tokens
+                base = self._first_fit(n, lambda o, cl: o < 0 and cl < 0)
+                if base < 0:
+                    raise BookError("CAPACITY", "initial cartridges do not fit the page budget")
+                for q in range(base, base + n):
+                    self.page_owner[q] = c
+                self.slot_base[c], self.slot_cap[c] = base * tile_tokens, n * tile_tokens
+            self.pool_tokens = self.budget
         else:
-            cap = up(max(self.cart_len))
-            self.slot_cap = [cap] * self.n_slots
-        self.slot_base = [0] * self.n_slots
-        for s in range(1, self.n_slots):
-            self.slot_base[s] = self.slot_base[s - 1] + self.slot_cap[s - 1]
-        self.pool_tokens = self.slot_base[-1] + self.slot_cap[-1] if self.n_slots else 0
+            # slot capacities: everything resident -> slot s is sized for cartridge s;
+            # otherwise uniform slots sized for the longest cartridge.
+            if self.n_slots == self.n_carts:
+                self.slot_cap = [up(l) for l in self.cart_len]
+            else:
+                cap = up(max(self.cart_len))
+                self.slot_cap = [cap] * self.n_slots
+            self.slot_base = [0] * self.n_slots
+            for s in range(1, self.n_slots):
+                self.slot_base[s] = self.slot_base[s - 1] + self.slot_cap[s - 1]
+            self.pool_tokens = self.slot_base[-1] + self.slot_cap[-1] if self.n_slots else 0
         # pinned homes: 6 fp32 tensors (pK,pV,mK,mV,vK,vV) of len*Hkv*D per cartridge, packed
         self.home_off = [0] * self.n_carts
         for c in range(1, self.n_carts):
@@ -91,6 +115,18 @@ class PoolBook:
         self.in_transit = [0] * self.n_carts        # 0 stable, 1 leaving, 2 arriving
         self.grad_dirty = [0] * self.n_slots
         self.pending: List[Tuple[ManifestEntry, int]] = []   # (entry, plan step)
+
+    def _first_fit(self, n: int, free) -> int:
+        """Lowest base page of a run of n pages that are all free(owner, claim); -1 if there is none."""
+        run = 0
+        for q in range(self.n_pages):
+            run = run + 1 if free(self.page_owner[q], self.page_claim[q]) else 0
+            if run == n:
+                return q - n + 1
+        return -1
+
+    def pages_of(self, c: int) -> List[int]:
+        return [q for q in range(self.n_pages) if self.page_owner[q] == c]
 
     def home_bytes(self, c: int) -> int:
         return self.n_layers * 6 * self.cart_len[c] * self.row_elems * 4
@@ -154,19 +190,45 @@ class PoolBook:
         free.sort()
         arrivals = []
         used = set()
-        for c in waiting:
-            if len(arrivals) >= max(0, n_in):
-                break
-            # first free slot (ascending) that is large enough and not yet paired
-            for s in free:
-                if s not in used and self.slot_cap[s] >= self.cart_len[c]:
-                    used.add(s)
-                    arrivals.append((c, s))
+        if self.paged:
+            # the lowest unused slot handle + the first-fit run of pages that are free now, or are freed by this round's
+            # evictees, and that no earlier arrival of this plan has taken; a cartridge that fits nowhere is skipped
+            ev = set(evictees)
+            taken = [False] * self.n_pages
+            for c in waiting:
+                if len(arrivals) >= max(0, n_in):
                     break
+                hs = [s for s in free if s not in used]
+                if not hs:
+                    break
+                n = -(-self.cart_len[c] // self.tile)
+                run, base = 0, -1
+                for q in range(self.n_pages):
+                    ok = (self.page_owner[q] < 0 or self.page_owner[q] in ev) and self.page_claim[q] < 0 and not taken[q]
+                    run = run + 1 if ok else 0
+                    if run == n:
+                        base = q - n + 1
+                        break
+                if base < 0:
+                    continue
+                for q in range(base, base + n):
+                    taken[q] = True
+                used.add(hs[0])
+                arrivals.append((c, hs[0], base * self.tile))
+        else:
+            for c in waiting:
+                if len(arrivals) >= max(0, n_in):
+                    break
+                # first free slot (ascending) that is large enough and not yet paired
+                for s in free:
+                    if s not in used and self.slot_cap[s] >= self.cart_len[c]:
+                        used.add(s)
+                        arrivals.append((c, s, self.slot_base[s]))
+                        break
         outs = sorted(((self.slot_of[c], c) for c in evictees))
-        man = [ManifestEntry(c, s, DIR_OUT, self.home_off[c], self.home_bytes(c)) for s, c in outs]
-        man += [ManifestEntry(c, s, DIR_IN, self.home_off[c], self.home_bytes(c))
-                for c, s in arrivals]
+        man = [ManifestEntry(c, s, DIR_OUT, self.home_off[c], self.home_bytes(c), self.slot_base[s]) for s, c in outs]
+        man += [ManifestEntry(c, s, DIR_IN, self.home_off[c], self.home_bytes(c), bt)
+                for c, s, bt in arrivals]
         return man
 
     # ---- K4 (state transitions of swap_out / swap_in / commit / adam) -------------------------
@@ -192,12 +254,27 @@ class PoolBook:
                 raise BookError("BUSY", "arrival already resident / in transit")
             if not (self.cart_in[e.slot] < 0 or e.slot in leaving):
                 raise BookError("BUSY", "slot occupied")
-            if self.slot_cap[e.slot] < self.cart_len[e.cart]:
+            if not self.paged and self.slot_cap[e.slot] < self.cart_len[e.cart]:
                 raise BookError("CAPACITY")
+            if self.paged:
+                n = -(-self.cart_len[e.cart] // self.tile)
+                b = e.base_tok // self.tile
+                if e.base_tok % self.tile or b < 0 or b + n > self.n_pages:
+                    raise BookError("INVALID_ARG", "extent")
+                for q in range(b, b + n):
+                    o = self.page_owner[q]
+                    if self.page_claim[q] >= 0 or (o >= 0 and self.in_transit[o] != 1):
+                        raise BookError("BUSY", "page occupied")
         for e in man:
             if e.dir == DIR_IN:
                 self.in_transit[e.cart] = 2
                 self.pending.append((e, step))
+                if self.paged:
+                    n = -(-self.cart_len[e.cart] // self.tile)
+                    b = e.base_tok // self.tile
+                    for q in range(b, b + n):
+                        self.page_claim[q] = e.cart
+                    self.slot_base[e.slot], self.slot_cap[e.slot] = e.base_tok, n * self.tile
 
     def commit(self):
         for e, step in self.pending:
@@ -206,12 +283,20 @@ class PoolBook:
                 self.in_transit[e.cart] = 0
                 if self.cart_in[e.slot] == e.cart:
                     self.cart_in[e.slot] = -1
+                if self.paged:
+                    for q in range(self.n_pages):
+                        if self.page_owner[q] == e.cart:
+                            self.page_owner[q] = -1
         for e, step in self.pending:
             if e.dir == DIR_IN:
                 self.slot_of[e.cart] = e.slot
                 self.cart_in[e.slot] = e.cart
                 self.in_transit[e.cart] = 0
                 self.last_used[e.cart] = step
+                if self.paged:
+                    for q in range(self.n_pages):
+                        if self.page_claim[q] == e.cart:
+                            self.page_owner[q], self.page_claim[q] = e.cart, -1
         self.pending = []
 
     def mark_grads(self, sel_slot: Sequence[int]):

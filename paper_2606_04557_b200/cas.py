@@ -33,7 +33,7 @@ class CasError(RuntimeError):
 class PoolDesc(C.Structure):
     _fields_ = [("dtype", C.c_int32), ("Hkv", C.c_int32), ("D", C.c_int32), ("n_carts", C.c_int32),
                 ("n_slots", C.c_int32), ("tile_tokens", C.c_int32), ("cart_len", C.POINTER(C.c_int32)),
-                ("n_layers", C.c_int32)]
+                ("n_layers", C.c_int32), ("pool_tokens_budget", C.c_int64)]
 
 
 class PoolLayout(C.Structure):
@@ -43,11 +43,11 @@ class PoolLayout(C.Structure):
 
 
 class ManifestEntry(C.Structure):
-    _fields_ = [("cart", C.c_int32), ("slot", C.c_int32), ("dir", C.c_int32), ("reserved", C.c_int32),
+    _fields_ = [("cart", C.c_int32), ("slot", C.c_int32), ("dir", C.c_int32), ("base_tok", C.c_int32),
                 ("host_off", C.c_int64), ("nbytes", C.c_int64)]
 
     def as_tuple(self):
-        return (self.cart, self.slot, self.dir, self.host_off, self.nbytes)
+        return (self.cart, self.slot, self.dir, self.base_tok, self.host_off, self.nbytes)
 
 
 class AdamCfg(C.Structure):
@@ -121,11 +121,12 @@ class Pool:
     """Owns the torch tensors backing the arenas + the opaque cas_pool handle."""
 
     def __init__(self, dtype: int, Hkv: int, D: int, cart_len: Sequence[int], n_slots: int,
-                 tile_tokens: int = 0, device: Optional[str] = "cuda:0", side_stream=None, n_layers: int = 1):
+                 tile_tokens: int = 0, device: Optional[str] = "cuda:0", side_stream=None, n_layers: int = 1,
+                 budget_tokens: int = 0):
         self._cart_len = _i32(cart_len)
         self.n_layers = n_layers
         self.desc = PoolDesc(dtype, Hkv, D, len(self._cart_len), n_slots, tile_tokens,
-                             _p(self._cart_len), n_layers)
+                             _p(self._cart_len), n_layers, budget_tokens)
         self.dtype, self.Hkv, self.D = dtype, Hkv, D
         self.n_carts, self.n_slots = len(self._cart_len), n_slots
         self.dev_bytes, self.host_bytes = cas_pool_query_bytes(self.desc)
@@ -146,9 +147,20 @@ class Pool:
         lay = PoolLayout()
         _check(lib().cas_pool_layout_get(self.handle, C.byref(lay)))
         self.layout = lay
-        self.slot_base = np.ctypeslib.as_array(lay.slot_base, (n_slots,)).copy()
-        self.slot_cap = np.ctypeslib.as_array(lay.slot_cap, (n_slots,)).copy()
         self.pool_tokens = lay.pool_tokens
+
+    @property
+    def slot_base(self) -> np.ndarray:
+        """First pool token of every slot (in a paged pool it changes with the slot's occupant: read it afresh)."""
+        lay = PoolLayout()
+        _check(lib().cas_pool_layout_get(self.handle, C.byref(lay)))
+        return np.ctypeslib.as_array(lay.slot_base, (self.n_slots,)).copy()
+
+    @property
+    def slot_cap(self) -> np.ndarray:
+        lay = PoolLayout()
+        _check(lib().cas_pool_layout_get(self.handle, C.byref(lay)))
+        return np.ctypeslib.as_array(lay.slot_cap, (self.n_slots,)).copy()
 
     def close(self):
         if self.handle:

@@ -64,17 +64,48 @@ static int check_desc(const cas_pool_desc* d) {
   if (d->n_carts < 1 || d->n_slots < 1 || d->n_slots > d->n_carts) { set_error("need 1 <= n_slots <= n_carts"); return CAS_ERR_INVALID_ARG; }
   if (d->n_slots > kMaxSlots) { set_error("at most %d slots", kMaxSlots); return CAS_ERR_CAPACITY; }
   if (d->n_layers < 0 || d->n_layers > 1024) { set_error("n_layers must be in [0, 1024] (0 = 1)"); return CAS_ERR_INVALID_ARG; }
+  if (d->pool_tokens_budget < 0 || (d->pool_tokens_budget > 0 && (d->tile_tokens == 0 || d->pool_tokens_budget % d->tile_tokens))) {
+    set_error("pool_tokens_budget must be a positive multiple of an explicit tile_tokens");
+    return CAS_ERR_INVALID_ARG;
+  }
   if (d->tile_tokens < 0 || (d->tile_tokens && d->tile_tokens % 16)) { set_error("tile_tokens must be a multiple of 16"); return CAS_ERR_INVALID_ARG; }
   for (int i = 0; i < d->n_carts; ++i)
     if (d->cart_len[i] < 1) { set_error("cart_len[%d] < 1", i); return CAS_ERR_INVALID_ARG; }
   return CAS_OK;
 }
 
-static void layout_slots(const cas_pool_desc* d, std::vector<int32_t>& base, std::vector<int32_t>& cap,
-                         int64_t& pool_tokens) {
+// Lowest base page of a run of n pages that are all free per `ok(page)`; -1 if there is none (first fit).
+template <typename F>
+static int32_t first_fit(int32_t n_pages, int32_t n, F ok) {
+  int32_t run = 0;
+  for (int32_t q = 0; q < n_pages; ++q) {
+    run = ok(q) ? run + 1 : 0;
+    if (run == n) return q - n + 1;
+  }
+  return -1;
+}
+
+// returns false if the initial cartridges of a paged pool do not fit its budget
+static bool layout_slots(const cas_pool_desc* d, std::vector<int32_t>& base, std::vector<int32_t>& cap,
+                         int64_t& pool_tokens, std::vector<int32_t>* page_owner = nullptr) {
   const int tile = d->tile_tokens ? d->tile_tokens : 128;
   base.assign(d->n_slots, 0);
   cap.assign(d->n_slots, 0);
+  if (d->pool_tokens_budget > 0) {
+    const int32_t n_pages = (int32_t)(d->pool_tokens_budget / tile);
+    std::vector<int32_t> owner(n_pages, -1);
+    for (int c = 0; c < d->n_slots; ++c) {
+      const int32_t n = (d->cart_len[c] + tile - 1) / tile;
+      const int32_t b = first_fit(n_pages, n, [&](int32_t q) { return owner[q] < 0; });
+      if (b < 0) return false;
+      for (int32_t q = b; q < b + n; ++q) owner[q] = c;
+      base[c] = b * tile;
+      cap[c] = n * tile;
+    }
+    pool_tokens = d->pool_tokens_budget;
+    if (page_owner) *page_owner = owner;
+    return true;
+  }
   if (d->n_slots == d->n_carts) {
     for (int s = 0; s < d->n_slots; ++s) cap[s] = (int32_t)round_up(d->cart_len[s], tile);
   } else {
@@ -85,6 +116,7 @@ static void layout_slots(const cas_pool_desc* d, std::vector<int32_t>& base, std
   int64_t o = 0;
   for (int s = 0; s < d->n_slots; ++s) { base[s] = (int32_t)o; o += cap[s]; }
   pool_tokens = o;
+  return true;
 }
 
 template <typename T>
@@ -119,7 +151,7 @@ int cas_pool_query_bytes(const cas_pool_desc* desc, size_t* dev_bytes, size_t* h
   if (rc) return rc;
   std::vector<int32_t> base, cap;
   int64_t pool_tokens;
-  layout_slots(desc, base, cap, pool_tokens);
+  if (!layout_slots(desc, base, cap, pool_tokens)) { set_error("the first n_slots cartridges do not fit pool_tokens_budget"); return CAS_ERR_CAPACITY; }
   if (pool_tokens >= (1ll << 31)) { set_error("pool too large for int32 token indices"); return CAS_ERR_CAPACITY; }
   const int64_t row = (int64_t)desc->Hkv * desc->D;
   Carve c = carve(pool_tokens, row, desc->dtype == CAS_BF16 ? 2 : 4);
@@ -151,7 +183,17 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
   p->desc.n_layers = p->n_layers;
   p->row_elems = (int64_t)desc->Hkv * desc->D;
   p->elem_bytes = desc->dtype == CAS_BF16 ? 2 : 4;
-  layout_slots(desc, p->slot_base, p->slot_cap, p->pool_tokens);
+  p->paged = desc->pool_tokens_budget > 0;
+  p->pack = p->tile == 16;
+  if (!layout_slots(desc, p->slot_base, p->slot_cap, p->pool_tokens, &p->page_owner)) {
+    delete p;
+    set_error("the first n_slots cartridges do not fit pool_tokens_budget");
+    return CAS_ERR_CAPACITY;
+  }
+  if (p->paged) {
+    p->n_pages = (int32_t)p->page_owner.size();
+    p->page_claim.assign(p->n_pages, -1);
+  }
   if (p->pool_tokens >= (1ll << 31)) { delete p; set_error("pool too large"); return CAS_ERR_CAPACITY; }
   p->home_off.assign(desc->n_carts, 0);
   for (int c = 1; c < desc->n_carts; ++c) p->home_off[c] = p->home_off[c - 1] + p->home_bytes(c - 1);
@@ -182,6 +224,7 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_main, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_side_in, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_out_last, cudaEventDisableTiming);
     if (e == cudaSuccess) {   // highest priority: its small refresh kernels must not queue behind the attention CTAs
       int lo = 0, hi = 0;
       cudaDeviceGetStreamPriorityRange(&lo, &hi);
@@ -212,6 +255,7 @@ int cas_pool_destroy(cas_pool* p) {
     if (p->ev_side) cudaEventDestroy(p->ev_side);
     if (p->ev_main) cudaEventDestroy(p->ev_main);
     if (p->ev_side_in) cudaEventDestroy(p->ev_side_in);
+    if (p->ev_out_last) cudaEventDestroy(p->ev_out_last);
     if (p->side_in) cudaStreamDestroy(p->side_in);
     if (p->st_h2d) cudaStreamDestroy(p->st_h2d);
     if (p->st_upload) cudaStreamDestroy(p->st_upload);
@@ -293,7 +337,9 @@ int cas_pool_read_layer(cas_pool* p, int32_t layer, int32_t cart, int32_t what, 
   const PoolLayer& L = p->layers[layer];
   CAS_CUDA(cudaDeviceSynchronize());
   if (what < 6) {
-    if (s >= 0 && p->in_transit[cart] != 2) {
+    // in transit (either way) the pinned home is the valid copy after the device-wide synchronisation above: an
+    // evictee's copy has landed, and in a paged pool its slot handle may already describe the arrival's extent
+    if (s >= 0 && !p->in_transit[cart]) {
       CAS_CUDA(cudaMemcpy(out, p->slot_state(layer, s, what), n * 4, cudaMemcpyDeviceToHost));
     } else {
       if (!p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
@@ -855,15 +901,35 @@ int cas_plan_rotation(const cas_pool* p, int64_t step, int32_t n_in, int32_t n_o
   for (int c : evictable) freeslots.push_back(p->slot_of[c]);
   std::sort(freeslots.begin(), freeslots.end());
   std::vector<char> used(freeslots.size(), 0);
-  std::vector<std::pair<int32_t, int32_t>> arrivals;   // (cart, slot)
-  for (int c : waiting) {
-    if ((int)arrivals.size() >= std::max(n_in, 0)) break;
-    for (size_t i = 0; i < freeslots.size(); ++i)
-      if (!used[i] && p->slot_cap[freeslots[i]] >= p->cart_len[c]) {
-        used[i] = 1;
-        arrivals.push_back({c, freeslots[i]});
-        break;
-      }
+  struct Arrival { int32_t cart, slot, base_tok; };
+  std::vector<Arrival> arrivals;
+  if (p->paged) {
+    // the lowest unused slot handle + the first-fit run of pages that are free now, or freed by this round's evictees,
+    // and that no earlier arrival of this plan has taken; a cartridge that fits nowhere is skipped
+    std::vector<char> leaving(N, 0), taken(p->n_pages, 0);
+    for (int c : evictable) leaving[c] = 1;
+    size_t next_handle = 0;
+    for (int c : waiting) {
+      if ((int)arrivals.size() >= std::max(n_in, 0) || next_handle >= freeslots.size()) break;
+      const int32_t n = p->pages_for(c);
+      const int32_t b = first_fit(p->n_pages, n, [&](int32_t q) {
+        const int32_t o = p->page_owner[q];
+        return (o < 0 || leaving[o]) && p->page_claim[q] < 0 && !taken[q];
+      });
+      if (b < 0) continue;
+      for (int32_t q = b; q < b + n; ++q) taken[q] = 1;
+      arrivals.push_back({c, freeslots[next_handle++], b * p->tile});
+    }
+  } else {
+    for (int c : waiting) {
+      if ((int)arrivals.size() >= std::max(n_in, 0)) break;
+      for (size_t i = 0; i < freeslots.size(); ++i)
+        if (!used[i] && p->slot_cap[freeslots[i]] >= p->cart_len[c]) {
+          used[i] = 1;
+          arrivals.push_back({c, freeslots[i], p->slot_base[freeslots[i]]});
+          break;
+        }
+    }
   }
   std::vector<std::pair<int32_t, int32_t>> outs;       // (slot, cart)
   for (int c : evictable) outs.push_back({p->slot_of[c], c});
@@ -871,8 +937,8 @@ int cas_plan_rotation(const cas_pool* p, int64_t step, int32_t n_in, int32_t n_o
   const int total = (int)(outs.size() + arrivals.size());
   if (total > capacity) { set_error("manifest needs %d entries", total); return CAS_ERR_CAPACITY; }
   int k = 0;
-  for (auto& o : outs) entries[k++] = {o.second, o.first, CAS_DIR_OUT, 0, p->home_off[o.second], p->home_bytes(o.second)};
-  for (auto& a : arrivals) entries[k++] = {a.first, a.second, CAS_DIR_IN, 0, p->home_off[a.first], p->home_bytes(a.first)};
+  for (auto& o : outs) entries[k++] = {o.second, o.first, CAS_DIR_OUT, p->slot_base[o.first], p->home_off[o.second], p->home_bytes(o.second)};
+  for (auto& a : arrivals) entries[k++] = {a.cart, a.slot, CAS_DIR_IN, a.base_tok, p->home_off[a.cart], p->home_bytes(a.cart)};
   *n_entries = k;
   return CAS_OK;
 }
@@ -924,6 +990,7 @@ int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t st
       // must not read its home before this copy has landed
       if (!p->ev_cart[e[i].cart]) CAS_CUDA(cudaEventCreateWithFlags(&p->ev_cart[e[i].cart], cudaEventDisableTiming));
       CAS_CUDA(cudaEventRecord(p->ev_cart[e[i].cart], p->side));
+      if (p->paged) CAS_CUDA(cudaEventRecord(p->ev_out_last, p->side));
     }
     p->in_transit[e[i].cart] = 1;
     p->pending.push_back({e[i], step});
@@ -934,6 +1001,7 @@ int cas_swap_out(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t st
 int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t step) {
   if (!p || (n && !e) || n < 0) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
   std::set<int32_t> leaving, taken;
+  std::vector<int32_t> claim = p->page_claim;   // paged pool: pages claimed by arrivals in flight (+ this call's)
   for (auto& q : p->pending) {
     if (q.e.dir == CAS_DIR_OUT) leaving.insert(q.e.slot);
     else taken.insert(q.e.slot);
@@ -944,10 +1012,30 @@ int cas_swap_in(cas_pool* p, const cas_manifest_entry* e, int32_t n, int64_t ste
     if (c < 0 || c >= p->desc.n_carts || s < 0 || s >= p->desc.n_slots) { set_error("bad manifest entry"); return CAS_ERR_INVALID_ARG; }
     if (p->slot_of[c] >= 0 || p->in_transit[c]) { set_error("cartridge %d already resident / in transit", c); return CAS_ERR_BUSY; }
     if (!(p->cart_in[s] < 0 || leaving.count(s)) || !taken.insert(s).second) { set_error("slot %d occupied", s); return CAS_ERR_BUSY; }
-    if (p->slot_cap[s] < p->cart_len[c]) { set_error("slot %d too small", s); return CAS_ERR_CAPACITY; }
+    if (!p->paged && p->slot_cap[s] < p->cart_len[c]) { set_error("slot %d too small", s); return CAS_ERR_CAPACITY; }
     if (e[i].host_off != p->home_off[c] || e[i].nbytes != p->home_bytes(c)) { set_error("manifest bytes mismatch"); return CAS_ERR_INVALID_ARG; }
+    if (p->paged) {
+      const int32_t np_ = p->pages_for(c), b = e[i].base_tok / p->tile;
+      if (e[i].base_tok % p->tile || b < 0 || b + np_ > p->n_pages) { set_error("bad extent for cartridge %d", c); return CAS_ERR_INVALID_ARG; }
+      for (int32_t q = b; q < b + np_; ++q) {
+        const int32_t o = p->page_owner[q];
+        if (claim[q] >= 0 || (o >= 0 && p->in_transit[o] != 1)) { set_error("page %d is occupied", q); return CAS_ERR_BUSY; }
+      }
+      for (int32_t q = b; q < b + np_; ++q) claim[q] = c;
+    }
   }
+  if (p->paged) p->page_claim = claim;   // every entry is valid: the claims stand
   if (p->dev && !p->pinned) { set_error("no pinned arena"); return CAS_ERR_INVALID_ARG; }
+  if (p->paged) {
+    // the slot handles take their arrivals' extents now: the copies below are addressed through them
+    for (int i = 0; i < n; ++i) {
+      if (e[i].dir != CAS_DIR_IN) continue;
+      p->slot_base[e[i].slot] = e[i].base_tok;
+      p->slot_cap[e[i].slot] = p->pages_for(e[i].cart) * p->tile;
+    }
+    // pages freed by ANY earlier eviction (this round's or an older one whose copy may still be in flight)
+    if (p->dev) CAS_CUDA(cudaStreamWaitEvent(p->side_in, p->ev_out_last, 0));
+  }
   // all copies first, then the refresh kernels: a kernel between two copies would hold the next copy
   // back until the kernel finds a free SM under the attention kernels of the main stream
   for (int i = 0; i < n && p->dev; ++i) {
@@ -993,6 +1081,8 @@ int cas_swap_commit(cas_pool* p, void* main_stream) {
       p->slot_of[q.e.cart] = -1;
       p->in_transit[q.e.cart] = 0;
       if (p->cart_in[q.e.slot] == q.e.cart) p->cart_in[q.e.slot] = -1;
+      if (p->paged)
+        for (int32_t& o : p->page_owner) if (o == q.e.cart) o = -1;
     }
   for (auto& q : p->pending)
     if (q.e.dir == CAS_DIR_IN) {
@@ -1000,6 +1090,9 @@ int cas_swap_commit(cas_pool* p, void* main_stream) {
       p->cart_in[q.e.slot] = q.e.cart;
       p->in_transit[q.e.cart] = 0;
       p->last_used[q.e.cart] = q.step;
+      if (p->paged)
+        for (int32_t pg = 0; pg < p->n_pages; ++pg)
+          if (p->page_claim[pg] == q.e.cart) { p->page_owner[pg] = q.e.cart; p->page_claim[pg] = -1; }
     }
   p->pending.clear();
   return CAS_OK;

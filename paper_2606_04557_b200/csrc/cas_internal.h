@@ -111,6 +111,14 @@ struct cas_pool {
   cudaStream_t side = nullptr;
   int n_layers = 1;
   std::vector<PoolLayer> layers;
+  // paged pool (desc.pool_tokens_budget > 0): pages of `tile` tokens, contiguous first-fit extents
+  bool paged = false;
+  int32_t n_pages = 0;
+  std::vector<int32_t> page_owner;   // committed owner (cartridge id) of every page, -1 = free
+  std::vector<int32_t> page_claim;   // arrival in flight that will own the page at commit, -1 = none
+  cudaEvent_t ev_out_last = nullptr; // end of the most recent eviction copy (paged arrivals wait for it)
+  bool pack = false;                 // tile == 16: remainders of the selected cartridges are packed into shared KV tiles
+  int32_t pages_for(int c) const { return (cart_len[c] + tile - 1) / tile; }
   cudaEvent_t ev_side = nullptr, ev_main = nullptr;
   // arrivals (H2D) run on a second, library-owned stream so that they overlap the evictions (D2H) on
   // the caller's side stream (full-duplex host link); ev_slot[s] orders an arrival after the eviction

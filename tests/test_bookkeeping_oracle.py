@@ -6,6 +6,7 @@ import pytest
 from oracle.bookkeeping import DIR_IN, DIR_OUT, BookError, PoolBook, mix64, position_offsets
 
 NB = 6 * 16 * 4 * 4          # bytes of one 16-token cartridge home: 6 tensors x 16 x (Hkv*D=4) x 4 B
+# manifest tuples: (cart, slot, dir, base_tok, host_off, nbytes); base_tok = first pool token of the slot (16 per slot)
 
 
 def make_book():
@@ -36,7 +37,7 @@ def test_hand_worked_rotation_trace():
     assert position_offsets(bk, P) == (48, [32, 16])          # 3 resident cartridges x 16 tokens
     assert bk.last_used == [0, 0, -1, -1, -1, -1]
     man = bk.plan_rotation(0, n_in=1, n_out=1, protect=[0, 1], seed=1)
-    assert [e.as_tuple() for e in man] == [(2, 2, DIR_OUT, 2 * NB, NB), (4, 2, DIR_IN, 4 * NB, NB)]
+    assert [e.as_tuple() for e in man] == [(2, 2, DIR_OUT, 32, 2 * NB, NB), (4, 2, DIR_IN, 32, 4 * NB, NB)]
     bk.swap_out(man, 0)
     bk.swap_in(man, 0)
     assert bk.stable_resident() == [0, 1]
@@ -50,7 +51,7 @@ def test_hand_worked_rotation_trace():
     assert sel_slot == [2, 0, 2]
     assert inv_off == [0, 1, 1, 3] and inv_seq == [1, 0, 1]
     man = bk.plan_rotation(1, n_in=2, n_out=2, protect=[0, 4], seed=1)
-    assert [e.as_tuple() for e in man] == [(1, 1, DIR_OUT, NB, NB), (2, 1, DIR_IN, 2 * NB, NB)]
+    assert [e.as_tuple() for e in man] == [(1, 1, DIR_OUT, 16, NB, NB), (2, 1, DIR_IN, 16, 2 * NB, NB)]
     bk.swap_out(man, 1)
     bk.swap_in(man, 1)
     assert bk.adam_slots() == [0, 2]
@@ -60,8 +61,8 @@ def test_hand_worked_rotation_trace():
     assert bk.last_used == [1, 0, 1, -1, 1, -1]
     # ---- step 2: LRU ties -> smaller cartridge id; arrivals fill freed slots ascending
     man = bk.plan_rotation(2, n_in=1, n_out=2, protect=[], seed=1)
-    assert [e.as_tuple() for e in man] == [(0, 0, DIR_OUT, 0, NB), (2, 1, DIR_OUT, 2 * NB, NB),
-                                           (1, 0, DIR_IN, NB, NB)]
+    assert [e.as_tuple() for e in man] == [(0, 0, DIR_OUT, 0, 0, NB), (2, 1, DIR_OUT, 16, 2 * NB, NB),
+                                           (1, 0, DIR_IN, 0, NB, NB)]
 
 
 def test_position_offsets_hand_worked_ragged():
@@ -224,3 +225,37 @@ def test_select_retrieved_hand_worked_and_order_preserving():
         assert select_retrieved(ranked, mp, 99) == list(dict.fromkeys(mp[c] for c in ranked))
     with pytest.raises(BookError):
         select_retrieved([40], [0] * 40, 3)
+
+
+def test_paged_pool_first_fit_hand_worked():
+    """16-token pages, a cartridge owns ceil(len/16) contiguous pages chosen
+    first-fit.  Budget 10 pages; cartridges of 3, 2, 4, 1, 2, 5 pages; three slot handles.  By hand:
+      creation:  c0 -> pages 0-2, c1 -> 3-4, c2 -> 5-8            (page 9 free)
+      round 0 (evict 2 LRU = c0, c1; arrivals by least steps = c3 (1 page), c4 (2 pages), c5 (5 pages)):
+                 c3 -> page 0 (first fit), c4 -> pages 1-2, c5 needs 5: pages 3,4 (freed) + 9 are not contiguous with
+                 anything long enough -> skipped; handles: c3 -> slot 0, c4 -> slot 1
+      after commit: pages [c3, c4, c4, -, -, c2, c2, c2, c2, -]
+      round 1 (evict c2; arrival c5, 5 pages): first fit over free + freed = pages 3..9 -> base 3."""
+    lens = [48, 32, 64, 16, 32, 80]
+    bk = PoolBook(lens, n_slots=3, Hkv=1, D=4, tile_tokens=16, budget_tokens=160)
+    assert bk.slot_base == [0, 48, 80] and bk.slot_cap == [48, 32, 64]
+    assert bk.page_owner == [0, 0, 0, 1, 1, 2, 2, 2, 2, -1]
+    bk.opt_steps = [0, 0, 0, 1, 2, 3]                       # arrival priority: c3, then c4, then c5
+    bk.slot_table([0, 2], [0, 1], [2], step=0)              # c2 is used at step 0 -> c0, c1 are the LRU pair
+    man = bk.plan_rotation(0, n_in=3, n_out=2, protect=[2], seed=1)
+    assert [(e.cart, e.slot, e.dir, e.base_tok) for e in man] == [(0, 0, DIR_OUT, 0), (1, 1, DIR_OUT, 48),
+                                                                   (3, 0, DIR_IN, 0), (4, 1, DIR_IN, 16)]
+    bk.swap_out(man, 0)
+    bk.swap_in(man, 0)
+    assert bk.slot_base[:2] == [0, 16] and bk.slot_cap[:2] == [16, 32]
+    bk.adam_slots()
+    bk.commit()
+    assert bk.page_owner == [3, 4, 4, -1, -1, 2, 2, 2, 2, -1]
+    bk.opt_steps[0] = bk.opt_steps[1] = 9                   # the 5-page cartridge c5 is now the least trained one waiting
+    man = bk.plan_rotation(1, n_in=1, n_out=1, protect=[3, 4], seed=1)
+    assert [(e.cart, e.slot, e.dir, e.base_tok) for e in man] == [(2, 2, DIR_OUT, 80), (5, 2, DIR_IN, 48)]
+    # an extent that overlaps a page of a resident, stable cartridge is refused
+    from oracle.bookkeeping import ManifestEntry
+    bad = ManifestEntry(5, 2, DIR_IN, bk.home_off[5], bk.home_bytes(5), 0)
+    with pytest.raises(BookError, match="BUSY"):
+        bk.swap_in([bad], 1)

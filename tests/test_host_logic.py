@@ -76,11 +76,12 @@ def test_layout_matches_oracle():
         counters_equal(pool, bk)
 
 
-def run_protocol(N, S, steps, n_in, n_out, seed, rng, lens=None, B=3, nsel=4):
+def run_protocol(N, S, steps, n_in, n_out, seed, rng, lens=None, B=3, nsel=4, tile=0, budget=0):
     """K4 step protocol driven identically through the library and the oracle."""
     lens = lens or [256] * N
-    pool = host_pool(lens, S)
-    bk = PoolBook(lens, S, 2, 32)
+    pool = cas.Pool(cas.CAS_BF16, 2, 32, lens, S, tile_tokens=tile, device=None, budget_tokens=budget)
+    bk = PoolBook(lens, S, 2, 32, tile_tokens=tile or 128, budget_tokens=budget)
+    assert pool.slot_base.tolist() == bk.slot_base and pool.slot_cap.tolist() == bk.slot_cap
     acfg = cas.AdamCfg(1e-3, 0.9, 0.999, 1e-8, 0, 1)
     for step in range(steps):
         stable = bk.stable_resident()
@@ -109,6 +110,7 @@ def run_protocol(N, S, steps, n_in, n_out, seed, rng, lens=None, B=3, nsel=4):
         bk.swap_out(wman, step)
         bk.swap_in(wman, step)
         counters_equal(pool, bk)
+        assert pool.slot_base.tolist() == bk.slot_base and pool.slot_cap.tolist() == bk.slot_cap
         cas.cas_adam_step(pool, acfg, host_only=True)
         bk.adam_slots()
         cas.cas_swap_commit(pool, host_only=True)
@@ -136,6 +138,20 @@ def test_protocol_bit_exact_ragged_lengths_and_uneven_in_out():
     run_protocol(N=30, S=9, steps=40, n_in=1, n_out=5, seed=8, rng=rng, lens=lens)
 
 
+def test_protocol_bit_exact_paged_pool():
+    """16-token pages, first-fit extents, Table 8's 50-100x size range (16-64 tokens) and a
+    wider one (fragmentation: some arrivals are skipped); manifests (with their extents), slot handles and counters
+    bit-exact against the oracle over many rotations."""
+    rng = np.random.default_rng(4)
+    lens = (16 * rng.integers(1, 5, size=60)).tolist()                      # 16..64 tokens
+    run_protocol(N=60, S=20, steps=60, n_in=5, n_out=5, seed=9, rng=rng, lens=lens, tile=16, budget=16 * 64)
+    lens = rng.integers(1, 400, size=40).tolist()                           # ragged, not multiples of the page
+    run_protocol(N=40, S=12, steps=60, n_in=4, n_out=3, seed=10, rng=rng, lens=lens, tile=16, budget=16 * 240)
+    with pytest.raises(cas.CasError) as e:                                  # the initial cartridges must fit
+        cas.Pool(cas.CAS_BF16, 2, 32, [64] * 8, 4, tile_tokens=16, device=None, budget_tokens=16 * 15)
+    assert e.value.name == "CAS_ERR_CAPACITY"
+
+
 def test_hand_worked_trace_through_the_library():
     NB = 6 * 16 * 4 * 4
     pool = cas.Pool(cas.CAS_F32, 1, 32, [16] * 6, 3, tile_tokens=16, device=None)
@@ -147,7 +163,7 @@ def test_hand_worked_trace_through_the_library():
     assert e["sel_slot"].tolist() == [1, 0, 1] and e["inv_off"].tolist() == [0, 1, 3, 3]
     assert e["inv_seq"].tolist() == [0, 0, 1] and e["P"].tolist() == [32, 16]
     man, n = cas.cas_plan_rotation(pool, 0, 1, 1, [0, 1], 1)
-    assert manifest_tuples(man, n) == [(2, 2, 0, 2 * NB, NB), (4, 2, 1, 4 * NB, NB)]
+    assert manifest_tuples(man, n) == [(2, 2, 0, 32, 2 * NB, NB), (4, 2, 1, 32, 4 * NB, NB)]
 
 
 @pytest.mark.parametrize("args,code", [
