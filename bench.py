@@ -241,7 +241,6 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
     stream = torch.cuda.current_stream()
     fwd_fl, bwd_fl = attn_flops(wl)
     # resident K+V elements the Adam call updates (with rotation: slots in transit this step are skipped, K4)
-    n_upd = cfg.n_slots - ((cfg.rotate_in + cfg.rotate_out) if (cfg.rotate_in > 0 and not no_swap) else 0)
     # algorithmic bytes: 30 B per element of a slot that holds gradients this step (read g,p,m,v,
     # write p,m,v + bf16 copy), 26 B per element of a clean slot (g = 0 is not read).  Counted per step in prepare().
     adam_acc = {"bytes": 0, "steps": 0}
@@ -255,6 +254,7 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
         tau = rot["step"]
         rot["step"] += 1
         sel_off, sel_cart = wl.sel_off, wl.sel_cart
+        stable = None
         if cfg.rotate_in > 0:
             # K4 step protocol: draw among resident+stable cartridges, protect them, plan, swap on
             # the side stream while fwd/bwd/Adam run on the main stream, commit.
@@ -262,15 +262,6 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
             stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
             sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
         rot["sel"] = (sel_off, sel_cart)
-        if cfg.backward:
-            used = set(int(x) for x in sel_cart)
-            el = lambda c: 2 * int(wl.cart_len[c]) * cfg.Hkv * cfg.D
-            if cfg.rotate_in > 0:       # uniform lengths: n_upd slots are updated, the selected ones hold gradients
-                per = el(0)
-                adam_acc["bytes"] += 30 * per * len(used) + 26 * per * (n_upd - len(used))
-            else:
-                adam_acc["bytes"] += sum((30 if c in used else 26) * el(c) for c in range(cfg.n_slots))
-            adam_acc["steps"] += 1
         if cfg.backward or tau == 0:
             # training: a new batch and a new slot table every step.  Decode (c5): the selection is fixed while
             # a request generates, so the table (and its split-KV work list) is built once and reused per token.
@@ -282,6 +273,17 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
             cas.cas_swap_out(sess.pool, man, n, tau, after_stream=stream)
             cas.cas_swap_in(sess.pool, man, n, tau)
             rot["bytes"] += sum(int(man[i].nbytes) for i in range(n))
+            leaving = set(int(man[i].cart) for i in range(n) if man[i].dir == cas.CAS_DIR_OUT)
+        else:
+            leaving = set()
+        if cfg.backward:
+            # Adam updates every resident cartridge that is not in transit this step (K4); algorithmic bytes: 30 B per
+            # element of a slot that holds gradients, 26 B per element of a clean one
+            used = set(int(x) for x in sel_cart)
+            el = lambda c: 2 * int(wl.cart_len[c]) * cfg.Hkv * cfg.D
+            upd = [c for c in (stable if cfg.rotate_in > 0 else range(cfg.n_slots)) if c not in leaving]
+            adam_acc["bytes"] += sum((30 if c in used else 26) * el(c) for c in upd)
+            adam_acc["steps"] += 1
 
     def finish():
         if rotate:
@@ -561,7 +563,8 @@ def main():
         # BASELINE.json's metric spans five configs: one compact record each for the others (fewer steps; the
         # headline stays c2).  c3 twice: with rotation overlapped, and the same steps without it.
         extra = {}
-        for name, kw in (("c3", {}), ("c3_no_swap", {"no_swap": True}), ("c4", {}), ("c5_all", {}), ("c5_top8", {})):
+        for name, kw in (("c3", {}), ("c3_no_swap", {"no_swap": True}), ("c4", {}), ("c5_all", {}), ("c5_top8", {}),
+                         ("c_pages", {})):
             cname = "c3" if name.startswith("c3") else name
             st = {"c3": 8, "c4": 4}.get(cname, 30)
             rec = run_config(args, cname, st, 3, rank, world, local_rank, do_e2e=False, do_cpu=False, **kw)

@@ -443,12 +443,32 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     }
   // KV tile lists + work lists
   const int tile = 128;
+  const bool pack = p->pack;   // 16-token pages: the remainders of a sequence's cartridges share packed KV tiles
   t->kv_tile_off.assign(B + 1, 0);
   t->qtile_off.assign(B + 1, 0);
+  t->ptile_off.assign(B + 1, 0);
   for (int b = 0; b < B; ++b) {
-    for (int k = sel_off[b]; k < sel_off[b + 1]; ++k)
-      for (int j = 0; j < t->sel_len[k]; j += tile)
-        t->kv_tiles.push_back({t->sel_base[k] + j, std::min(tile, t->sel_len[k] - j)});
+    std::vector<std::pair<int32_t, int32_t>> pages;   // (first token, valid keys) of the remainder pages
+    for (int k = sel_off[b]; k < sel_off[b + 1]; ++k) {
+      const int len = t->sel_len[k], whole = pack ? len / tile * tile : len;
+      for (int j = 0; j < whole; j += tile)
+        t->kv_tiles.push_back({t->sel_base[k] + j, std::min(tile, len - j)});
+      for (int j = whole; j < len; j += 16) pages.push_back({t->sel_base[k] + j, std::min(16, len - j)});
+    }
+    for (size_t i = 0; i < pages.size(); i += 8) {
+      PackedTile pt{};
+      int nvalid = 0;
+      for (int u = 0; u < 8; ++u) {
+        const bool have = i + u < pages.size();
+        pt.tok[u] = have ? pages[i + u].first : pages[i].first;
+        const int cnt = have ? pages[i + u].second : 0;
+        for (int x = 0; x < cnt; ++x) pt.mask[(16 * u + x) >> 5] |= 1u << ((16 * u + x) & 31);
+        nvalid += cnt;
+      }
+      t->kv_tiles.push_back({-1 - (int32_t)t->ptiles.size(), nvalid});
+      t->ptiles.push_back(pt);
+    }
+    t->ptile_off[b + 1] = (int32_t)t->ptiles.size();
     t->kv_tile_off[b + 1] = (int32_t)t->kv_tiles.size();
     const int64_t lq = seq_off[b + 1] - seq_off[b];
     t->qtile_off[b + 1] = t->qtile_off[b] + (int32_t)((lq + 127) / 128);
@@ -470,15 +490,26 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
       const int b = t->inv_seq[e];
       cost += (seq_off[b + 1] - seq_off[b] + 127) / 128;
     }
-    const int len = p->cart_len[p->cart_in[s]];
-    for (int j = 0; j < len; j += tile)
+    const int len = p->cart_len[p->cart_in[s]], whole = pack ? len / tile * tile : len;
+    for (int j = 0; j < whole; j += tile)
       t->bwd_items.push_back({0, s, p->slot_base[s] + j, std::min(tile, len - j), j / tile, cost});
+    for (int j = 0; j < len; j += tile)      // the CUDA-core kernels never pack: every tile of the slot, ragged end included
+      t->simt_bwd_items.push_back({0, s, p->slot_base[s] + j, std::min(tile, len - j), j / tile, cost});
   }
+  // packed tiles belong to ONE sequence: their CTA walks that sequence only and ADDS its rows to the gradient slots
+  for (int b = 0; b < B; ++b)
+    for (int i = t->ptile_off[b]; i < t->ptile_off[b + 1]; ++i) {
+      int nvalid = 0;
+      for (uint32_t w : t->ptiles[i].mask) nvalid += __builtin_popcount(w);
+      t->bwd_items.push_back({2, b, i, nvalid, 0, (seq_off[b + 1] - seq_off[b] + 127) / 128});
+    }
   for (int b = 0; b < B; ++b) {
     const int lq = seq_off[b + 1] - seq_off[b];
     const int nt = (lq + tile - 1) / tile;
-    for (int j = 0; j < nt; ++j)
+    for (int j = 0; j < nt; ++j) {
       t->bwd_items.push_back({1, b, seq_off[b] + j * tile, std::min(tile, lq - j * tile), j, nt - j});
+      t->simt_bwd_items.push_back(t->bwd_items.back());
+    }
   }
   std::stable_sort(t->bwd_items.begin(), t->bwd_items.end(),
                    [](const BwdItem& a, const BwdItem& b) { return a.cost > b.cost; });
@@ -490,7 +521,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
                  o_iseq = blob_add(off, t->inv_seq, 1), o_kto = blob_add(off, t->kv_tile_off),
                  o_kt = blob_add(off, t->kv_tiles, 1), o_fw = blob_add(off, t->fwd_items),
                  o_si = blob_add(off, t->simt_items), o_bw = blob_add(off, t->bwd_items),
-                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off);
+                 o_us = blob_add(off, t->used_slots, 1), o_qt = blob_add(off, t->qtile_off),
+                 o_pt = blob_add(off, t->ptiles, 1), o_sb = blob_add(off, t->simt_bwd_items);
     const size_t o_cnt = off;
     off += 256;
     // a recycled blob whose last reader has finished, else a new one (device memory + pinned mirror)
@@ -544,6 +576,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     put(o_bw, t->bwd_items.data(), t->bwd_items.size() * sizeof(BwdItem));
     put(o_us, t->used_slots.data(), t->used_slots.size() * 4);
     put(o_qt, t->qtile_off.data(), t->qtile_off.size() * 4);
+    put(o_pt, t->ptiles.data(), t->ptiles.size() * sizeof(PackedTile));
+    put(o_sb, t->simt_bwd_items.data(), t->simt_bwd_items.size() * sizeof(BwdItem));
     cudaError_t e = cudaMemcpyAsync(blob.d, blob.h, off, cudaMemcpyHostToDevice, p->st_upload);
     if (e == cudaSuccess) e = cudaEventRecord(blob.ready, p->st_upload);
     if (e != cudaSuccess) { p->tab_free.push_back(blob); delete t; return cuda_fail(e, "slot table upload"); }
@@ -564,6 +598,8 @@ int cas_slot_table_build(cas_pool* p, int32_t B, const int32_t* seq_off, const i
     t->d_bwd_items = (BwdItem*)(d + o_bw);
     t->d_used_slots = (int32_t*)(d + o_us);
     t->d_qtile_off = (int32_t*)(d + o_qt);
+    t->d_ptiles = (PackedTile*)(d + o_pt);
+    t->d_simt_bwd_items = (BwdItem*)(d + o_sb);
     t->d_counters = (int32_t*)(d + o_cnt);
   }
   *out = t;
@@ -770,8 +806,9 @@ int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
   a.layer = layer; a.L = &p->layers[layer];
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
-  if (!tc) {
-    // the CUDA-core path accumulates read-modify-write: give the clean slots it is about to touch real zeros
+  if (!tc || p->pack) {
+    // the CUDA-core path accumulates read-modify-write, and so do the per-sequence packed tiles of a paged pool
+    // (several CTAs add to one cartridge's rows): give the clean slots about to be touched real zeros
     for (int sl : t->used_slots)
       if (!dirty[sl]) {
         const int64_t o = (int64_t)p->slot_base[sl] * p->row_elems, nb = (int64_t)p->slot_cap[sl] * p->row_elems * 4;

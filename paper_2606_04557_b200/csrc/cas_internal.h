@@ -33,9 +33,19 @@ struct KvTile {
   int32_t len;   // valid keys in the tile, 1..128
 };
 
+// A KV tile PACKED from 16-token pages of several cartridges (pools with tile_tokens == 16; SURVEY.md 8(f) NEXT-2,
+// cartridges are whole 16-token pages, down to ONE page at 50-100x compression): KvTile.tok < 0
+// names packed tile -1 - tok.  Page i lands in rows [16 i, 16 i + 16) of the 128-row MMA tile; bit k of `mask` = key k
+// is a real token (a cartridge's last page may be partly filled; unused page slots repeat page 0 with no bits set,
+// so the tile always holds finite data).
+struct PackedTile {
+  int32_t tok[8];     // first pool token of each page
+  uint32_t mask[4];   // 128 key-valid bits
+};
+
 // Backward work item: one KV tile of one KV head is owned by one CTA (deterministic dK/dV).
 struct BwdItem {
-  int32_t kind;     // 0 = prefix tile of a slot, 1 = self tile of a sequence
+  int32_t kind;     // 0 = prefix tile of a slot, 1 = self tile of a sequence, 2 = packed prefix tile of a sequence (tok = its index)
   int32_t id;       // slot (kind 0) or sequence (kind 1)
   int32_t tok;      // first key token of the tile (pool token / packed token)
   int32_t len;      // valid keys
@@ -85,6 +95,7 @@ struct PoolLayer {
   float* grad_V = nullptr;
   float* state = nullptr;
   CUtensorMap tm_K, tm_V;        // [pool_tokens, Hkv, 128] bf16, 128-token boxes (bf16, D == 128 only)
+  CUtensorMap tm_K16, tm_V16;    // the same tensors with 16-token boxes: one page of a packed tile
 };
 
 // Layout of cas_train_step_host's device scratch (byte offsets of the staged inputs, outputs and workspace).
@@ -161,9 +172,12 @@ struct cas_slot_table {
   std::vector<int32_t> kv_tile_off;           // [B+1] into kv_tiles (prefix tiles of sequence b)
   std::vector<int32_t> qtile_off;             // [B+1] 128-row query tiles before sequence b
   std::vector<cas::KvTile> kv_tiles;
+  std::vector<cas::PackedTile> ptiles;        // packed prefix tiles (pools with 16-token pages)
+  std::vector<int32_t> ptile_off;             // [B+1] packed tiles of sequence b
   std::vector<cas::FwdItem> fwd_items;        // 256-row blocks, longest first
   std::vector<cas::FwdItem> simt_items;       // 32-row blocks
   std::vector<cas::BwdItem> bwd_items;        // longest first
+  std::vector<cas::BwdItem> simt_bwd_items;   // the CUDA-core path's tiles (never packed)
   int64_t pairs = 0, prefix_tokens = 0, unique_prefix_tokens = 0;
   int32_t max_lq = 0;
   // one device blob holding all the arrays above (recycled through the pool)
@@ -175,8 +189,10 @@ struct cas_slot_table {
           *d_inv_off = nullptr, *d_inv_seq = nullptr, *d_kv_tile_off = nullptr,
           *d_used_slots = nullptr, *d_sel_slot = nullptr, *d_qtile_off = nullptr;
   cas::KvTile* d_kv_tiles = nullptr;
+  cas::PackedTile* d_ptiles = nullptr;
   cas::FwdItem *d_fwd_items = nullptr, *d_simt_items = nullptr;
   cas::BwdItem* d_bwd_items = nullptr;
+  cas::BwdItem* d_simt_bwd_items = nullptr;
   int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
   // decode-shaped batches: segments of the persistent split-KV kernel, built lazily for a given Hq by cas_tc_decode.cu
   int32_t dec_Hq = 0;
@@ -191,6 +207,7 @@ struct cas_slot_table {
   int32_t *d_dec_cta_off = nullptr, *d_dec_seqs = nullptr, *d_comb_off = nullptr, *d_comb_row = nullptr,
           *d_dec_cnt = nullptr, *d_dec_ticket = nullptr;
   cas::KvTile* d_dec_tiles = nullptr;
+  cas::PackedTile* d_dec_ptiles = nullptr;
   float* d_dec_part = nullptr;
 };
 

@@ -284,7 +284,7 @@ template <typename T, int D>
 static int run_fwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
   SimtTab tab{t->d_seq_off, t->d_sel_off, t->d_sel_base, t->d_sel_len, t->d_inv_off, t->d_inv_seq,
-              t->d_simt_items, t->d_bwd_items};
+              t->d_simt_items, t->d_simt_bwd_items};
   dim3 grid((unsigned)t->simt_items.size(), (unsigned)a.Hq);
   simt_rowwise_kernel<T, D, 0><<<grid, 128, 0, a.stream>>>(
       tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
@@ -297,7 +297,7 @@ template <typename T, int D>
 static int run_bwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
   SimtTab tab{t->d_seq_off, t->d_sel_off, t->d_sel_base, t->d_sel_len, t->d_inv_off, t->d_inv_seq,
-              t->d_simt_items, t->d_bwd_items};
+              t->d_simt_items, t->d_simt_bwd_items};
   float* delta = (float*)a.workspace;
   const int64_t rows = (int64_t)t->T * a.Hq;
   delta_kernel<T><<<(unsigned)((rows * 32 + 255) / 256), 256, 0, a.stream>>>((const T*)a.O, (const T*)a.dO, delta, rows, D);
@@ -305,7 +305,7 @@ static int run_bwd(const AttnArgs& a) {
   simt_rowwise_kernel<T, D, 1><<<grid, 128, 0, a.stream>>>(
       tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
       (const T*)a.dO, a.LSE_in, delta, (T*)a.dQ, nullptr, a.Hq, a.Hkv, a.scale);
-  dim3 grid2((unsigned)(4 * t->bwd_items.size()), (unsigned)a.Hkv);
+  dim3 grid2((unsigned)(4 * t->simt_bwd_items.size()), (unsigned)a.Hkv);
   simt_dkdv_kernel<T, D><<<grid2, 128, 0, a.stream>>>(
       tab, (const T*)a.Q, (const T*)a.L->pool_K, (const T*)a.L->pool_V, (const T*)a.Ks, (const T*)a.Vs,
       (const T*)a.dO, a.LSE_in, delta, a.L->grad_K, a.L->grad_V, (T*)a.dKs, (T*)a.dVs, a.Hq, a.Hkv, a.scale);

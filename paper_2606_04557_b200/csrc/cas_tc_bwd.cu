@@ -106,6 +106,7 @@ enum { C_KV = 0, C_QF = 1, C_DOF = 3, C_QE = 5, C_DOE = 7, C_SF = 9, C_DPF = 10,
 struct BwdParams {
   const int32_t *seq_off, *inv_off, *inv_seq, *qtile_off;
   const BwdItem* items;
+  const PackedTile* ptiles;     // packed prefix tiles (kind 2 items)
   const float *auxL, *auxD;
   float* dQacc;
   float *gradK, *gradV;
@@ -164,6 +165,7 @@ __global__ void __launch_bounds__(kBwdThreads, 1)
 tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmdO,
               const __grid_constant__ CUtensorMap tmKp, const __grid_constant__ CUtensorMap tmVp,
               const __grid_constant__ CUtensorMap tmKs, const __grid_constant__ CUtensorMap tmVs,
+              const __grid_constant__ CUtensorMap tmKp16, const __grid_constant__ CUtensorMap tmVp16,
               const BwdParams prm, const __grid_constant__ SlotMask dirty) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
@@ -176,6 +178,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   const int g = blockIdx.x / n_items;
   const BwdItem it = prm.items[blockIdx.x % n_items];
   if (it.kind == 1 && !prm.has_self) return;     // prefix-only call: no self tiles (block-uniform)
+  const PackedTile* pt = it.kind == 2 ? prm.ptiles + it.tok : nullptr;   // a sequence's packed 16-token pages
 
   if (threadIdx.x == 0) {
     if (sbase & 1023u) __trap();
@@ -200,10 +203,19 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const CUtensorMap* mk = it.kind == 0 ? &tmKp : &tmKs;
       const CUtensorMap* mv = it.kind == 0 ? &tmVp : &tmVs;
       mbar_expect_tx(bar(C_KV), 2 * kT);
-      tma_load_3d(sbase + oK, mk, bar(C_KV), 0, g, it.tok);
-      tma_load_3d(sbase + oK + kH, mk, bar(C_KV), 64, g, it.tok);
-      tma_load_3d(sbase + oV, mv, bar(C_KV), 0, g, it.tok);
-      tma_load_3d(sbase + oV + kH, mv, bar(C_KV), 64, g, it.tok);
+      if (pt) {
+        for (int u = 0; u < 8; ++u) {
+          tma_load_3d(sbase + oK + u * 2048, &tmKp16, bar(C_KV), 0, g, pt->tok[u]);
+          tma_load_3d(sbase + oK + kH + u * 2048, &tmKp16, bar(C_KV), 64, g, pt->tok[u]);
+          tma_load_3d(sbase + oV + u * 2048, &tmVp16, bar(C_KV), 0, g, pt->tok[u]);
+          tma_load_3d(sbase + oV + kH + u * 2048, &tmVp16, bar(C_KV), 64, g, pt->tok[u]);
+        }
+      } else {
+        tma_load_3d(sbase + oK, mk, bar(C_KV), 0, g, it.tok);
+        tma_load_3d(sbase + oK + kH, mk, bar(C_KV), 64, g, it.tok);
+        tma_load_3d(sbase + oV, mv, bar(C_KV), 0, g, it.tok);
+        tma_load_3d(sbase + oV + kH, mv, bar(C_KV), 64, g, it.tok);
+      }
       Walk w(prm, it, g);
       const int n = w.total();
       for (int i = 0; i < n; ++i) {
@@ -290,7 +302,8 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     const int k = threadIdx.x & 127;                 // key lane
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tSw = tS + lane_base + wg * 64, tdPw = tdP + lane_base + wg * 64;
-    const bool key_ok = k < it.len;
+    const bool key_ok = pt ? ((pt->mask[k >> 5] >> (k & 31)) & 1u) != 0 : k < it.len;
+    const bool tile_full = it.len == 128;            // (a packed tile with 128 valid keys has every mask bit set)
     const uint32_t ds_row = sbase + oDS + wg * kH + k * 128;
     Walk w(prm, it, g);
     const int n = w.total();
@@ -299,7 +312,7 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const uint32_t ph = (i >> 1) & 1;
       const int rows = w.rows();
       const bool diag = it.kind == 1 && w.qt == it.jt;
-      const bool masked = diag || rows < 128 || it.len < 128;          // block-uniform
+      const bool masked = diag || rows < 128 || !tile_full;            // block-uniform
       // valid query columns of this key: qlo <= q < qhi
       const int qlo = diag ? k : 0;
       const int qhi = key_ok ? rows : 0;
@@ -438,9 +451,10 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
     tc_fence_after();
     const uint32_t src = (isK ? tdK : tdV) + lane_base;
     const float mul = isK ? prm.scale : 1.f;
-    const int64_t row = ((int64_t)(it.tok + k) * prm.Hkv + g) * 128;
-    const bool ok = k < it.len;
-    if (it.kind == 0) {
+    const int key_tok = pt ? pt->tok[k >> 4] + (k & 15) : it.tok + k;       // packed: the key's own cartridge row
+    const int64_t row = ((int64_t)key_tok * prm.Hkv + g) * 128;
+    const bool ok = pt ? ((pt->mask[k >> 5] >> (k & 31)) & 1u) != 0 : k < it.len;
+    if (it.kind != 1) {
       const uint32_t srow = sbase + (isK ? 67584u : 0u) + k * 528;     // 528 B row pitch: conflict-free v4 stores
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
@@ -456,7 +470,9 @@ tc_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       fence_proxy_async();
       if (ok) {
         // a slot that already holds gradients is added to; a clean slot's buffer is undefined and is overwritten
-        if ((dirty.w[it.id >> 5] >> (it.id & 31)) & 1u)
+        // a packed tile always ADDS: other sequences' CTAs write the same cartridge rows (the host has zeroed the
+        // clean slots it touches)
+        if (pt || ((dirty.w[it.id >> 5] >> (it.id & 31)) & 1u))
           asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
                        ::"l"((isK ? prm.gradK : prm.gradV) + row), "r"(srow), "r"(512u) : "memory");
         else
@@ -533,7 +549,7 @@ int tc_attn_bwd(const AttnArgs& a) {
     tmKs = a.L->tm_K;
     tmVs = a.L->tm_V;
   }
-  BwdParams prm{t->d_seq_off, t->d_inv_off, t->d_inv_seq, t->d_qtile_off, t->d_bwd_items, auxL, auxD, dQacc,
+  BwdParams prm{t->d_seq_off, t->d_inv_off, t->d_inv_seq, t->d_qtile_off, t->d_bwd_items, t->d_ptiles, auxL, auxD, dQacc,
                 a.L->grad_K, a.L->grad_V, (__nv_bfloat16*)a.dKs, (__nv_bfloat16*)a.dVs, (int64_t)nqt * 128,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale, a.scale * kLog2e};
   const unsigned grid = (unsigned)(t->bwd_items.size() * a.Hkv);
@@ -541,7 +557,10 @@ int tc_attn_bwd(const AttnArgs& a) {
   const int32_t* gd = a.pool->grad_dirty.data() + (size_t)a.layer * a.pool->desc.n_slots;   // this layer's flags
   for (int sl = 0; sl < a.pool->desc.n_slots; ++sl)
     if (gd[sl]) dirty.w[sl >> 5] |= 1u << (sl & 31);
-  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.L->tm_K, a.L->tm_V, tmKs, tmVs, prm, dirty);
+  if (a.pool->pack)   // paged pool: the clean slots of this table were zeroed by the caller, every tile adds
+    for (int sl : t->used_slots) dirty.w[sl >> 5] |= 1u << (sl & 31);
+  tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.L->tm_K, a.L->tm_V, tmKs, tmVs, a.L->tm_K16,
+                                                           a.L->tm_V16, prm, dirty);
   dq_convert_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
       dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows);
   cudaError_t e = cudaGetLastError();

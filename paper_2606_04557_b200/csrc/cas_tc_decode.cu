@@ -58,6 +58,7 @@ struct DecParams {
   const int32_t* cta_seg_off;   // [grid + 1]
   const int32_t* seqs;          // row-block sequence lists
   const KvTile* tiles;
+  const PackedTile* ptiles;     // packed prefix tiles (16-token pages), named by KvTile.tok < 0
   const int32_t* seq_off;       // packed token index of every sequence (one token each)
   const int32_t* comb_off;      // [B + 1] partial rows (in units of sequences) of the prefix segments covering sequence b
   const int32_t* comb_row;
@@ -284,6 +285,7 @@ decode_combine_kernel(const __grid_constant__ DecParams prm, const __grid_consta
 __global__ void __launch_bounds__(kDecThreads, 1)
 tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV,
                  const __grid_constant__ CUtensorMap tmKc, const __grid_constant__ CUtensorMap tmVc,
+                 const __grid_constant__ CUtensorMap tmK16, const __grid_constant__ CUtensorMap tmV16,
                  const __grid_constant__ DecParams prm, const __grid_constant__ SelfLens slen) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
@@ -339,14 +341,29 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             const uint32_t ph = (t / kDecStages) & 1;
             const uint32_t kb = sbase + dOffKV + s * 2 * dT, vb = kb + dT;
             const int tok = d.kind == 0 ? prm.tiles[d.tile_off + j].tok : d.seq_off * prm.cache_cap + 128 * j;
+            const PackedTile* pt = (d.kind == 0 && tok < 0) ? prm.ptiles + (-1 - tok) : nullptr;
             mbar_wait(bar(D_KE + s), ph ^ 1);
             mbar_expect_tx(bar(D_KF + s), dT);
-            tma_load_3d(kb, mk, bar(D_KF + s), 0, d.g, tok);
-            tma_load_3d(kb + dH, mk, bar(D_KF + s), 64, d.g, tok);
+            if (pt) {
+              for (int u = 0; u < 8; ++u) {
+                tma_load_3d(kb + u * 2048, &tmK16, bar(D_KF + s), 0, d.g, pt->tok[u]);
+                tma_load_3d(kb + dH + u * 2048, &tmK16, bar(D_KF + s), 64, d.g, pt->tok[u]);
+              }
+            } else {
+              tma_load_3d(kb, mk, bar(D_KF + s), 0, d.g, tok);
+              tma_load_3d(kb + dH, mk, bar(D_KF + s), 64, d.g, tok);
+            }
             mbar_wait(bar(D_VE + s), ph ^ 1);
             mbar_expect_tx(bar(D_VF + s), dT);
-            tma_load_3d(vb, mv, bar(D_VF + s), 0, d.g, tok);
-            tma_load_3d(vb + dH, mv, bar(D_VF + s), 64, d.g, tok);
+            if (pt) {
+              for (int u = 0; u < 8; ++u) {
+                tma_load_3d(vb + u * 2048, &tmV16, bar(D_VF + s), 0, d.g, pt->tok[u]);
+                tma_load_3d(vb + dH + u * 2048, &tmV16, bar(D_VF + s), 64, d.g, pt->tok[u]);
+              }
+            } else {
+              tma_load_3d(vb, mv, bar(D_VF + s), 0, d.g, tok);
+              tma_load_3d(vb + dH, mv, bar(D_VF + s), 64, d.g, tok);
+            }
           }
         };
         // source of segments: this CTA's static list, then self-cache units (one per (sequence with a long cache, KV
@@ -501,8 +518,20 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
       const int n = d.n_tiles;
       float m = -INFINITY, l = 0.f;
       for (int j = w; j < n; j += 2) {
-        const int limit = d.kind == 0 ? prm.tiles[d.tile_off + j].len : min(128, d.self_len - 128 * j);
-        const bool ragged = limit < 128;
+        // key-valid bits of the tile, one word per 32-column chunk: a prefix of `limit` keys, or a packed tile's pages
+        uint32_t mw[4];
+        {
+          const KvTile tl = d.kind == 0 ? prm.tiles[d.tile_off + j] : KvTile{0, min(128, d.self_len - 128 * j)};
+          if (d.kind == 0 && tl.tok < 0) {
+            const uint4 mk = *reinterpret_cast<const uint4*>(prm.ptiles[-1 - tl.tok].mask);
+            mw[0] = mk.x; mw[1] = mk.y; mw[2] = mk.z; mw[3] = mk.w;
+          } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+              mw[c] = tl.len >= 32 * (c + 1) ? 0xffffffffu : (tl.len > 32 * c ? (1u << (tl.len - 32 * c)) - 1u : 0u);
+          }
+        }
+        const bool ragged = (mw[0] & mw[1] & mw[2] & mw[3]) != 0xffffffffu;
         mbar_wait(bar(D_SF + w), cme & 1);
         tc_fence_after();
         // Two passes over the 128 scores (row max, then exp) in 32-column chunks with the NEXT chunk's TMEM load in
@@ -518,7 +547,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
           if (ragged) {
 #pragma unroll
             for (int cc = 0; cc < 32; ++cc)
-              if (32 * c + cc >= limit) s[cc] = 0xff800000u;
+              if (!((mw[c] >> cc) & 1u)) s[cc] = 0xff800000u;
           }
 #pragma unroll
           for (int cc = 0; cc < 32; cc += 8) {
@@ -565,11 +594,10 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
             else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
             if (ragged) {
               // a masked key weighs EXACTLY 0 (its raw score may be anything; its V row may be a stale cache row)
-              const int c0 = 32 * c + 2 * i;
-              a0 = c0 < limit ? a0 : 0.f;
-              a1 = c0 + 1 < limit ? a1 : 0.f;
-              b0 = c0 + 2 < limit ? b0 : 0.f;
-              b1 = c0 + 3 < limit ? b1 : 0.f;
+              a0 = (mw[c] >> (2 * i)) & 1u ? a0 : 0.f;
+              a1 = (mw[c] >> (2 * i + 1)) & 1u ? a1 : 0.f;
+              b0 = (mw[c] >> (2 * i + 2)) & 1u ? b0 : 0.f;
+              b1 = (mw[c] >> (2 * i + 3)) & 1u ? b1 : 0.f;
             }
             sum2a = add2(sum2a, pack2(a0, a1));
             sum2b = add2(sum2b, pack2(b0, b1));
@@ -630,11 +658,27 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
     groups[std::vector<int32_t>(t->inv_seq.begin() + t->inv_off[s], t->inv_seq.begin() + t->inv_off[s + 1])].push_back(s);
   int64_t units = 0;
   std::vector<std::vector<KvTile>> gtiles;
+  std::vector<PackedTile> ptiles;
   for (auto& kv : groups) {
     std::vector<KvTile> tl;
+    std::vector<std::pair<int32_t, int32_t>> pages;   // 16-token pages left over (pools with tile_tokens == 16)
     for (int s : kv.second) {
-      const int len = p->cart_len[p->cart_in[s]];
-      for (int j = 0; j < len; j += 128) tl.push_back({p->slot_base[s] + j, std::min(128, len - j)});
+      const int len = p->cart_len[p->cart_in[s]], whole = p->pack ? len / 128 * 128 : len;
+      for (int j = 0; j < whole; j += 128) tl.push_back({p->slot_base[s] + j, std::min(128, len - j)});
+      for (int j = whole; j < len; j += 16) pages.push_back({p->slot_base[s] + j, std::min(16, len - j)});
+    }
+    for (size_t i = 0; i < pages.size(); i += 8) {      // the group's remainders share packed tiles
+      PackedTile pt{};
+      int nvalid = 0;
+      for (int u = 0; u < 8; ++u) {
+        const bool have = i + u < pages.size();
+        pt.tok[u] = have ? pages[i + u].first : pages[i].first;
+        const int cnt = have ? pages[i + u].second : 0;
+        for (int x = 0; x < cnt; ++x) pt.mask[(16 * u + x) >> 5] |= 1u << ((16 * u + x) & 31);
+        nvalid += cnt;
+      }
+      tl.push_back({-1 - (int32_t)ptiles.size(), nvalid});
+      ptiles.push_back(pt);
     }
     units += (int64_t)((kv.first.size() + R - 1) / R) * (int64_t)tl.size() * Hkv;
     gtiles.push_back(std::move(tl));
@@ -702,7 +746,8 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   const size_t o_sg = 0, o_cs = up(segs.size() * sizeof(DecSeg) + 32), o_sq = o_cs + up(cta_seg_off.size() * 4),
                o_tl = o_sq + up(seqs.size() * 4 + 4), o_co = o_tl + up(tiles.size() * sizeof(KvTile) + 8),
                o_cr = o_co + up(comb_off.size() * 4), o_cn = o_cr + up(comb_row.size() * 4 + 4),
-               o_tk = o_cn + up((size_t)t->B * Hq * 4), o_pt = o_tk + 256;
+               o_tk = o_cn + up((size_t)t->B * Hq * 4), o_pk = o_tk + 256,
+               o_pt = o_pk + up(ptiles.size() * sizeof(PackedTile) + 16);
   const int64_t part_rows = (int64_t)row_off + t->B;               // prefix partial rows + one self row per sequence
   const size_t part_bytes = (size_t)Hkv * part_rows * G * kPartStride * 4;
   cudaError_t e = cudaMalloc((void**)&t->d_dec_blob, o_pt + part_bytes + 256);
@@ -723,6 +768,7 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   if (!tiles.empty()) memcpy(h + o_tl, tiles.data(), tiles.size() * sizeof(KvTile));
   memcpy(h + o_co, comb_off.data(), comb_off.size() * 4);
   if (!comb_row.empty()) memcpy(h + o_cr, comb_row.data(), comb_row.size() * 4);
+  if (!ptiles.empty()) memcpy(h + o_pk, ptiles.data(), ptiles.size() * sizeof(PackedTile));
   cudaStream_t up_st = t->pool->st_upload;
   e = cudaMemcpyAsync(t->d_dec_blob, h, o_pt, cudaMemcpyHostToDevice, up_st);
   if (e == cudaSuccess) e = cudaEventRecord(t->dec_ready, up_st);
@@ -736,6 +782,7 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   t->d_comb_row = (int32_t*)(d + o_cr);
   t->d_dec_cnt = (int32_t*)(d + o_cn);
   t->d_dec_ticket = (int32_t*)(d + o_tk);
+  t->d_dec_ptiles = (PackedTile*)(d + o_pk);
   t->d_dec_part = (float*)(d + o_pt);
   t->dec_comb_off = comb_off;
   t->dec_grid = grid;
@@ -778,11 +825,12 @@ int tc_decode_fwd(const AttnArgs& a, const void* Kc, const void* Vc, int cache_c
     if (rc) return rc;
   }
   const float scale_log2 = a.scale * 1.4426950408889634f;
-  DecParams prm{t->d_dec_segs, t->d_dec_cta_off, t->d_dec_seqs, t->d_dec_tiles, t->d_seq_off, t->d_comb_off,
+  DecParams prm{t->d_dec_segs, t->d_dec_cta_off, t->d_dec_seqs, t->d_dec_tiles, t->d_dec_ptiles, t->d_seq_off, t->d_comb_off,
                 t->d_comb_row, (const __nv_bfloat16*)a.Q, (const __nv_bfloat16*)Kc, (const __nv_bfloat16*)Vc,
                 (__nv_bfloat16*)a.O_out, a.LSE_out, t->d_dec_part, t->d_dec_cnt, t->d_dec_ticket, t->dec_rows,
                 t->dec_self_row_base, cache_cap, t->B, a.Hq, a.Hkv, t->dec_fused, scale_log2};
-  tc_decode_kernel<<<(unsigned)t->dec_grid, kDecThreads, kDecSmem, a.stream>>>(a.L->tm_K, a.L->tm_V, tmKc, tmVc, prm, sl);
+  tc_decode_kernel<<<(unsigned)t->dec_grid, kDecThreads, kDecSmem, a.stream>>>(a.L->tm_K, a.L->tm_V, tmKc, tmVc, a.L->tm_K16,
+                                                                               a.L->tm_V16, prm, sl);
   if (!t->dec_fused) {
     const int n_w = t->B * a.Hq;
     decode_combine_kernel<<<(n_w * 32 + 255) / 256, 256, 0, a.stream>>>(prm, sl);

@@ -54,6 +54,10 @@ int tc_make_pool_maps(cas_pool* p) {
     if (rc) return rc;
     rc = make_thd_map(&L.tm_V, L.pool_V, p->pool_tokens, p->desc.Hkv, 128);
     if (rc) return rc;
+    rc = make_thd_map(&L.tm_K16, L.pool_K, p->pool_tokens, p->desc.Hkv, 16);
+    if (rc) return rc;
+    rc = make_thd_map(&L.tm_V16, L.pool_V, p->pool_tokens, p->desc.Hkv, 16);
+    if (rc) return rc;
   }
   p->has_tma = true;
   return CAS_OK;
@@ -74,6 +78,7 @@ struct FwdParams {
   const int32_t* seq_off;
   const int32_t* kv_tile_off;
   const KvTile* kv_tiles;
+  const PackedTile* ptiles;      // packed prefix tiles (16-token pages), named by KvTile.tok < 0
   const FwdItem* items;
   __nv_bfloat16* O;
   float* LSE;
@@ -90,7 +95,8 @@ __device__ __forceinline__ float ex2(float x) {
 __global__ void __launch_bounds__(kFwdThreads, 1)
 tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmKp,
               const __grid_constant__ CUtensorMap tmVp, const __grid_constant__ CUtensorMap tmKs,
-              const __grid_constant__ CUtensorMap tmVs, const FwdParams prm) {
+              const __grid_constant__ CUtensorMap tmVs, const __grid_constant__ CUtensorMap tmKp16,
+              const __grid_constant__ CUtensorMap tmVp16, const FwdParams prm) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* sptr = smem_raw + (sbase - smem_u32(smem_raw));
@@ -147,14 +153,29 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const int tok = pre ? tiles[j].tok : t0 + 128 * (j - n_pre);
         const CUtensorMap* mk = pre ? &tmKp : &tmKs;
         const CUtensorMap* mv = pre ? &tmVp : &tmVs;
+        const PackedTile* pt = (pre && tok < 0) ? prm.ptiles + (-1 - tok) : nullptr;
         mbar_wait(bar(B_KE + s), ph ^ 1);
         mbar_expect_tx(bar(B_KF + s), kTile);
-        tma_load_3d(sbase + kOffK + s * kTile, mk, bar(B_KF + s), 0, g, tok);
-        tma_load_3d(sbase + kOffK + s * kTile + kHalf, mk, bar(B_KF + s), 64, g, tok);
+        if (pt) {   // eight 16-token pages, each in place from its own cartridge
+          for (int u = 0; u < 8; ++u) {
+            tma_load_3d(sbase + kOffK + s * kTile + u * 2048, &tmKp16, bar(B_KF + s), 0, g, pt->tok[u]);
+            tma_load_3d(sbase + kOffK + s * kTile + kHalf + u * 2048, &tmKp16, bar(B_KF + s), 64, g, pt->tok[u]);
+          }
+        } else {
+          tma_load_3d(sbase + kOffK + s * kTile, mk, bar(B_KF + s), 0, g, tok);
+          tma_load_3d(sbase + kOffK + s * kTile + kHalf, mk, bar(B_KF + s), 64, g, tok);
+        }
         mbar_wait(bar(B_VE + s), ph ^ 1);
         mbar_expect_tx(bar(B_VF + s), kTile);
-        tma_load_3d(sbase + kOffV + s * kTile, mv, bar(B_VF + s), 0, g, tok);
-        tma_load_3d(sbase + kOffV + s * kTile + kHalf, mv, bar(B_VF + s), 64, g, tok);
+        if (pt) {
+          for (int u = 0; u < 8; ++u) {
+            tma_load_3d(sbase + kOffV + s * kTile + u * 2048, &tmVp16, bar(B_VF + s), 0, g, pt->tok[u]);
+            tma_load_3d(sbase + kOffV + s * kTile + kHalf + u * 2048, &tmVp16, bar(B_VF + s), 64, g, pt->tok[u]);
+          }
+        } else {
+          tma_load_3d(sbase + kOffV + s * kTile, mv, bar(B_VF + s), 0, g, tok);
+          tma_load_3d(sbase + kOffV + s * kTile + kHalf, mv, bar(B_VF + s), 64, g, tok);
+        }
       }
     }
   } else if (warp == 9) {
@@ -234,8 +255,10 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       float m = -INFINITY, l = 0.f;
       for (int j = 0; j < nkv; ++j) {
         int limit;
+        const PackedTile* pt = nullptr;
         if (j < n_pre) {
           limit = tiles[j].len;
+          if (tiles[j].tok < 0) { pt = prm.ptiles + (-1 - tiles[j].tok); limit = 128; }
         } else {
           const int k0 = 128 * (j - n_pre);
           limit = min(min(128, lq - k0), row - k0 + 1);
@@ -252,6 +275,15 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #pragma unroll
           for (int c = 0; c < 128; ++c)
             if (c >= limit) s[c] = 0xff800000u;      // -inf: masked key
+        }
+        if (pt) {                                    // packed tile: the valid keys are those of its pages (warp-uniform)
+          const uint4 mk = *reinterpret_cast<const uint4*>(pt->mask);
+          const uint32_t mw[4] = {mk.x, mk.y, mk.z, mk.w};
+          if ((mk.x & mk.y & mk.z & mk.w) != 0xffffffffu) {
+#pragma unroll
+            for (int c = 0; c < 128; ++c)
+              if (!((mw[c >> 5] >> (c & 31)) & 1u)) s[c] = 0xff800000u;
+          }
         }
         float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;   // four independent chains
 #pragma unroll
@@ -355,10 +387,10 @@ int tc_attn_fwd(const AttnArgs& a) {
     tmKs = a.L->tm_K;
     tmVs = a.L->tm_V;
   }
-  FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
+  FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, t->d_ptiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
                 a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale * 1.4426950408889634f};
   const unsigned grid = (unsigned)(n_items * a.Hq);
-  tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.L->tm_K, a.L->tm_V, tmKs, tmVs, prm);
+  tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.L->tm_K, a.L->tm_V, tmKs, tmVs, a.L->tm_K16, a.L->tm_V16, prm);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc fwd launch");
 }

@@ -21,7 +21,8 @@ class Session:
         self.wl, self.cfg, self.device = wl, cfg, device
         self.tdt = torch_dtype(cfg.dtype)
         self.pool = cas.Pool(cas.CAS_F32 if cfg.dtype == "f32" else cas.CAS_BF16, cfg.Hkv, cfg.D,
-                             wl.cart_len, cfg.n_slots, device=device)
+                             wl.cart_len, cfg.n_slots, tile_tokens=getattr(cfg, "tile_tokens", 0), device=device,
+                             budget_tokens=getattr(cfg, "budget_tokens", 0))
         if load:
             for c in range(cfg.n_carts):
                 K, V = wl.cart_kv(c)

@@ -33,7 +33,8 @@ def counters_equal(pool, bk):
 def run_rotation(cfg, steps, seed, check_attn_every=1):
     wl = make_workload(cfg, seed)
     sess = Session(wl)
-    bk = PoolBook(wl.cart_len.tolist(), cfg.n_slots, cfg.Hkv, cfg.D)
+    bk = PoolBook(wl.cart_len.tolist(), cfg.n_slots, cfg.Hkv, cfg.D, tile_tokens=cfg.tile_tokens or 128,
+                  budget_tokens=cfg.budget_tokens)
     bk.slot_table(wl.seq_off.tolist(), wl.sel_off.tolist(), wl.sel_cart.tolist(), 0)   # Session's own table
     rng = np.random.Generator(np.random.PCG64(seed + 1))
     main = torch.cuda.current_stream()
@@ -59,6 +60,7 @@ def run_rotation(cfg, steps, seed, check_attn_every=1):
         cas.cas_swap_in(sess.pool, man, n, step)
         bk.swap_out(wman, step)
         bk.swap_in(wman, step)
+        assert sess.pool.slot_base.tolist() == bk.slot_base and sess.pool.slot_cap.tolist() == bk.slot_cap
         # compute overlaps with the copies in flight on the side stream
         sess.fwd()
         sess.bwd()

@@ -35,6 +35,11 @@ class CasConfig:
     lq_min: int = 256
     lq_max: int = 4096
     n_dist_max: int = 31
+    # paged pools: page size of the pool (0 = the 128-token default),
+    # token budget of a paged pool with rotation (0 = static slots), cartridge lengths = 16 x U{1..len_pages_max}
+    tile_tokens: int = 0
+    budget_tokens: int = 0
+    len_pages_max: int = 0
     # Adam (BASELINE.json config 1; Table 5 gives no eps/betas, Kingma & Ba defaults)
     lr: float = 1e-3
     beta1: float = 0.9
@@ -67,6 +72,13 @@ CONFIGS = {
     "c5_top8": CasConfig("c5_decode_top8_bf16", "bf16", Hq=32, Hkv=8, D=128, n_carts=500,
                          n_slots=500, cart_len=512, B=64, Lq=1, n_dist=7, kv_std=0.02,
                          selection="topk", backward=False),
+    # NEXT-2, paper-true cartridge sizes at 50-100x compression (Table 8: FinQA / TechQA rows with
+    # min 16, max 64-ish tokens; sizes are whole 16-token pages): 400 cartridges of 16..64 tokens, 200
+    # resident in a paged pool, packed batch of 32 samples x 256 tokens (8,192 tokens, Table 5), each
+    # sample sees its target + U{0..10} distractors, 20 in / 20 out per step.
+    "c_pages": CasConfig("c_pages_16tok_bf16", "bf16", Hq=32, Hkv=8, D=128, n_carts=400, n_slots=200, cart_len=0,
+                         B=32, Lq=256, n_dist=-1, n_dist_max=10, kv_std=0.02, selection="uniform", rotate_in=20,
+                         rotate_out=20, tile_tokens=16, budget_tokens=16 * 560, len_pages_max=4),
 }
 
 

@@ -76,6 +76,8 @@ def _normal(rng: np.random.Generator, shape, std: float, dtype: str) -> np.ndarr
 def draw_cart_lengths(cfg: CasConfig, rng: np.random.Generator) -> np.ndarray:
     if cfg.cart_len > 0:
         return np.full(cfg.n_carts, cfg.cart_len, dtype=np.int32)
+    if cfg.len_pages_max > 0:        # whole 16-token pages, 1..len_pages_max of them
+        return (16 * rng.integers(1, cfg.len_pages_max + 1, size=cfg.n_carts)).astype(np.int32)
     # config 4: round(lognormal(mu, sigma)) clamped to [len_min, len_max]
     raw = np.exp(rng.normal(cfg.len_mu, cfg.len_sigma, size=cfg.n_carts))
     return np.clip(np.rint(raw), cfg.len_min, cfg.len_max).astype(np.int32)
