@@ -134,6 +134,33 @@ int launch_refresh(float* pK, float* pV, void* wK, void* wV, float* gK, float* g
   return CAS_OK;
 }
 
+// Zero the gradient rows of many (small) slots in ONE launch: the descriptors travel as kernel parameters, like Adam's
+// (a cudaMemsetAsync per slot costs more than the attention itself when the cartridges are 16-64 tokens long).
+__global__ void __launch_bounds__(256)
+zero_slots_kernel(const __grid_constant__ ZeroBatch batch) {
+  const ZeroDesc& d = batch.d[blockIdx.y];
+  const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+  for (int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < d.n; i += (int64_t)gridDim.x * blockDim.x * 4) {
+    st4(d.a + i, z);
+    st4(d.b + i, z);
+  }
+}
+
+int launch_zero_slots(const ZeroDesc* h, int n, cudaStream_t st) {
+  for (int i0 = 0; i0 < n; i0 += kZeroBatch) {
+    const int cnt = std::min(kZeroBatch, n - i0);
+    ZeroBatch batch;
+    int64_t mx = 0;
+    for (int i = 0; i < cnt; ++i) { batch.d[i] = h[i0 + i]; mx = std::max(mx, h[i0 + i].n); }
+    if (mx <= 0) continue;
+    const int64_t gx = std::min<int64_t>((mx / 4 + 255) / 256, 148 * 4);
+    zero_slots_kernel<<<dim3((unsigned)gx, (unsigned)cnt), 256, 0, st>>>(batch);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "zero_slots_kernel launch");
+  }
+  return CAS_OK;
+}
+
 int launch_zero(float* p, int64_t n, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(p, 0, (size_t)n * 4, st);
   if (e != cudaSuccess) return cuda_fail(e, "zero");

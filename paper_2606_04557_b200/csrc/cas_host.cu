@@ -809,12 +809,16 @@ int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
   if (!tc || p->pack) {
     // the CUDA-core path accumulates read-modify-write, and so do the per-sequence packed tiles of a paged pool
     // (several CTAs add to one cartridge's rows): give the clean slots about to be touched real zeros
+    std::vector<ZeroDesc> zs;
     for (int sl : t->used_slots)
       if (!dirty[sl]) {
-        const int64_t o = (int64_t)p->slot_base[sl] * p->row_elems, nb = (int64_t)p->slot_cap[sl] * p->row_elems * 4;
-        CAS_CUDA(cudaMemsetAsync(a.L->grad_K + o, 0, nb, (cudaStream_t)stream));
-        CAS_CUDA(cudaMemsetAsync(a.L->grad_V + o, 0, nb, (cudaStream_t)stream));
+        const int64_t o = (int64_t)p->slot_base[sl] * p->row_elems;
+        zs.push_back({a.L->grad_K + o, a.L->grad_V + o, (int64_t)p->slot_cap[sl] * p->row_elems});
       }
+    if (!zs.empty()) {
+      rc = launch_zero_slots(zs.data(), (int)zs.size(), (cudaStream_t)stream);
+      if (rc) return rc;
+    }
   }
   rc = tc ? tc_attn_bwd(a) : simt_attn_bwd(a);
   if (rc) return rc;

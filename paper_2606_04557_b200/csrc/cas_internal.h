@@ -271,5 +271,14 @@ int launch_adam(const AdamSlotDesc* h_desc, int n, const cas_adam_cfg& cfg, int 
 int launch_refresh(float* pK, float* pV, void* wK, void* wV, float* gK, float* gV, int64_t n,
                    int dtype, cudaStream_t st);
 int launch_zero(float* p, int64_t n, cudaStream_t st);
+struct ZeroDesc {
+  float *a, *b;     // gradient rows of one slot (K and V), 16-byte aligned
+  int64_t n;        // elements (multiple of 4)
+};
+constexpr int kZeroBatch = 512;
+struct ZeroBatch {
+  ZeroDesc d[kZeroBatch];
+};
+int launch_zero_slots(const ZeroDesc* h, int n, cudaStream_t st);
 
 }  // namespace cas
