@@ -33,13 +33,13 @@ namespace cas {
 using namespace sm100;
 
 constexpr int kDecThreads = 384;
-constexpr int kDecStages = 3;
+constexpr int kRing = 5;           // K/V ring: five 32 KB slots filled in the order K(0) V(0) K(1) V(1) ...
 constexpr int kDescRing = 4;
 constexpr int kInlineSelf = 4;     // caches up to this length are dotted on the CUDA cores inside the merge
 constexpr int kMaxDecB = 1024;     // sequences per decode call with a self cache (their lengths travel as kernel parameters)
 constexpr uint32_t dT = 32768, dH = 16384;
-constexpr uint32_t dOffQ = 0, dOffKV = dT, dOffBar = dT + kDecStages * 2 * dT;
-enum { D_KF = 0, D_KE = 3, D_VF = 6, D_VE = 9, D_SF = 12, D_PF = 14, D_OV = 16, D_QF = 18, D_QE = 19, D_DF = 20, D_DE = 24, D_PW = 28, D_N = 32 };
+constexpr uint32_t dOffQ = 0, dOffKV = 2 * dT, dOffBar = 2 * dT + kRing * dT;   // Q tile A | Q tile B | ring
+enum { D_RF = 0, D_RE = 5, D_SF = 10, D_PF = 12, D_OV = 14, D_QF = 16, D_QE = 17, D_DF = 18, D_DE = 22, D_PW = 26, D_N = 30 };
 constexpr uint32_t dOffDesc = dOffBar + D_N * 8 + 32;                       // after the barriers and the TMEM slot
 constexpr uint32_t dOffML = dOffDesc + kDescRing * 32;                      // (m, l) of both warpgroups: 2 x 128 x 8 B
 constexpr uint32_t kDecSmem = dOffML + 2048;
@@ -131,6 +131,33 @@ __device__ __forceinline__ void dec_segment_epilogue(const DecParams& prm, const
   asm volatile("bar.sync 2, 256;" ::: "memory");
   // no fence here: the partial is published by the thread that counts it (warp 11 fences after its barrier wait;
   // a wide table is merged by the next launch)
+}
+
+// End of a PAIRED segment: warpgroup w owns row block w (its own S_w / O_w); thread r writes the whole partial row.
+__device__ __forceinline__ void dec_paired_epilogue(const DecParams& prm, const DecSeg d, const int w, const int r,
+                                                    const uint32_t tbase, const uint32_t lane_base, const float m,
+                                                    const float l, const int c_own, const uint32_t bar_ov) {
+  const int G = prm.Hq / prm.Hkv;
+  mbar_wait(bar_ov, (c_own - 1) & 1);                              // this warpgroup's last PV
+  tc_fence_after();
+  const int n_rows = (w ? d.self_len : d.n_seqs) * G;
+  float* prow = prm.part + ((int64_t)d.g * prm.rows_total + (int64_t)(d.part_row + (w ? d.n_seqs : 0)) * G + r) * kPartStride;
+  const uint32_t tO = tbase + 256 + w * 128 + lane_base;
+#pragma unroll
+  for (int cc = 0; cc < 4; ++cc) {
+    uint32_t o[32];
+    tmem_ld32(tO + cc * 32, o);
+    tc_wait_ld();
+    if (r < n_rows) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+        __stcg(reinterpret_cast<float4*>(prow + cc * 32 + 4 * i),
+               make_float4(__uint_as_float(o[4 * i]), __uint_as_float(o[4 * i + 1]), __uint_as_float(o[4 * i + 2]),
+                           __uint_as_float(o[4 * i + 3])));
+    }
+  }
+  if (r < n_rows) __stcg(reinterpret_cast<float2*>(prow + 128), make_float2(m, l));
+  tc_fence_before();
 }
 
 // Merge of ONE output row (sequence seq, query head g*G + hh): all split-KV partials of the row -- the prefix segments
@@ -235,7 +262,7 @@ __device__ __forceinline__ void dec_merge_row(const DecParams& prm, const SelfLe
 
 // Fused merge (small batches only -- a few sequences generating: at most kFusedOut output rows in all and row blocks of
 // at most 32 rows): warp 11, after a segment's partials are written, counts them per row and merges the rows whose
-// LAST partial this was, four rows at a time (eight lanes per row).  It saves the second launch of a latency-bound
+// LAST partial this was, two rows at a time (sixteen lanes per row).  It saves the second launch of a latency-bound
 // step.  Measured on the full-size top-8 config (2048 rows, 3-9 partials each) the same scheme is 2x SLOWER than a
 // separate launch: one warp per CTA walks ~3 dependent L2 round trips per row, and the descriptor ring makes the
 // whole pipeline wait for it -- so bigger batches use decode_combine_kernel (one warp per row, 2048 warps at once).
@@ -257,17 +284,18 @@ __device__ __forceinline__ void dec_count_and_merge(const DecParams& prm, const 
   uint32_t todo = __ballot_sync(0xffffffffu, last);
   if (todo) __threadfence();
   while (todo) {
-    // the (lane / 8)-th pending row goes to this group of eight lanes
+    // the (lane / 16)-th pending row goes to this half warp (sixteen lanes per row: eight columns each keep the
+    // warp within its small register budget)
     uint32_t t = todo;
     int mine = -1;
-    for (int q = 0; q < 4 && t; ++q) {
+    for (int q = 0; q < 2 && t; ++q) {
       const int bit = __ffs(t) - 1;
-      if (q == (lane >> 3)) mine = bit;
+      if (q == (lane >> 4)) mine = bit;
       t &= t - 1;
     }
     todo = t;
     const int rseq = __shfl_sync(0xffffffffu, seq, mine < 0 ? 0 : mine);
-    dec_merge_row<8>(prm, slen, d.g, rseq, (mine < 0 ? 0 : mine) % G, lane & 7, mine >= 0);
+    dec_merge_row<16>(prm, slen, d.g, rseq, (mine < 0 ? 0 : mine) % G, lane & 15, mine >= 0);
   }
 }
 
@@ -334,35 +362,35 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
           ++nseg;
         };
         auto load_tiles = [&](const DecSeg& d) {
-          const CUtensorMap* mk = d.kind == 0 ? &tmK : &tmKc;
-          const CUtensorMap* mv = d.kind == 0 ? &tmV : &tmVc;
+          const CUtensorMap* mk = d.kind != 1 ? &tmK : &tmKc;
+          const CUtensorMap* mv = d.kind != 1 ? &tmV : &tmVc;
           for (int j = 0; j < d.n_tiles; ++j, ++t) {
-            const int s = t % kDecStages;
-            const uint32_t ph = (t / kDecStages) & 1;
-            const uint32_t kb = sbase + dOffKV + s * 2 * dT, vb = kb + dT;
-            const int tok = d.kind == 0 ? prm.tiles[d.tile_off + j].tok : d.seq_off * prm.cache_cap + 128 * j;
-            const PackedTile* pt = (d.kind == 0 && tok < 0) ? prm.ptiles + (-1 - tok) : nullptr;
-            mbar_wait(bar(D_KE + s), ph ^ 1);
-            mbar_expect_tx(bar(D_KF + s), dT);
+            const int uk = 2 * t, uv = 2 * t + 1;                    // ring units of this tile's K and V
+            const int sk = uk % kRing, sv = uv % kRing;
+            const uint32_t kb = sbase + dOffKV + sk * dT, vb = sbase + dOffKV + sv * dT;
+            const int tok = d.kind != 1 ? prm.tiles[d.tile_off + j].tok : d.seq_off * prm.cache_cap + 128 * j;
+            const PackedTile* pt = (d.kind != 1 && tok < 0) ? prm.ptiles + (-1 - tok) : nullptr;
+            mbar_wait(bar(D_RE + sk), ((uk / kRing) & 1) ^ 1);
+            mbar_expect_tx(bar(D_RF + sk), dT);
             if (pt) {
               for (int u = 0; u < 8; ++u) {
-                tma_load_3d(kb + u * 2048, &tmK16, bar(D_KF + s), 0, d.g, pt->tok[u]);
-                tma_load_3d(kb + dH + u * 2048, &tmK16, bar(D_KF + s), 64, d.g, pt->tok[u]);
+                tma_load_3d(kb + u * 2048, &tmK16, bar(D_RF + sk), 0, d.g, pt->tok[u]);
+                tma_load_3d(kb + dH + u * 2048, &tmK16, bar(D_RF + sk), 64, d.g, pt->tok[u]);
               }
             } else {
-              tma_load_3d(kb, mk, bar(D_KF + s), 0, d.g, tok);
-              tma_load_3d(kb + dH, mk, bar(D_KF + s), 64, d.g, tok);
+              tma_load_3d(kb, mk, bar(D_RF + sk), 0, d.g, tok);
+              tma_load_3d(kb + dH, mk, bar(D_RF + sk), 64, d.g, tok);
             }
-            mbar_wait(bar(D_VE + s), ph ^ 1);
-            mbar_expect_tx(bar(D_VF + s), dT);
+            mbar_wait(bar(D_RE + sv), ((uv / kRing) & 1) ^ 1);
+            mbar_expect_tx(bar(D_RF + sv), dT);
             if (pt) {
               for (int u = 0; u < 8; ++u) {
-                tma_load_3d(vb + u * 2048, &tmV16, bar(D_VF + s), 0, d.g, pt->tok[u]);
-                tma_load_3d(vb + dH + u * 2048, &tmV16, bar(D_VF + s), 64, d.g, pt->tok[u]);
+                tma_load_3d(vb + u * 2048, &tmV16, bar(D_RF + sv), 0, d.g, pt->tok[u]);
+                tma_load_3d(vb + dH + u * 2048, &tmV16, bar(D_RF + sv), 64, d.g, pt->tok[u]);
               }
             } else {
-              tma_load_3d(vb, mv, bar(D_VF + s), 0, d.g, tok);
-              tma_load_3d(vb + dH, mv, bar(D_VF + s), 64, d.g, tok);
+              tma_load_3d(vb, mv, bar(D_RF + sv), 0, d.g, tok);
+              tma_load_3d(vb + dH, mv, bar(D_RF + sv), 64, d.g, tok);
             }
           }
         };
@@ -408,46 +436,76 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         constexpr uint32_t idesc_qk = make_idesc(128, 128, 0, 0);
         constexpr uint32_t idesc_pv = make_idesc(128, 128, 0, 1);
         int t = 0, c0 = 0, c1 = 0;
-        auto issue_qk = [&](int tt, int w) {
-          const int s = tt % kDecStages;
-          mbar_wait(bar(D_KF + s), (tt / kDecStages) & 1);
-          tc_fence_after();
-          const uint32_t qa = sbase + dOffQ, ka = sbase + dOffKV + s * 2 * dT;
+        // S_w = Q_q K(tt)^T; K(tt) sits in ring unit 2 tt.  `release`: the K slot is free once this MMA is done.
+        auto issue_qk = [&](int tt, int w, int q, bool wait_k, bool release) {
+          const int u = 2 * tt, sl = u % kRing;
+          if (wait_k) {
+            mbar_wait(bar(D_RF + sl), (u / kRing) & 1);
+            tc_fence_after();
+          }
+          const uint32_t qa = sbase + dOffQ + q * dT, ka = sbase + dOffKV + sl * dT;
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk) {
             const uint32_t o = (kk >> 2) * dH + (kk & 3) * 32;
             mma_ss(tbase + w * 128, desc_kmajor(qa + o), desc_kmajor(ka + o), idesc_qk, kk > 0);
           }
           mma_commit(bar(D_SF + w));
-          mma_commit(bar(D_KE + s));
+          if (release) mma_commit(bar(D_RE + sl));
+        };
+        // O_w (+)= P_w V(tt); V(tt) sits in ring unit 2 tt + 1
+        auto issue_pv = [&](int tt, int w, bool wait_v, bool release, bool accum) {
+          const int u = 2 * tt + 1, sl = u % kRing;
+          if (wait_v) mbar_wait(bar(D_RF + sl), (u / kRing) & 1);
+          tc_fence_after();
+          const uint32_t va = sbase + dOffKV + sl * dT;
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk)
+            mma_ts(tbase + 256 + w * 128, tbase + w * 128 + kk * 8, desc_mnmajor(va + kk * 2048, dH), idesc_pv,
+                   (accum || kk > 0) ? 1u : 0u);
+          if (release) mma_commit(bar(D_RE + sl));
+          mma_commit(bar(D_OV + w));
         };
         for (int nseg = 0;; ++nseg) {
           const int k = nseg & (kDescRing - 1);
           mbar_wait(bar(D_DF + k), (nseg / kDescRing) & 1);
           const int n = dring[k].n_tiles;
-          if (dring[k].kind < 0) break;
+          const int kind = dring[k].kind;
+          if (kind < 0) break;
           mbar_wait(bar(D_QF), nseg & 1);
           tc_fence_after();
-          issue_qk(t, 0);
-          if (n > 1) issue_qk(t + 1, 1);
-          if (n <= 2) mma_commit(bar(D_QE));
-          for (int j = 0; j < n; ++j) {
-            const int w = j & 1, s = (t + j) % kDecStages;
-            const int cw = w ? c1 : c0;
-            mbar_wait(bar(D_PF + w), cw & 1);
-            if (w) ++c1; else ++c0;
-            mbar_wait(bar(D_VF + s), ((t + j) / kDecStages) & 1);
-            tc_fence_after();
-            const uint32_t va = sbase + dOffKV + s * 2 * dT + dT;
-#pragma unroll
-            for (int kk = 0; kk < 8; ++kk)
-              mma_ts(tbase + 256 + w * 128, tbase + w * 128 + kk * 8, desc_mnmajor(va + kk * 2048, dH), idesc_pv,
-                     (j >= 2 || kk > 0) ? 1u : 0u);
-            mma_commit(bar(D_VE + s));
-            mma_commit(bar(D_OV + w));
-            if (j + 2 < n) {
-              issue_qk(t + j + 2, w);
-              if (j + 2 == n - 1) mma_commit(bar(D_QE));
+          if (kind == 2) {
+            // PAIRED row blocks: Q tile A -> S0/O0 (warpgroup 0), Q tile B -> S1/O1 (warpgroup 1), every K/V tile is
+            // fetched once and used by both:  PV_a(j) QK_a(j+1) PV_b(j) QK_b(j+1)
+            issue_qk(t, 0, 0, true, false);
+            issue_qk(t, 1, 1, false, true);
+            if (n == 1) mma_commit(bar(D_QE));
+            for (int j = 0; j < n; ++j) {
+              mbar_wait(bar(D_PF), c0 & 1);
+              ++c0;
+              issue_pv(t + j, 0, true, false, j > 0);
+              if (j + 1 < n) issue_qk(t + j + 1, 0, 0, true, false);
+              mbar_wait(bar(D_PF + 1), c1 & 1);
+              ++c1;
+              issue_pv(t + j, 1, false, true, j > 0);
+              if (j + 1 < n) {
+                issue_qk(t + j + 1, 1, 1, false, true);
+                if (j + 1 == n - 1) mma_commit(bar(D_QE));
+              }
+            }
+          } else {
+            // ONE row block: the warpgroups take alternate tiles
+            issue_qk(t, 0, 0, true, true);
+            if (n > 1) issue_qk(t + 1, 1, 0, true, true);
+            if (n <= 2) mma_commit(bar(D_QE));
+            for (int j = 0; j < n; ++j) {
+              const int w = j & 1;
+              mbar_wait(bar(D_PF + w), (w ? c1 : c0) & 1);
+              if (w) ++c1; else ++c0;
+              issue_pv(t + j, w, true, true, j >= 2);
+              if (j + 2 < n) {
+                issue_qk(t + j + 2, w, 0, true, true);
+                if (j + 2 == n - 1) mma_commit(bar(D_QE));
+              }
             }
           }
           t += n;
@@ -464,13 +522,15 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
           const DecSeg d = dring[k];
           if (d.kind < 0) break;
           mbar_wait(bar(D_QE), (nseg & 1) ^ 1);                      // the previous segment's last QK has read the tile
-          const int n_rows = d.n_seqs * G;
+          // a paired segment (kind 2) has a second row block: sequences seq_off + n_seqs .., self_len of them -> Q tile B
+          const int n_tiles_q = d.kind == 2 ? 2 : 1;
 #pragma unroll 1
-          for (int rr = 0; rr < 4; ++rr) {
-            const int r = lane + 32 * rr;
+          for (int rr = 0; rr < 4 * n_tiles_q; ++rr) {
+            const int qt = rr >> 2, r = lane + 32 * (rr & 3);
+            const int n_rows = (qt ? d.self_len : d.n_seqs) * G;
             const uint4* src = nullptr;
             if (r < n_rows) {
-              const int seq = d.kind == 0 ? prm.seqs[d.seq_off + r / G] : d.seq_off, h = d.g * G + r % G;
+              const int seq = d.kind != 1 ? prm.seqs[d.seq_off + (qt ? d.n_seqs : 0) + r / G] : d.seq_off, h = d.g * G + r % G;
               src = reinterpret_cast<const uint4*>(prm.Q + ((int64_t)prm.seq_off[seq] * prm.Hq + h) * 128);
             }
 #pragma unroll
@@ -480,7 +540,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
               for (int c = 0; c < 8; ++c) q[c] = src ? src[half * 8 + c] : make_uint4(0, 0, 0, 0);
 #pragma unroll
               for (int c = 0; c < 8; ++c) {
-                const uint32_t addr = sbase + dOffQ + half * dH + r * 128 + ((uint32_t)(c ^ (r & 7)) << 4);
+                const uint32_t addr = sbase + dOffQ + qt * dT + half * dH + r * 128 + ((uint32_t)(c ^ (r & 7)) << 4);
                 asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(q[c].x), "r"(q[c].y), "r"(q[c].z), "r"(q[c].w) : "memory");
               }
             }
@@ -516,13 +576,15 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
       const DecSeg d = dring[k];
       if (d.kind < 0) break;
       const int n = d.n_tiles;
+      const bool paired = d.kind == 2;               // two row blocks: this warpgroup owns ONE of them and takes EVERY tile
+      const int jstep = paired ? 1 : 2;
       float m = -INFINITY, l = 0.f;
-      for (int j = w; j < n; j += 2) {
+      for (int j = paired ? 0 : w; j < n; j += jstep) {
         // key-valid bits of the tile, one word per 32-column chunk: a prefix of `limit` keys, or a packed tile's pages
         uint32_t mw[4];
         {
-          const KvTile tl = d.kind == 0 ? prm.tiles[d.tile_off + j] : KvTile{0, min(128, d.self_len - 128 * j)};
-          if (d.kind == 0 && tl.tok < 0) {
+          const KvTile tl = d.kind != 1 ? prm.tiles[d.tile_off + j] : KvTile{0, min(128, d.self_len - 128 * j)};
+          if (d.kind != 1 && tl.tok < 0) {
             const uint4 mk = *reinterpret_cast<const uint4*>(prm.ptiles[-1 - tl.tok].mask);
             mw[0] = mk.x; mw[1] = mk.y; mw[2] = mk.z; mw[3] = mk.w;
           } else {
@@ -558,7 +620,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
           }
         }
         const float m_new = fmaxf(m, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * prm.scale_log2);
-        if (j < 2) {
+        if (j < jstep) {                             // this warpgroup's first tile of the segment
           m = m_new;
         } else if (__any_sync(0xffffffffu, m_new > m + 8.f)) {
           mbar_wait(bar(D_OV + w), (cme - 1) & 1);                   // this warpgroup's previous PV has updated O
@@ -582,6 +644,9 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           tc_wait_ld();
+          // buf[(c+1)&1] was the SOURCE of the P store of chunk c-1: that store must have read its registers before
+          // the next load overwrites them
+          if (c > 0) tc_wait_st();
           if (c < 3) tmem_ld32(tS + 32 * (c + 1), buf[(c + 1) & 1]);
           uint32_t* s = buf[c & 1];
 #pragma unroll
@@ -616,8 +681,9 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
         mbar_arrive(bar(D_PF + w));
         ++cme;
       }
-      cother += (n - (w ^ 1) + 1) >> 1;                             // the other warpgroup's tiles of this segment
-      dec_segment_epilogue(prm, d, w, r, tbase, lane_base, m, l, w ? cother : cme, w ? cme : cother, bar(D_OV), ml);
+      cother += paired ? n : (n - (w ^ 1) + 1) >> 1;                // the other warpgroup's tiles of this segment
+      if (paired) dec_paired_epilogue(prm, d, w, r, tbase, lane_base, m, l, cme, bar(D_OV + w));
+      else dec_segment_epilogue(prm, d, w, r, tbase, lane_base, m, l, w ? cother : cme, w ? cme : cother, bar(D_OV), ml);
       mbar_arrive(bar(D_PW + k));                                    // warp 11 counts and merges (fused tables)
       if ((threadIdx.x & 127) == 0) mbar_arrive(bar(D_DE + k));
     }
@@ -680,7 +746,9 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
       tl.push_back({-1 - (int32_t)ptiles.size(), nvalid});
       ptiles.push_back(pt);
     }
-    units += (int64_t)((kv.first.size() + R - 1) / R) * (int64_t)tl.size() * Hkv;
+    // cost in tile times: a PAIR of row blocks shares every K/V tile in one CTA (4 MMAs per tile, ~1.5 tile times)
+    const int64_t nrb = (int64_t)(kv.first.size() + R - 1) / R;
+    units += ((nrb / 2) * 3 + (nrb & 1) * 2) * (int64_t)tl.size() * Hkv / 2;
     gtiles.push_back(std::move(tl));
   }
   const int64_t quota = std::max<int64_t>(1, (units + n_sm - 1) / n_sm);   // tiles per CTA
@@ -695,7 +763,8 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
     const int nt = (int)tl.size();
     // whole chunks of about `quota` tiles: the row blocks of one chunk land on CTAs that start together and walk the
     // same tiles at the same time, so a tile that several row blocks need is fetched from HBM once
-    const int nchunk = (int)std::max<int64_t>(1, (nt + quota / 2) / quota);
+    const bool pairs = kv.first.size() > (size_t)R;                 // two or more row blocks: pair them
+    const int nchunk = (int)std::min<int64_t>(nt, std::max<int64_t>(1, (pairs ? (int64_t)nt * 3 / 2 : nt) / quota));   // rounded down: never more segments than CTAs' worth of work, never an empty one
     std::vector<int> seq_offs;
     for (size_t r0 = 0; r0 < kv.first.size(); r0 += R) {
       const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
@@ -709,6 +778,16 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
       for (size_t rb = 0; rb < seq_offs.size(); ++rb) {
         const size_t r0 = rb * R;
         const int ns = (int)std::min<size_t>(R, kv.first.size() - r0);
+        if (rb + 1 < seq_offs.size()) {
+          // row blocks rb and rb + 1 as ONE paired segment: both Q tiles resident, every K/V tile fetched once
+          // (their sequences are consecutive in `seqs`, their partial rows consecutive from row_off)
+          const int ns2 = (int)std::min<size_t>(R, kv.first.size() - r0 - R);
+          for (int g = 0; g < Hkv; ++g) segs.push_back(DecSeg{2, to + a, b - a, g, seq_offs[rb], ns, row_off, ns2});
+          for (int j = 0; j < ns + ns2; ++j) comb[kv.first[r0 + j]].push_back(row_off + j);
+          row_off += ns + ns2;
+          ++rb;
+          continue;
+        }
         for (int g = 0; g < Hkv; ++g) segs.push_back(DecSeg{0, to + a, b - a, g, seq_offs[rb], ns, row_off, 0});
         for (int j = 0; j < ns; ++j) comb[kv.first[r0 + j]].push_back(row_off + j);
         row_off += ns;
@@ -722,11 +801,12 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   std::vector<int32_t> cta_seg_off(grid + 1, 0);
   {
     int64_t total = 0;
-    for (const DecSeg& sg : segs) total += sg.n_tiles + kSegCost;
+    auto cost = [&](const DecSeg& sg) { return (sg.kind == 2 ? (int64_t)sg.n_tiles * 3 / 2 : sg.n_tiles) + kSegCost; };
+    for (const DecSeg& sg : segs) total += cost(sg);
     int64_t load = 0, done = 0;
     int cta = 0;
     for (size_t i = 0; i < segs.size(); ++i) {
-      const int64_t c = segs[i].n_tiles + kSegCost;
+      const int64_t c = cost(segs[i]);
       const int64_t share = (total - done + (grid - cta) - 1) / std::max(1, grid - cta);
       if (load > 0 && load + c / 2 >= share && cta < grid - 1) {
         cta_seg_off[++cta] = (int32_t)i;
@@ -791,7 +871,7 @@ static int decode_prepare(cas_slot_table* t, int Hq) {
   t->dec_n_segs = (int32_t)segs.size();
   t->dec_fused = t->B * Hq <= kFusedOut ? 1 : 0;
   for (const DecSeg& sg : segs)
-    if (sg.n_seqs * G > kFusedRows) t->dec_fused = 0;
+    if (sg.n_seqs * G > kFusedRows || sg.kind == 2) t->dec_fused = 0;
   t->dec_Hq = Hq;
   return CAS_OK;
 }

@@ -71,6 +71,14 @@ def check_attention(wl, impl, kv_heads, self_block=True, backward=True, pre_grad
     Oo, Lo = orc.attn_fwd(wl.Q, bK, bV, sel, wl.seq_off, Ks, Vs, sess.scale, cfg.Hkv, kv_heads=kv_heads)
     res = {"O": err(O[:, hs], Oo[:, hs], cfg.dtype), "LSE": rel_max(LSE[:, hs], Lo[:, hs])}
     assert np.isfinite(O).all() and np.isfinite(LSE).all()
+    if res["O"] > tolO:      # say WHERE: worst (token, head) rows and the error of each 32-column quarter
+        d = O[:, hs] - Oo[:, hs]
+        per_row = np.linalg.norm(d, axis=2) / (np.linalg.norm(Oo[:, hs], axis=2) + 1e-30)
+        worst = np.argsort(-per_row.ravel())[:8]
+        res["worst_rows(token,head,err)"] = [(int(i // len(hs)), hs[int(i % len(hs))], float(per_row.ravel()[i])) for i in worst]
+        t0, h0 = int(worst[0] // len(hs)), int(worst[0] % len(hs))
+        res["quarters_of_worst_row"] = [float(np.linalg.norm(d[t0, h0, 32 * q:32 * q + 32]) /
+                                              (np.linalg.norm(Oo[t0, hs[h0], 32 * q:32 * q + 32]) + 1e-30)) for q in range(4)]
     assert res["O"] <= tolO, res
     assert res["LSE"] <= (TOL_F32 if cfg.dtype == "f32" else 2e-3), res
     if backward and cfg.backward:
