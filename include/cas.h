@@ -368,19 +368,35 @@ int cas_train_step_layers(cas_pool* pool, const cas_slot_table* const* tables, i
  * H2D copies of hQ,hK_self,hV_self,hdO (pinned host, dtype), fwd, bwd, Adam over all stable
  * resident slots, D2H of O, LSE, dQ and (when hdK_self/hdV_self are given: both or neither) dK_self, dV_self --
  * every result of the backward pass that does not stay in the pool.  Kernels run on `stream`; the copies run on
- * two internal copy streams so that dO arrives under the forward pass, O/LSE leave under the backward pass and
- * dQ, dK_self, dV_self leave under Adam; `stream` finally waits for the last copy.  dev_scratch must hold
- * cas_train_step_host_scratch_bytes() (single-layer pools only) and belongs to the library between back-to-back calls that reuse it: when
- * the next call has the SAME scratch layout (same T, Hq, workspace size) its input copies start as soon as the
- * previous backward pass is done; with a different layout (ragged batches) they wait for the previous call's last
- * read-back, because the regions move.  Asynchronous; synchronise `stream` before reading the host results or
- * overwriting the host inputs. */
+ * two internal copy streams: dO arrives under the forward pass, O/LSE leave under the backward pass, dQ, dK_self,
+ * dV_self leave under Adam.  dev_scratch must hold cas_train_step_host_scratch_bytes() (single-layer pools only):
+ * TWO sets of input and result buffers, used alternately by consecutive calls, plus the backward workspace; it
+ * belongs to the library between back-to-back calls that reuse it.  When the next call has the SAME scratch layout
+ * (same scratch, stream, T, Hq, workspace size) its inputs are copied into the other set while this call still
+ * computes (they wait only for the backward pass two calls back, the last reader of that set); with a different
+ * layout (ragged batches) the call first waits for everything in flight, because the regions move.
+ *   cas_train_step_host        `stream` finally waits for this call's last read-back: once `stream` has completed
+ *                              the call, the host results are valid and the host inputs may be overwritten.
+ *   cas_train_step_host_async  does NOT make `stream` wait for the read-back, so the next call's kernels start while
+ *                              this call's dQ is still crossing the host link (steady state: a step costs
+ *                              max(kernels, H2D bytes, D2H bytes) instead of their sum).  The host inputs may be
+ *                              overwritten once `stream` has completed the call; the host RESULTS are valid only
+ *                              after cas_train_step_host_wait.  Result buffers of calls in flight must be distinct
+ *                              or the caller accepts that a later call overwrites them (copies run in call order).
+ *   cas_train_step_host_wait   makes `stream` wait for the read-backs of all earlier calls (no host blocking).
+ * In every variant the host inputs must hold their data when the call is MADE (the input copies are ordered after
+ * earlier copies, not after the caller's stream).  Asynchronous. */
 int cas_train_step_host_scratch_bytes(const cas_pool* pool, const cas_slot_table* table, int32_t Hq,
                                       size_t* bytes);
 int cas_train_step_host(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,
                         const void* hK_self, const void* hV_self, const void* hdO, float scale,
                         const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ, void* hdK_self,
                         void* hdV_self, void* dev_scratch, size_t scratch_bytes, void* stream);
+int cas_train_step_host_async(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* hQ,
+                              const void* hK_self, const void* hV_self, const void* hdO, float scale,
+                              const cas_adam_cfg* cfg, void* hO, float* hLSE, void* hdQ, void* hdK_self,
+                              void* hdV_self, void* dev_scratch, size_t scratch_bytes, void* stream);
+int cas_train_step_host_wait(cas_pool* pool, void* stream);
 
 /* ---- hardware self-test (not on the hot path) --------------------------------------------------
  * D[256,128] fp32 = A[256,64] * B[128,64]^T (bf16, row-major, device) computed by ONE tcgen05.mma.cta_group::2

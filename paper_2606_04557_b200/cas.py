@@ -419,9 +419,23 @@ def cas_train_step_host_scratch_bytes(pool: Pool, tab: SlotTable, Hq: int) -> in
     return n.value
 
 
+def _train_step_host(fn, pool, tab, Hq, hQ, hKs, hVs, hdO, scale, cfg, hO, hLSE, hdQ, hdKs, hdVs, scratch, stream):
+    _check(fn(pool.handle, tab.handle, C.c_int32(Hq), _dptr(hQ), _dptr(hKs), _dptr(hVs), _dptr(hdO), C.c_float(scale),
+              C.byref(cfg), _dptr(hO), _dptr(hLSE), _dptr(hdQ), _dptr(hdKs), _dptr(hdVs), _dptr(scratch),
+              C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)))
+
+
 def cas_train_step_host(pool: Pool, tab: SlotTable, Hq: int, hQ, hKs, hVs, hdO, scale: float, cfg: AdamCfg,
                         hO, hLSE, hdQ, hdKs, hdVs, scratch, stream=None):
-    _check(lib().cas_train_step_host(pool.handle, tab.handle, C.c_int32(Hq), _dptr(hQ), _dptr(hKs),
-                                     _dptr(hVs), _dptr(hdO), C.c_float(scale), C.byref(cfg), _dptr(hO),
-                                     _dptr(hLSE), _dptr(hdQ), _dptr(hdKs), _dptr(hdVs), _dptr(scratch),
-                                     C.c_size_t(scratch.numel() * scratch.element_size()), _stream(stream)))
+    _train_step_host(lib().cas_train_step_host, pool, tab, Hq, hQ, hKs, hVs, hdO, scale, cfg, hO, hLSE, hdQ, hdKs,
+                     hdVs, scratch, stream)
+
+
+def cas_train_step_host_async(pool: Pool, tab: SlotTable, Hq: int, hQ, hKs, hVs, hdO, scale: float, cfg: AdamCfg,
+                              hO, hLSE, hdQ, hdKs, hdVs, scratch, stream=None):
+    _train_step_host(lib().cas_train_step_host_async, pool, tab, Hq, hQ, hKs, hVs, hdO, scale, cfg, hO, hLSE, hdQ,
+                     hdKs, hdVs, scratch, stream)
+
+
+def cas_train_step_host_wait(pool: Pool, stream=None):
+    _check(lib().cas_train_step_host_wait(pool.handle, _stream(stream)))

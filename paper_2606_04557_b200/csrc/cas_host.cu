@@ -233,7 +233,7 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_upload, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking);
-    for (int i = 0; i < 6 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
+    for (int i = 0; i < 11 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
     p->ev_cart.assign(desc->n_carts, nullptr);   // created at a cartridge's first eviction
     p->ev_slot.assign(desc->n_slots, nullptr);
     for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
@@ -1150,9 +1150,10 @@ static StepScratch step_scratch(const cas_pool* p, const cas_slot_table* t, int 
   s.oQ = add(T * Hq * D * eb);   s.oKs = add(T * Hkv * D * eb); s.oVs = add(T * Hkv * D * eb);
   s.odO = add(T * Hq * D * eb);  s.oO = add(T * Hq * D * eb);   s.oLSE = add(T * Hq * 4);
   s.odQ = add(T * Hq * D * eb);  s.odKs = add(T * Hkv * D * eb); s.odVs = add(T * Hkv * D * eb);
+  s.set_bytes = o;
   cas_prefix_attn_bwd_workspace_bytes(p, t, Hq, &s.ws_bytes);
-  s.oWs = add(s.ws_bytes);
-  s.total = o;
+  s.oWs = 2 * s.set_bytes;
+  s.total = s.oWs + s.ws_bytes;
   return s;
 }
 
@@ -1162,10 +1163,23 @@ int cas_train_step_host_scratch_bytes(const cas_pool* p, const cas_slot_table* t
   return CAS_OK;
 }
 
-int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
-                        const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
-                        float* hLSE, void* hdQ, void* hdKs, void* hdVs, void* scratch, size_t scratch_bytes,
-                        void* stream) {
+int cas_train_step_host_wait(cas_pool* p, void* stream) {
+  if (!p) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  // an event that was never recorded counts as complete
+  for (int k = 0; k < 2; ++k) CAS_CUDA(cudaStreamWaitEvent((cudaStream_t)stream, p->ev_step[5 + 5 * k], 0));
+  return CAS_OK;
+}
+
+// One step.  Streams: the caller's (kernels), st_h2d (inputs), st_d2h (results).  Consecutive steps alternate between
+// two device buffer sets, so the inputs of step i+1 cross the host link while step i computes and the results of
+// step i leave while step i+1 computes: in steady state a step costs max(kernels, H2D bytes, D2H bytes), not their
+// sum.  Hazards, all expressed as events: set k's inputs are overwritten only after the backward pass of step i-2
+// (their last reader), set k's results only after the read-back of step i-2; the backward workspace is shared and
+// ordered by the caller's stream.
+static int train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
+                           const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
+                           float* hLSE, void* hdQ, void* hdKs, void* hdVs, void* scratch, size_t scratch_bytes,
+                           void* stream, bool wait_readback) {
   int rc = need_data(p);
   if (rc) return rc;
   if (!t || !hQ || !hKs || !hVs || !hdO || !cfg || !hO || !hLSE || !hdQ || !scratch) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
@@ -1173,60 +1187,81 @@ int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const 
   if ((hdKs == nullptr) != (hdVs == nullptr)) { set_error("hdK_self / hdV_self: both or none"); return CAS_ERR_INVALID_ARG; }
   const StepScratch s = step_scratch(p, t, Hq);
   if (scratch_bytes < s.total) { set_error("scratch too small: need %zu", s.total); return CAS_ERR_CAPACITY; }
-  char* d = (char*)scratch;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t eb = p->elem_bytes, T = t->T, D = p->desc.D, Hkv = p->desc.Hkv;
-  // Inputs arrive on st_h2d (Q, K_self, V_self first: the forward pass starts as soon as they are in;
-  // dO lands under the forward pass), results leave on st_d2h (O and LSE under the backward pass, dQ and
-  // dK_self/dV_self under Adam).  The main stream ends by waiting for the last copy, so "main stream done"
-  // still means "everything done".
   cudaEvent_t* ev = p->ev_step;
-  CAS_CUDA(cudaEventRecord(ev[0], st));
   const bool same_layout = p->step_prev_scratch == scratch && p->step_prev_stream == st &&
                            memcmp(&p->step_prev_layout, &s, sizeof(StepScratch)) == 0;
-  if (same_layout) {
-    // back-to-back steps on the same scratch WITH THE SAME LAYOUT (same T, Hq, workspace size): the input regions
-    // are free as soon as the PREVIOUS backward pass is done (ev[4] still holds that record) and they do not
-    // overlap the output regions the previous step's read-back may still be copying from, so these copies run
-    // under the previous Adam and dQ read-back.  With a different layout (ragged batches: T changes per step) the
-    // regions move and may overlap O / LSE / dQ of the previous step: wait for its last read-back instead.
-    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[4], 0));
-  } else {
-    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
+  if (!same_layout) {
+    // first call, or the regions moved (ragged batches: T changes per step; another scratch or stream): everything
+    // still in flight on the old layout has to finish first
+    rc = cas_train_step_host_wait(p, stream);
+    if (rc) return rc;
+    p->step_count = 0;
   }
+  const int k = (int)(p->step_count & 1);
+  ++p->step_count;
   p->step_prev_scratch = scratch;
   p->step_prev_stream = st;
   p->step_prev_layout = s;
-  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[0], 0));
+  char* d = (char*)scratch + (size_t)k * s.set_bytes;
+  char* ws = (char*)scratch + s.oWs;
+  cudaEvent_t eIn1 = ev[1 + 5 * k], eIn2 = ev[2 + 5 * k], eFwd = ev[3 + 5 * k], eBwd = ev[4 + 5 * k], eOut = ev[5 + 5 * k];
+  if (same_layout) {
+    // step i-2 has read this set's inputs.  NOT ordered after the caller's stream: that would put these copies behind
+    // the previous step's Adam -- the host inputs must hold their data when the call is made.
+    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, eBwd, 0));
+  } else {
+    CAS_CUDA(cudaEventRecord(ev[0], st));
+    CAS_CUDA(cudaStreamWaitEvent(p->st_h2d, ev[0], 0));
+    CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[0], 0));
+  }
   CAS_CUDA(cudaMemcpyAsync(d + s.oQ, hQ, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
   CAS_CUDA(cudaMemcpyAsync(d + s.oKs, hKs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
   CAS_CUDA(cudaMemcpyAsync(d + s.oVs, hVs, T * Hkv * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
-  CAS_CUDA(cudaEventRecord(ev[1], p->st_h2d));
+  CAS_CUDA(cudaEventRecord(eIn1, p->st_h2d));
   CAS_CUDA(cudaMemcpyAsync(d + s.odO, hdO, T * Hq * D * eb, cudaMemcpyHostToDevice, p->st_h2d));
-  CAS_CUDA(cudaEventRecord(ev[2], p->st_h2d));
-  CAS_CUDA(cudaStreamWaitEvent(st, ev[1], 0));
+  CAS_CUDA(cudaEventRecord(eIn2, p->st_h2d));
+  CAS_CUDA(cudaStreamWaitEvent(st, eIn1, 0));
+  if (same_layout) { CAS_CUDA(cudaStreamWaitEvent(st, eOut, 0)); }       // step i-2's results have left this set
   rc = cas_prefix_attn_fwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, scale, d + s.oO, (float*)(d + s.oLSE), stream);
   if (rc) return rc;
-  CAS_CUDA(cudaEventRecord(ev[3], st));
-  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[3], 0));
+  CAS_CUDA(cudaEventRecord(eFwd, st));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, eFwd, 0));
   CAS_CUDA(cudaMemcpyAsync(hO, d + s.oO, T * Hq * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
   CAS_CUDA(cudaMemcpyAsync(hLSE, d + s.oLSE, T * Hq * 4, cudaMemcpyDeviceToHost, p->st_d2h));
-  CAS_CUDA(cudaStreamWaitEvent(st, ev[2], 0));
+  CAS_CUDA(cudaStreamWaitEvent(st, eIn2, 0));
   rc = cas_prefix_attn_bwd(p, t, Hq, d + s.oQ, d + s.oKs, d + s.oVs, d + s.oO, (float*)(d + s.oLSE), d + s.odO,
-                           scale, d + s.odQ, d + s.odKs, d + s.odVs, d + s.oWs, s.ws_bytes, stream);
+                           scale, d + s.odQ, d + s.odKs, d + s.odVs, ws, s.ws_bytes, stream);
   if (rc) return rc;
-  CAS_CUDA(cudaEventRecord(ev[4], st));
-  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, ev[4], 0));
+  CAS_CUDA(cudaEventRecord(eBwd, st));
+  CAS_CUDA(cudaStreamWaitEvent(p->st_d2h, eBwd, 0));
   CAS_CUDA(cudaMemcpyAsync(hdQ, d + s.odQ, T * Hq * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
   if (hdKs) {
     CAS_CUDA(cudaMemcpyAsync(hdKs, d + s.odKs, T * Hkv * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
     CAS_CUDA(cudaMemcpyAsync(hdVs, d + s.odVs, T * Hkv * D * eb, cudaMemcpyDeviceToHost, p->st_d2h));
   }
-  CAS_CUDA(cudaEventRecord(ev[5], p->st_d2h));
+  CAS_CUDA(cudaEventRecord(eOut, p->st_d2h));
   rc = cas_adam_step(p, cfg, nullptr, 0, nullptr, stream);
   if (rc) return rc;
-  CAS_CUDA(cudaStreamWaitEvent(st, ev[5], 0));
+  if (wait_readback) CAS_CUDA(cudaStreamWaitEvent(st, eOut, 0));
   return CAS_OK;
+}
+
+int cas_train_step_host(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
+                        const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
+                        float* hLSE, void* hdQ, void* hdKs, void* hdVs, void* scratch, size_t scratch_bytes,
+                        void* stream) {
+  return train_step_host(p, t, Hq, hQ, hKs, hVs, hdO, scale, cfg, hO, hLSE, hdQ, hdKs, hdVs, scratch, scratch_bytes,
+                         stream, true);
+}
+
+int cas_train_step_host_async(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* hQ, const void* hKs,
+                              const void* hVs, const void* hdO, float scale, const cas_adam_cfg* cfg, void* hO,
+                              float* hLSE, void* hdQ, void* hdKs, void* hdVs, void* scratch, size_t scratch_bytes,
+                              void* stream) {
+  return train_step_host(p, t, Hq, hQ, hKs, hVs, hdO, scale, cfg, hO, hLSE, hdQ, hdKs, hdVs, scratch, scratch_bytes,
+                         stream, false);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -99,8 +99,10 @@ struct PoolLayer {
 };
 
 // Layout of cas_train_step_host's device scratch (byte offsets of the staged inputs, outputs and workspace).
+// Device scratch of cas_train_step_host: TWO buffer sets (inputs Q, K_self, V_self, dO and results O, LSE, dQ,
+// dK_self, dV_self; offsets relative to the set) used alternately by consecutive steps, then the backward workspace.
 struct StepScratch {
-  size_t oQ, oKs, oVs, odO, oO, oLSE, odQ, odKs, odVs, oWs, ws_bytes, total;
+  size_t oQ, oKs, oVs, odO, oO, oLSE, odQ, odKs, odVs, set_bytes, oWs, ws_bytes, total;
 };
 
 struct cas_pool {
@@ -142,7 +144,10 @@ struct cas_pool {
   cudaStream_t st_upload = nullptr;  // slot-table uploads
   // cas_train_step_host: input / output copies on their own streams so they overlap the kernels
   cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
-  cudaEvent_t ev_step[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  // events of cas_train_step_host: [0] call begin; per buffer set k: [1+5k] Q/K_self/V_self in, [2+5k] dO in,
+  // [3+5k] forward done, [4+5k] backward done, [5+5k] last read-back done
+  cudaEvent_t ev_step[11] = {};
+  int64_t step_count = 0;                // steps since the last layout change (buffer set = step_count & 1)
   void* step_prev_scratch = nullptr;     // scratch / stream of the previous cas_train_step_host call
   cudaStream_t step_prev_stream = nullptr;
   StepScratch step_prev_layout{};

@@ -239,6 +239,49 @@ def test_train_step_host_back_to_back_with_changing_layout():
     sess.close()
 
 
+def test_train_step_host_async_pipelines_steps_over_two_buffer_sets():
+    """cas_train_step_host_async: six steps with DIFFERENT inputs are issued back to back without any
+    synchronisation (step i+1's inputs are copied into the other buffer set while step i computes, step i's dQ is
+    still leaving while step i+1 runs); after cas_train_step_host_wait every step's host results equal those of
+    the same step run alone with the per-call-complete variant (lr = 0: the parameters stay fixed, so each input
+    has one right answer).  Catches a buffer set overwritten before its last reader, results read back from the
+    wrong set, and a wait that does not cover both sets."""
+    base = CONFIGS["c2"].scaled(name="c2_async", n_carts=8, n_slots=8, cart_len=300, B=3, Lq=700, n_dist=2, lr=0.0)
+    wls = [make_workload(base, 43)]
+    cas.cas_set_impl(cas.CAS_IMPL_AUTO)
+    sess = Session(wls[0])
+    rng = np.random.Generator(np.random.PCG64(44))
+    from workloads import round_to_dtype
+    hs = []
+    for i in range(6):                              # same table (same layout), fresh Q / K_self / V_self / dO per step
+        h = _host_step_buffers(sess, wls[0])
+        if i:
+            for k in ("Q", "Ks", "Vs", "dO"):
+                a = round_to_dtype(rng.standard_normal(tuple(h[k].shape), dtype=np.float32) * (0.5 + 0.3 * i), "bf16")
+                h[k].copy_(torch.from_numpy(a).to(sess.tdt))
+        hs.append(h)
+    scratch = torch.empty(cas.cas_train_step_host_scratch_bytes(sess.pool, sess.tab, base.Hq), dtype=torch.uint8,
+                          device="cuda")
+    want = []
+    for h in hs:                                    # each step alone, fully synchronised
+        _host_step(sess, sess.tab, h, scratch)
+        torch.cuda.synchronize()
+        want.append({k: h[k].clone() for k in ("O", "LSE", "dKs", "dVs", "dQ")})
+        for k in ("O", "LSE", "dKs", "dVs", "dQ"):
+            h[k].fill_(7.0)
+    assert not torch.equal(want[0]["O"], want[1]["O"])
+    for h in hs:
+        cas.cas_train_step_host_async(sess.pool, sess.tab, base.Hq, h["Q"], h["Ks"], h["Vs"], h["dO"], sess.scale,
+                                      sess.adam_cfg(), h["O"], h["LSE"], h["dQ"], h["dKs"], h["dVs"], scratch)
+    cas.cas_train_step_host_wait(sess.pool)
+    torch.cuda.current_stream().synchronize()       # the CALLER's stream only: the wait made it cover the copies
+    for i, h in enumerate(hs):
+        for k in ("O", "LSE", "dKs", "dVs"):
+            assert torch.equal(h[k], want[i][k]), (i, k)
+        assert rel_fro(h["dQ"].float().numpy(), want[i]["dQ"].float().numpy()) < 1e-2, i
+    sess.close()
+
+
 def test_cta_pair_mma_selftest():
     """tcgen05.mma.cta_group::2 on a 2-CTA cluster (the primitives kept in cas_sm100.cuh for the next kernels):
     exact against an integer-valued reference."""
