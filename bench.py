@@ -448,8 +448,13 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
             gbs = (kv_bytes + io_bytes) / (t_fwd * 1e-3) / 1e9
             roof = {"kernel": "attn_fwd", "bound": "hbm", "achieved": gbs, "peak": peaks["hbm"], "unit": "GB/s",
                     "frac": gbs / peaks["hbm"], "traffic": traffic, "peak_source": peaks["src"] + " hbm_gbs",
-                    "algorithmic_bytes": kv_bytes + io_bytes, "tflops": achieved}
-        n_launch = 5 if cfg.backward else (1 if sess.tab.B * cfg.Hq <= 256 else 2)
+                    "algorithmic_bytes": kv_bytes + io_bytes, "tflops": achieved,
+                    # c5 "all loaded" (256 rows x 256 k keys per KV head) needs as long on the tensor pipe at its
+                    # peak as on HBM at its peak: both fractions are reported
+                    "frac_of_bf16_burst_peak": achieved / peaks["bf16"]}
+        # fwd (+ fwd_combine when the tail is split), bwd_prep, bwd, dq_convert, adam  /  decode (+ decode_combine)
+        fwd_split = tc and cas.cas_slot_table_fwd_split(sess.tab)[0] > 0
+        n_launch = (5 + int(fwd_split)) if cfg.backward else (1 if sess.tab.B * cfg.Hq <= 256 else 2)
         line = {
             "metric": METRIC, "value": total_flops / (ms_step_max * 1e-3) / 1e12, "unit": UNIT,
             "n_gpus": world, "steps": steps, "warmup": max(warmup, 3), "ms_per_step": ms_step_max,

@@ -184,6 +184,12 @@ int cas_slot_table_info(const cas_slot_table* table, cas_table_info* out);
  * tokens visible to sequence b). */
 int cas_slot_table_export(const cas_slot_table* table, int32_t* sel_slot, int32_t* inv_off,
                           int32_t* inv_seq, int64_t* P);
+/* Diagnostic: the tail split the last tensor-core forward call planned for this table (0 blocks / 1 part before
+ * the first call or when nothing is split).  The forward kernel runs one CTA per (256 query rows, head); when
+ * the last wave of CTAs would fill less than half of the SMs, those n_tail blocks are cut along the KV axis into
+ * n_parts CTAs each, whose un-normalised partials a small second kernel merges -- the result is the same
+ * attention, summed in a different order. */
+int cas_slot_table_fwd_split(const cas_slot_table* table, int32_t* n_tail, int32_t* n_parts);
 /* "query token position IDs must be offset by the total number of active cartridge
  * KV tokens".  total_resident = tokens of all resident cartridges (the packed layout of
  * PAPER.md:71); P[b] = tokens visible to sequence b.  Either may be NULL. */
@@ -211,7 +217,8 @@ int cas_rope_apply(int32_t dtype, int32_t B, const int32_t* seq_off, const int64
  *   s_j = scale*q.k_j ; LSE[t,h] = ln sum_j exp(s_j) ; O[t,h,:] = sum_j exp(s_j-LSE) v_j.
  * Q,O device [T,Hq,D] dtype; K_self,V_self device [T,Hkv,D] dtype or both NULL (prefix only; then
  * every sequence must select >= 1 cartridge); LSE device [T,Hq] fp32.  scale must be positive and finite
- * (CAS_ERR_INVALID_ARG otherwise: the kernels take row maxima on the raw scores).  Pool rows past a cartridge's
+ * (CAS_ERR_INVALID_ARG otherwise: the kernels take row maxima on the raw scores).  Forward calls on one pool must be
+ * ordered by the caller (one stream, or events): they share the pool's split-KV partial scratch.  Pool rows past a cartridge's
  * length inside its slot are read by the tile loads and masked; they must stay finite (the arena is zero-filled at
  * creation and the library never writes there). */
 int cas_prefix_attn_fwd(cas_pool* pool, const cas_slot_table* table, int32_t Hq, const void* Q,

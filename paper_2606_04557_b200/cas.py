@@ -413,6 +413,12 @@ def cas_warmup_scales(pool: Pool, slots, w_c: int, n_b: int) -> np.ndarray:
     return out
 
 
+def cas_slot_table_fwd_split(tab: SlotTable):
+    a, b = C.c_int32(0), C.c_int32(0)
+    _check(lib().cas_slot_table_fwd_split(tab.handle, C.byref(a), C.byref(b)))
+    return a.value, b.value
+
+
 def cas_train_step_host_scratch_bytes(pool: Pool, tab: SlotTable, Hq: int) -> int:
     n = C.c_size_t(0)
     _check(lib().cas_train_step_host_scratch_bytes(pool.handle, tab.handle, C.c_int32(Hq), C.byref(n)))

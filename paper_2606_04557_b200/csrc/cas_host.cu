@@ -234,6 +234,11 @@ int cas_pool_create(const cas_pool_desc* desc, void* dev_arena, void* pinned_are
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_upload, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking);
     for (int i = 0; i < 11 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&p->ev_step[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) {
+      int dev = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    }
     p->ev_cart.assign(desc->n_carts, nullptr);   // created at a cartridge's first eviction
     p->ev_slot.assign(desc->n_slots, nullptr);
     for (int s2 = 0; s2 < desc->n_slots && e == cudaSuccess; ++s2)
@@ -267,6 +272,7 @@ int cas_pool_destroy(cas_pool* p) {
     }
     p->tab_free.clear();
     if (p->st_d2h) cudaStreamDestroy(p->st_d2h);
+    if (p->fwd_part) cudaFree(p->fwd_part);
     for (cudaEvent_t ev : p->ev_step) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : p->ev_slot) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : p->ev_cart) if (ev) cudaEventDestroy(ev);
@@ -638,6 +644,13 @@ int cas_slot_table_export(const cas_slot_table* t, int32_t* sel_slot, int32_t* i
   if (inv_off) memcpy(inv_off, t->inv_off.data(), t->inv_off.size() * 4);
   if (inv_seq && t->nsel) memcpy(inv_seq, t->inv_seq.data(), t->nsel * 4);
   if (P) memcpy(P, t->P.data(), t->B * 8);
+  return CAS_OK;
+}
+
+int cas_slot_table_fwd_split(const cas_slot_table* t, int32_t* n_tail, int32_t* n_parts) {
+  if (!t || !n_tail || !n_parts) { set_error("null arg"); return CAS_ERR_INVALID_ARG; }
+  *n_tail = t->fwd_plan_key < 0 ? 0 : t->fwd_n_tail;
+  *n_parts = t->fwd_plan_key < 0 ? 1 : t->fwd_n_parts;
   return CAS_OK;
 }
 

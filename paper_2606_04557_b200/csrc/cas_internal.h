@@ -148,6 +148,9 @@ struct cas_pool {
   // [3+5k] forward done, [4+5k] backward done, [5+5k] last read-back done
   cudaEvent_t ev_step[11] = {};
   int64_t step_count = 0;                // steps since the last layout change (buffer set = step_count & 1)
+  void* fwd_part = nullptr;              // split-KV partials of the forward kernel's tail blocks (grow-only)
+  size_t fwd_part_bytes = 0;
+  int n_sm = 148;
   void* step_prev_scratch = nullptr;     // scratch / stream of the previous cas_train_step_host call
   cudaStream_t step_prev_stream = nullptr;
   StepScratch step_prev_layout{};
@@ -199,6 +202,7 @@ struct cas_slot_table {
   cas::BwdItem* d_bwd_items = nullptr;
   cas::BwdItem* d_simt_bwd_items = nullptr;
   int32_t* d_counters = nullptr;              // persistent-scheduler tickets (zeroed per launch)
+  int fwd_plan_key = -1, fwd_n_tail = 0, fwd_n_parts = 1;   // forward tail split, planned at the first forward call
   // decode-shaped batches: segments of the persistent split-KV kernel, built lazily for a given Hq by cas_tc_decode.cu
   int32_t dec_Hq = 0;
   int64_t dec_rows = 0;                       // partial rows per KV head (prefix segments + one self row per sequence) x G

@@ -15,13 +15,21 @@
 //  * One segment = one (row block, KV head, run of tiles).  Two softmax warpgroups take alternate tiles (even tiles:
 //    S0/O0, odd tiles: S1/O1 in TMEM), each with its own running max and sum, so the exp work of tile j+1 overlaps
 //    the MMAs of tiles j and j+2; at the end of the segment the two accumulators are merged and written as ONE
-//    un-normalised partial (O, m, l) per row.
-//  * FUSED MERGE: every row (sequence, head) has a counter; the CTA that writes the row's last partial merges all of
-//    them (plus the few self keys of a young cache, dotted on the CUDA cores), normalises and writes O and LSE.
-//    No second launch.
-// Warps: 0-3 / 4-7 softmax warpgroups (thread = row = TMEM lane), 8 scheduler + TMA producer, 9 MMA issuer,
-// 10-11 query gather (the rows of the next segment while the current one drains).
-// SMEM: Q tile 32 KB + 3-stage K/V ring 192 KB.  TMEM (512 cols): S0 | S1 | O0 | O1.
+//    un-normalised partial (O, m, l) per row.  A group with MORE rows than one block (c5 "all loaded": 64 sequences
+//    x 4 heads = 256 rows) runs PAIRED segments (kind 2): two resident Q tiles, warpgroup w owns row block w and
+//    takes every tile, so a K/V tile is fetched once for both blocks (4 MMAs per tile) and each block writes its
+//    own partial.  Measured: same time as two separate segments (the period is the softmax -> PV -> QK chain of
+//    one warpgroup either way, and at 256 rows x 256 k keys the step is as tensor-bound as it is HBM-bound:
+//    0.27 PFLOP against 1.05 GB), but half the L2 -> SMEM traffic.
+//  * MERGE of a row's split-KV partials (plus the few self keys of a young cache, dotted on the CUDA cores),
+//    normalisation, O and LSE: small batches (<= 256 output rows, row blocks <= 32 rows, no paired segment) are merged
+//    IN this launch by warp 11 -- every row has a counter, the CTA that writes a row's last partial merges it --
+//    which saves the second launch of a latency-bound step; bigger batches by decode_combine_kernel (one warp per
+//    output row; measured 2x faster than the in-kernel merge at 2048 rows).
+// Warps: 0-3 / 4-7 softmax warpgroups (thread = row = TMEM lane), 8 scheduler + TMA producer (descriptors published
+// one segment ahead through a 4-deep ring), 9 MMA issuer, 10 query gather (the rows of the next segment while the
+// current one drains), 11 row counters + fused merge.
+// SMEM: two Q tiles 64 KB + K/V ring of five 32 KB slots (unit 2t = K(t), 2t+1 = V(t)).  TMEM (512 cols): S0 | S1 | O0 | O1.
 #include <algorithm>
 #include <cstring>
 #include <map>

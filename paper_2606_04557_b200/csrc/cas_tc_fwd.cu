@@ -16,7 +16,9 @@
 // rescaled when the running max grows by more than 2^8).
 #include "cas_sm100.cuh"
 #include "cas_tc_common.cuh"
+#include <algorithm>
 #include <cstdlib>
+#include <vector>
 
 namespace cas {
 using namespace sm100;
@@ -82,9 +84,14 @@ struct FwdParams {
   const FwdItem* items;
   __nv_bfloat16* O;
   float* LSE;
+  float* part;                   // split-KV partials of the tail blocks: [tail block][part][256 rows][kFwdPartStride]
   int Hq, Hkv, has_self;
+  int n_blocks;                  // (item, head) blocks = items x Hq, in KV-group-major order
+  int n_whole;                   // blocks [0, n_whole) run whole; each later one is cut into n_parts CTAs
+  int n_parts;
   float scale_log2;
 };
+constexpr int kFwdPartStride = 132;   // 128 O + m + l + pad (16-byte aligned rows)
 
 __device__ __forceinline__ float ex2(float x) {
   float y;
@@ -107,8 +114,14 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   // KV-group-major block order (inside a group: items longest first, the G heads of an item adjacent): the CTAs
   // in flight work on one KV group at a time, so its K/V tiles (shared by the G heads and by every sequence that
   // selected the cartridge) stay in L2
-  const int Gq = prm.Hq / prm.Hkv, per_group = gridDim.x / prm.Hkv;      // blocks of one KV group: items x G heads
-  const int g = blockIdx.x / per_group, rem = blockIdx.x % per_group;
+  const int Gq = prm.Hq / prm.Hkv, per_group = prm.n_blocks / prm.Hkv;    // blocks of one KV group: items x G heads
+  // TAIL SPLIT: the last blocks of the launch order (the ones that would run alone in a part-filled last wave) are
+  // cut along the KV axis into n_parts CTAs each, which write un-normalised partials merged by fwd_combine_kernel
+  const bool split = (int)blockIdx.x >= prm.n_whole;
+  const int tail_idx = split ? ((int)blockIdx.x - prm.n_whole) / prm.n_parts : 0;
+  const int part = split ? ((int)blockIdx.x - prm.n_whole) % prm.n_parts : 0;
+  const int blk = split ? prm.n_whole + tail_idx : (int)blockIdx.x;
+  const int g = blk / per_group, rem = blk % per_group;
   const int item_idx = rem / Gq, h = g * Gq + rem % Gq;
   const FwdItem it = prm.items[item_idx];
   const int t0 = prm.seq_off[it.seq], lq = prm.seq_off[it.seq + 1] - t0;
@@ -116,8 +129,12 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   const KvTile* tiles = prm.kv_tiles + prm.kv_tile_off[it.seq];
   const int nq = it.rows > 128 ? 2 : 1;
   const int diag0 = it.row0 >> 7;
-  const int nkv0 = n_pre + (prm.has_self ? diag0 + 1 : 0);
-  const int nkv1 = n_pre + (prm.has_self ? diag0 + 2 : 0);
+  const int n_all = n_pre + (prm.has_self ? diag0 + nq : 0);      // KV tiles of the block (tile 1 sees one more)
+  // this CTA's run of KV tiles [ja, jb): every part has >= 2 tiles (host), so Q tile 0 always has work
+  const int ja = split ? (int)((int64_t)part * n_all / prm.n_parts) : 0;
+  const int jb = split ? (int)((int64_t)(part + 1) * n_all / prm.n_parts) : n_all;
+  const int nkv0 = min(jb, n_pre + (prm.has_self ? diag0 + 1 : 0)) - ja;     // tiles of Q tile 0 / 1, counted from ja
+  const int nkv1 = jb - ja;
   const int n_max = nq == 2 ? nkv1 : nkv0;
 
   if (threadIdx.x == 0) {
@@ -149,8 +166,8 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       for (int j = 0; j < n_max; ++j) {
         const int s = j & 1;
         const uint32_t ph = (j >> 1) & 1;
-        const bool pre = j < n_pre;
-        const int tok = pre ? tiles[j].tok : t0 + 128 * (j - n_pre);
+        const bool pre = ja + j < n_pre;
+        const int tok = pre ? tiles[ja + j].tok : t0 + 128 * (ja + j - n_pre);
         const CUtensorMap* mk = pre ? &tmKp : &tmKs;
         const CUtensorMap* mv = pre ? &tmVp : &tmVs;
         const PackedTile* pt = (pre && tok < 0) ? prm.ptiles + (-1 - tok) : nullptr;
@@ -256,11 +273,11 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       for (int j = 0; j < nkv; ++j) {
         int limit;
         const PackedTile* pt = nullptr;
-        if (j < n_pre) {
-          limit = tiles[j].len;
-          if (tiles[j].tok < 0) { pt = prm.ptiles + (-1 - tiles[j].tok); limit = 128; }
+        if (ja + j < n_pre) {
+          limit = tiles[ja + j].len;
+          if (tiles[ja + j].tok < 0) { pt = prm.ptiles + (-1 - tiles[ja + j].tok); limit = 128; }
         } else {
-          const int k0 = 128 * (j - n_pre);
+          const int k0 = 128 * (ja + j - n_pre);
           limit = min(min(128, lq - k0), row - k0 + 1);
         }
         mbar_wait(bar(B_SF + t), j & 1);
@@ -340,6 +357,22 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       // epilogue: O = acc / l, LSE = ln2 * m + ln(l)
       mbar_wait(bar(B_OD), 0);
       tc_fence_after();
+      if (split) {
+        // un-normalised partial (O, m, l) of this row over the CTA's run of tiles
+        float* prow = prm.part + ((((int64_t)tail_idx * prm.n_parts + part) * 256) + 128 * t + r) * kFwdPartStride;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tO + c * 32, o);
+          tc_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            __stcg(reinterpret_cast<float4*>(prow + c * 32 + 4 * i),
+                   make_float4(__uint_as_float(o[4 * i]), __uint_as_float(o[4 * i + 1]), __uint_as_float(o[4 * i + 2]),
+                               __uint_as_float(o[4 * i + 3])));
+        }
+        __stcg(reinterpret_cast<float2*>(prow + 128), make_float2(m, l));
+      } else {
       const float inv = 1.f / l;
       const bool ok = row < lq && r < it.rows - 128 * t;
       __nv_bfloat16* orow = prm.O + ((int64_t)(t0 + row) * prm.Hq + h) * 128;
@@ -361,11 +394,89 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         }
       }
       if (ok) prm.LSE[(int64_t)(t0 + row) * prm.Hq + h] = m * 0.6931471805599453f + logf(l);
+      }
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 8) tmem_dealloc(tbase, 512);
+}
+
+// Merge of the tail blocks' split-KV partials: one warp per (tail block, row); lane = 4 output columns.
+__global__ void __launch_bounds__(256)
+fwd_combine_kernel(const FwdParams prm, int n_tail) {
+  const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (w >= n_tail * 256) return;
+  const int tail_idx = w >> 8, rr = w & 255;
+  const int Gq = prm.Hq / prm.Hkv, per_group = prm.n_blocks / prm.Hkv;
+  const int blk = prm.n_whole + tail_idx;
+  const int g = blk / per_group, rem = blk % per_group;
+  const FwdItem it = prm.items[rem / Gq];
+  const int h = g * Gq + rem % Gq;
+  const int t0 = prm.seq_off[it.seq], lq = prm.seq_off[it.seq + 1] - t0;
+  const int row = it.row0 + rr;
+  if (rr >= it.rows || row >= lq) return;
+  const float* p0 = prm.part + (((int64_t)tail_idx * prm.n_parts) * 256 + rr) * kFwdPartStride;
+  float M = -INFINITY;
+  for (int q = 0; q < prm.n_parts; ++q) M = fmaxf(M, __ldcg(p0 + (int64_t)q * 256 * kFwdPartStride + 128));
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  float L = 0.f;
+  for (int q = 0; q < prm.n_parts; ++q) {
+    const float* pr = p0 + (int64_t)q * 256 * kFwdPartStride;
+    const float2 ml = __ldcg(reinterpret_cast<const float2*>(pr + 128));
+    const float4 v = __ldcg(reinterpret_cast<const float4*>(pr + 4 * lane));
+    const float f = ex2(ml.x - M);
+    L += f * ml.y;
+    acc.x += f * v.x; acc.y += f * v.y; acc.z += f * v.z; acc.w += f * v.w;
+  }
+  const float inv = 1.f / L;
+  uint2 o;
+  o.x = pack_bf16(acc.x * inv, acc.y * inv);
+  o.y = pack_bf16(acc.z * inv, acc.w * inv);
+  *reinterpret_cast<uint2*>(prm.O + ((int64_t)(t0 + row) * prm.Hq + h) * 128 + 4 * lane) = o;
+  if (lane == 0) prm.LSE[(int64_t)(t0 + row) * prm.Hq + h] = M * 0.6931471805599453f + logf(L);
+}
+
+// How many blocks at the end of the launch order to cut, and into how many parts.  Greedy list schedule of the
+// blocks (cost = KV tiles + a constant for prologue and epilogue) on the SMs, in launch order, the way the
+// hardware block scheduler deals them; the blocks that end later than the balanced makespan are the tail.
+static void plan_tail_split(const cas_slot_table* t, int Hq, int Hkv, bool has_self, int n_sm, int* n_tail, int* n_parts) {
+  *n_tail = 0;
+  *n_parts = 1;
+  const int Gq = Hq / Hkv;
+  const size_t n_items = t->fwd_items.size(), n_blocks = n_items * Hq;
+  if (n_blocks <= (size_t)n_sm || getenv("CAS_FWD_NO_SPLIT")) return;
+  std::vector<int> cost(n_items), tiles(n_items);
+  double total = 0;
+  for (size_t i = 0; i < n_items; ++i) {
+    const FwdItem& it = t->fwd_items[i];
+    const int n_pre = t->kv_tile_off[it.seq + 1] - t->kv_tile_off[it.seq];
+    tiles[i] = n_pre + (has_self ? (it.row0 >> 7) + (it.rows > 128 ? 2 : 1) : 0);
+    cost[i] = (it.rows > 128 ? 2 : 1) * tiles[i] + 3;
+    total += (double)cost[i] * Hq;
+  }
+  std::vector<int64_t> heap(n_sm, 0);               // min-heap of SM free times
+  auto cmp = [](int64_t a, int64_t b) { return a > b; };
+  std::vector<int64_t> finish(n_blocks);
+  for (size_t b = 0; b < n_blocks; ++b) {
+    const size_t item = (b % (n_items * Gq)) / Gq;
+    std::pop_heap(heap.begin(), heap.end(), cmp);
+    heap.back() += cost[item];
+    finish[b] = heap.back();
+    std::push_heap(heap.begin(), heap.end(), cmp);
+  }
+  const double balanced = total / n_sm * 1.03;
+  int r = 0;
+  while ((size_t)r < n_blocks && finish[n_blocks - 1 - r] > balanced) ++r;
+  if (r == 0 || 2 * r > n_sm) return;               // nothing sticks out, or the last wave is at least half full
+  int parts = std::min(n_sm / r, 8);
+  for (int i = 0; i < r; ++i) {
+    const size_t b = n_blocks - 1 - i;
+    parts = std::min(parts, tiles[(b % (n_items * Gq)) / Gq] / 2);      // every part keeps >= 2 KV tiles
+  }
+  if (parts < 2) return;
+  *n_tail = r;
+  *n_parts = parts;
 }
 
 int tc_attn_fwd(const AttnArgs& a) {
@@ -387,12 +498,45 @@ int tc_attn_fwd(const AttnArgs& a) {
     tmKs = a.L->tm_K;
     tmVs = a.L->tm_V;
   }
+  // tail split (cached per table and head count: a table serves every layer of a step)
+  cas_slot_table* tm = const_cast<cas_slot_table*>(t);
+  const int has_self = a.Ks ? 1 : 0;
+  if (tm->fwd_plan_key != a.Hq * 2 + has_self) {
+    plan_tail_split(t, a.Hq, a.Hkv, has_self != 0, a.pool->n_sm, &tm->fwd_n_tail, &tm->fwd_n_parts);
+    tm->fwd_plan_key = a.Hq * 2 + has_self;
+  }
+  const int n_blocks = (int)(n_items * a.Hq), n_tail = t->fwd_n_tail, n_parts = t->fwd_n_parts;
+  float* part = nullptr;
+  if (n_tail) {
+    // pool-owned, grow-only: forward calls on one pool are ordered by the caller's stream (cas.h)
+    const size_t need = (size_t)n_tail * n_parts * 256 * kFwdPartStride * sizeof(float);
+    cas_pool* pm = const_cast<cas_pool*>(a.pool);
+    if (pm->fwd_part_bytes < need) {
+      if (pm->fwd_part) {
+        cudaError_t e = cudaStreamSynchronize(a.stream);     // the old buffer may still be read by an earlier call
+        if (e != cudaSuccess) return cuda_fail(e, "fwd partial scratch sync");
+        cudaFree(pm->fwd_part);
+        pm->fwd_part = nullptr;
+        pm->fwd_part_bytes = 0;
+      }
+      cudaError_t e = cudaMalloc(&pm->fwd_part, need);
+      if (e != cudaSuccess) return cuda_fail(e, "fwd partial scratch");
+      pm->fwd_part_bytes = need;
+    }
+    part = (float*)pm->fwd_part;
+  }
   FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, t->d_ptiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
-                a.Hq, a.Hkv, a.Ks ? 1 : 0, a.scale * 1.4426950408889634f};
-  const unsigned grid = (unsigned)(n_items * a.Hq);
+                part, a.Hq, a.Hkv, has_self, n_blocks, n_blocks - n_tail, n_parts, a.scale * 1.4426950408889634f};
+  const unsigned grid = (unsigned)(n_blocks - n_tail + n_tail * n_parts);
   tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.L->tm_K, a.L->tm_V, tmKs, tmVs, a.L->tm_K16, a.L->tm_V16, prm);
   cudaError_t e = cudaGetLastError();
-  return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc fwd launch");
+  if (e != cudaSuccess) return cuda_fail(e, "tc fwd launch");
+  if (n_tail) {
+    fwd_combine_kernel<<<(n_tail * 256 * 32 + 255) / 256, 256, 0, a.stream>>>(prm, n_tail);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fwd combine launch");
+  }
+  return CAS_OK;
 }
 
 }  // namespace cas

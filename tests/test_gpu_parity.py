@@ -282,6 +282,45 @@ def test_train_step_host_async_pipelines_steps_over_two_buffer_sets():
     sess.close()
 
 
+@pytest.mark.parametrize("self_block", [True, False])
+def test_forward_tail_split_matches_whole_blocks_and_the_oracle(self_block):
+    """tc_fwd_kernel's tail split (cas.h cas_slot_table_fwd_split): 25 row blocks x 8 heads = 200 CTAs on 148 SMs,
+    the 52 that would run alone in the last wave are cut along the KV axis and merged by fwd_combine_kernel.  The
+    split rows live in the LAST KV head group: that group is compared with the oracle (a wrong tile range or merge
+    weight fails 2e-2 there), and every row of O / LSE is compared with the same launch run unsplit (row by row: a
+    single wrong tail row cannot hide in a Frobenius norm over the batch).  Ragged lengths: partly filled last
+    row blocks, 128-row blocks (one Q tile) and prefix tiles with a ragged end."""
+    import os
+    cfg = CONFIGS["c2"].scaled(name="c2_tail", Hq=8, Hkv=2, n_carts=9, n_slots=9, cart_len=0, len_mu=6.0,
+                               len_sigma=0.5, len_min=200, len_max=900, B=5, Lq=0, lq_min=1050, lq_max=1270, n_dist=2)
+    wl = make_workload(cfg, 47)
+    assert sum((int(l) + 255) // 256 for l in np.diff(wl.seq_off)) * cfg.Hq > 148
+    cas.cas_set_impl(cas.CAS_IMPL_AUTO)
+    sess = check_attention(wl, cas.CAS_IMPL_AUTO, kv_heads=[cfg.Hkv - 1], self_block=self_block, backward=False)
+    n_tail, n_parts = cas.cas_slot_table_fwd_split(sess.tab)
+    assert n_tail > 0 and n_parts >= 2, (n_tail, n_parts)
+    O1, L1 = sess.O.clone(), sess.LSE.clone()
+    os.environ["CAS_FWD_NO_SPLIT"] = "1"
+    try:
+        tab2 = cas.cas_slot_table_build(sess.pool, wl.seq_off, wl.sel_off, wl.sel_cart, 0)
+        old, sess.tab = sess.tab, tab2
+        sess.O.zero_()
+        sess.fwd(self_block=self_block)
+        torch.cuda.synchronize()
+        assert cas.cas_slot_table_fwd_split(tab2) == (0, 1)
+    finally:
+        del os.environ["CAS_FWD_NO_SPLIT"]
+    a, b = O1.float().cpu().numpy(), sess.O.float().cpu().numpy()
+    per_row = np.linalg.norm(a - b, axis=2) / (np.linalg.norm(b, axis=2) + 1e-30)
+    assert per_row.max() <= 1e-2, per_row.max()                  # bf16 rounding of a differently ordered sum
+    assert (per_row > 0).sum() <= n_tail * 256                   # only the split rows may differ at all
+    np.testing.assert_allclose(L1.cpu().numpy(), sess.LSE.cpu().numpy(), rtol=1e-5, atol=1e-5)
+    sess.tab = old
+    tab2.close()
+    sess.close()
+    print("tail split", n_tail, n_parts)
+
+
 def test_cta_pair_mma_selftest():
     """tcgen05.mma.cta_group::2 on a 2-CTA cluster (the primitives kept in cas_sm100.cuh for the next kernels):
     exact against an integer-valued reference."""
