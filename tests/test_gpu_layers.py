@@ -43,8 +43,8 @@ def make_pool(cfg, L, seed, n_slots=None):
     return wl, pool, KV
 
 
-def test_train_step_layers_L3_two_micro_batches():
-    L, n_micro = 3, 2
+def test_train_step_layers_L4_four_micro_batches():
+    L, n_micro = 4, 4
     cfg = CONFIGS["c2"].scaled(name="c2_layers", Hq=8, Hkv=2, n_carts=7, n_slots=7, cart_len=200, B=2, Lq=260,
                                n_dist=2)
     wl, pool, KV = make_pool(cfg, L, 81)
@@ -53,7 +53,7 @@ def test_train_step_layers_L3_two_micro_batches():
     scale = 1.0 / float(np.sqrt(cfg.D))
     tabs, batches, io = [], [], []
     for m in range(n_micro):
-        lq = [260, 131] if m == 0 else [77, 300]                   # different packing per micro-batch
+        lq = [[260, 131], [77, 300], [129, 128], [1, 257]][m]      # different packing per micro-batch
         seq_off = np.concatenate([[0], np.cumsum(lq)]).astype(np.int32)
         sel_off, sel_cart = draw_batch_selection(cfg, rng, list(range(cfg.n_carts)), wl.cart_len)
         tabs.append(cas.cas_slot_table_build(pool, seq_off, sel_off, sel_cart, m))
@@ -97,7 +97,7 @@ def test_train_step_layers_L3_two_micro_batches():
             assert rel_fro(t["dV_self"].float().cpu().numpy(), dVso) <= TOL_BF16_DKV
         for c in range(cfg.n_carts):
             g_gpu = {kv: cas.cas_pool_read(pool, c, "g" + kv, layer=l) for kv in "KV"}
-            if c in gK:                                              # accumulated over both micro-batches, per slot
+            if c in gK:                                              # accumulated over all micro-batches, per slot
                 assert rel_fro(g_gpu["K"], gK[c]) <= TOL_BF16_DKV, (l, c)
                 assert rel_fro(g_gpu["V"], gV[c]) <= TOL_BF16_DKV, (l, c)
             else:
