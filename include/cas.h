@@ -352,12 +352,43 @@ int cas_prefix_attn_bwd_layer(cas_pool* pool, const cas_slot_table* table, int32
 int cas_decode_attn_layer(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
                           const void* K_cache, const void* V_cache, int32_t cache_cap, const int32_t* self_len,
                           float scale, void* O, float* LSE, void* stream);
-/* Device buffers of one (micro-batch, layer): shapes as in cas_prefix_attn_fwd / _bwd. */
+/* ---- RoPE fused into the attention calls (PAPER.md:77 the offset is "recomputed at each
+ * step") -----------------------------------------------------------------------------------------------------
+ * cas_rope_table writes, once per packed batch (it serves every head and every layer), cs[t][k] = (cos, sin) of
+ * m_t * base^(-2k/D) as device fp32 [T, D/2, 2]; position ids, angle arithmetic (double) and argument checks as
+ * cas_rope_apply.  cas_prefix_attn_fwd_rope takes UN-rotated Q / K_self: the forward kernel rotates every Q tile
+ * in shared memory as it arrives and writes the rotated rows to Q_rot (device [T, Hq, D] bf16) -- no separate pass
+ * reads and re-writes Q -- and K_self (1/G of the query bytes) is rotated into K_self_rot by a small pass in the same
+ * call; the attention is that of cas_prefix_attn_fwd on the rotated tensors.  cas_prefix_attn_bwd_rope takes Q_rot
+ * and K_self_rot as left by the forward call and returns dQ and dK_self with respect to the UN-rotated inputs: the
+ * transpose rotation is applied to dQ in fp32 inside the kernel that converts the dQ accumulators to bf16, and to
+ * dK_self in place.  Cartridge K/V in the pool are not rotated (they are trained as they are).  Tensor-core path only
+ * (bf16, D = 128, more than one query token per sequence somewhere): otherwise CAS_ERR_SHAPE -- use cas_rope_apply. */
+typedef struct cas_rope {
+  const float* cs;    /* device [T, D/2, 2], written by cas_rope_table for the SAME seq_off as the slot table */
+  int32_t layout;     /* 0: pairs (2k, 2k+1); 1: pairs (k, k + D/2) -- as cas_rope_apply */
+  int32_t reserved;
+} cas_rope;
+int cas_rope_table(int32_t B, const int32_t* seq_off, const int64_t* pos_off, int32_t D, double base, float* cs,
+                   void* stream);
+int cas_prefix_attn_fwd_rope(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
+                             const void* K_self, const void* V_self, const cas_rope* rope, void* Q_rot,
+                             void* K_self_rot, float scale, void* O, float* LSE, void* stream);
+int cas_prefix_attn_bwd_rope(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq,
+                             const void* Q_rot, const void* K_self_rot, const void* V_self, const void* O,
+                             const float* LSE, const void* dO, const cas_rope* rope, float scale, void* dQ,
+                             void* dK_self, void* dV_self, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Device buffers of one (micro-batch, layer): shapes as in cas_prefix_attn_fwd / _bwd.  rope != NULL: Q and K_self
+ * are un-rotated, the step runs the *_rope calls with Q_rot / K_self_rot as scratch outputs (K_self_rot may be NULL
+ * when K_self is). */
 typedef struct {
   const void *Q, *K_self, *V_self, *dO;
   void* O;
   float* LSE;
   void *dQ, *dK_self, *dV_self;
+  const cas_rope* rope;
+  void *Q_rot, *K_self_rot;
 } cas_layer_io;
 /* One optimizer step: for every micro-batch m (its own slot table tables[m], all built against the current
  * residency) the forward pass of layers 0..L-1, then the backward pass of layers L-1..0 -- dK/dV ACCUMULATE into the

@@ -309,22 +309,56 @@ def cas_prefix_attn_bwd(pool: Pool, tab: SlotTable, Hq: int, Q, K_self, V_self, 
                                            _stream(stream)))
 
 
+class Rope(C.Structure):
+    """cas_rope: the device cos/sin table of cas_rope_table (kept alive here) and the pair layout."""
+    _fields_ = [("cs", C.c_void_p), ("layout", C.c_int32), ("reserved", C.c_int32)]
+
+    def __init__(self, table, layout: int):
+        super().__init__(table.data_ptr(), layout, 0)
+        self.table = table
+
+
+def cas_rope_table(seq_off, pos_off, D: int, base: float, cs, stream=None):
+    so, po = _i32(seq_off), np.ascontiguousarray(pos_off, dtype=np.int64)
+    _check(lib().cas_rope_table(C.c_int32(len(so) - 1), _p(so), _p(po, C.c_int64), C.c_int32(D), C.c_double(base),
+                                _dptr(cs), _stream(stream)))
+
+
+def cas_prefix_attn_fwd_rope(pool: Pool, tab: SlotTable, Hq: int, Q, Ks, Vs, rope: Rope, Q_rot, Ks_rot, scale: float,
+                             O, LSE, stream=None, layer: int = 0):
+    _check(lib().cas_prefix_attn_fwd_rope(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q), _dptr(Ks),
+                                          _dptr(Vs), C.byref(rope), _dptr(Q_rot), _dptr(Ks_rot), C.c_float(scale),
+                                          _dptr(O), _dptr(LSE), _stream(stream)))
+
+
+def cas_prefix_attn_bwd_rope(pool: Pool, tab: SlotTable, Hq: int, Q_rot, Ks_rot, Vs, O, LSE, dO, rope: Rope,
+                             scale: float, dQ, dKs, dVs, workspace, stream=None, layer: int = 0):
+    _check(lib().cas_prefix_attn_bwd_rope(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q_rot),
+                                          _dptr(Ks_rot), _dptr(Vs), _dptr(O), _dptr(LSE), _dptr(dO), C.byref(rope),
+                                          C.c_float(scale), _dptr(dQ), _dptr(dKs), _dptr(dVs), _dptr(workspace),
+                                          C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream)))
+
+
 class LayerIO(C.Structure):
     _fields_ = [("Q", C.c_void_p), ("K_self", C.c_void_p), ("V_self", C.c_void_p), ("dO", C.c_void_p),
                 ("O", C.c_void_p), ("LSE", C.c_void_p), ("dQ", C.c_void_p), ("dK_self", C.c_void_p),
-                ("dV_self", C.c_void_p)]
+                ("dV_self", C.c_void_p), ("rope", C.c_void_p), ("Q_rot", C.c_void_p), ("K_self_rot", C.c_void_p)]
 
 
 def cas_train_step_layers(pool: Pool, tabs, Hq: int, io, scale: float, cfg: AdamCfg, lr_scale=None, workspace=None,
                           stream=None):
-    """io[m][l]: dict of torch tensors Q, K_self, V_self, dO, O, LSE, dQ, dK_self, dV_self (micro-batch m, layer l)."""
+    """io[m][l]: dict of torch tensors Q, K_self, V_self, dO, O, LSE, dQ, dK_self, dV_self (micro-batch m, layer l);
+    optional fused RoPE: "rope" (a Rope), "Q_rot", "K_self_rot"."""
     n_micro, L = len(tabs), pool.n_layers
     arr = (LayerIO * (n_micro * L))()
     for m in range(n_micro):
         for l in range(L):
             for k, _ in LayerIO._fields_:
                 t = io[m][l].get(k)
-                setattr(arr[m * L + l], k, None if t is None else t.data_ptr())
+                if k == "rope":         # a Rope structure (kept alive by the caller's dict), passed by address
+                    setattr(arr[m * L + l], k, None if t is None else C.addressof(t))
+                else:
+                    setattr(arr[m * L + l], k, None if t is None else t.data_ptr())
     tp = (C.c_void_p * n_micro)(*[t.handle for t in tabs])
     ls = None if lr_scale is None else np.ascontiguousarray(lr_scale, dtype=np.float32)
     _check(lib().cas_train_step_layers(pool.handle, tp, C.c_int32(n_micro), C.c_int32(Hq), arr, C.c_float(scale),

@@ -711,8 +711,21 @@ static bool use_tc(const cas_pool* p, const cas_slot_table* t, int Hq, int* rc) 
   return ok;
 }
 
-int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
-                              const void* Ks, const void* Vs, float scale, void* O, float* LSE, void* stream) {
+static int check_rope(const cas_pool* p, const cas_slot_table* t, int Hq, const cas_rope* rope) {
+  if (!rope->cs) { set_error("rope: null cos/sin table"); return CAS_ERR_INVALID_ARG; }
+  if (rope->layout != 0 && rope->layout != 1) { set_error("rope: layout must be 0 or 1"); return CAS_ERR_INVALID_ARG; }
+  int rc = CAS_OK;
+  if (!use_tc(p, t, Hq, &rc) || rc || tc_decode_supported(p, t, Hq)) {
+    if (rc) return rc;
+    set_error("fused RoPE runs on the tensor-core training kernels (bf16, D = 128, not decode-shaped): use cas_rope_apply");
+    return CAS_ERR_SHAPE;
+  }
+  return CAS_OK;
+}
+
+static int attn_fwd_impl(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                         const void* Ks, const void* Vs, float scale, void* O, float* LSE, void* stream,
+                         const cas_rope* rope, void* Q_rot, void* Ks_rot) {
   int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
   if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
@@ -724,6 +737,18 @@ int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
   a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O_out = O; a.LSE_out = LSE; a.scale = scale;
   a.stream = (cudaStream_t)stream;
   a.layer = layer; a.L = &p->layers[layer];
+  if (rope) {
+    rc = check_rope(p, t, Hq, rope);
+    if (rc) return rc;
+    if (!Q_rot || (Ks && !Ks_rot)) { set_error("rope: Q_rot / K_self_rot outputs missing"); return CAS_ERR_INVALID_ARG; }
+    if (Ks) {   // K_self (1/G of the query bytes) is rotated by its own small pass; Q inside the forward kernel
+      rc = rope_table_rotate(Ks, Ks_rot, rope->cs, t->T, p->desc.Hkv, rope->layout, 0, (cudaStream_t)stream);
+      if (rc) return rc;
+      a.Ks = Ks_rot;
+    }
+    a.rope_cs = rope->cs; a.rope_layout = rope->layout; a.Q_rot = Q_rot;
+    return tc_attn_fwd(a);
+  }
   const bool tc = use_tc(p, t, Hq, &rc);
   if (rc) return rc;
   if (tc && tc_decode_supported(p, t, Hq)) {
@@ -732,6 +757,18 @@ int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
     return tc_decode_fwd(a, Ks, Vs, 1, ones.data());
   }
   return tc ? tc_attn_fwd(a) : simt_attn_fwd(a);
+}
+
+int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                              const void* Ks, const void* Vs, float scale, void* O, float* LSE, void* stream) {
+  return attn_fwd_impl(p, t, layer, Hq, Q, Ks, Vs, scale, O, LSE, stream, nullptr, nullptr, nullptr);
+}
+
+int cas_prefix_attn_fwd_rope(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                             const void* Ks, const void* Vs, const cas_rope* rope, void* Q_rot, void* Ks_rot,
+                             float scale, void* O, float* LSE, void* stream) {
+  if (!rope) { set_error("null rope"); return CAS_ERR_INVALID_ARG; }
+  return attn_fwd_impl(p, t, layer, Hq, Q, Ks, Vs, scale, O, LSE, stream, rope, Q_rot, Ks_rot);
 }
 
 int cas_prefix_attn_fwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
@@ -796,12 +833,16 @@ int cas_prefix_attn_bwd_workspace_bytes(const cas_pool* p, const cas_slot_table*
   return CAS_OK;
 }
 
-int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
-                              const void* Ks, const void* Vs, const void* O, const float* LSE, const void* dO,
-                              float scale, void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes,
-                              void* stream) {
+static int attn_bwd_impl(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                         const void* Ks, const void* Vs, const void* O, const float* LSE, const void* dO,
+                         float scale, void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes,
+                         void* stream, const cas_rope* rope) {
   int rc = check_attn(p, t, Hq, Ks, Vs, scale);
   if (rc) return rc;
+  if (rope) {
+    rc = check_rope(p, t, Hq, rope);
+    if (rc) return rc;
+  }
   if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
   int32_t* dirty = p->grad_dirty.data() + (size_t)layer * p->desc.n_slots;
   rc = table_on_stream(t, stream);
@@ -833,10 +874,30 @@ int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
       if (rc) return rc;
     }
   }
+  if (rope) { a.rope_cs = rope->cs; a.rope_layout = rope->layout; }      // dq_convert_kernel applies R^T to dQ
   rc = tc ? tc_attn_bwd(a) : simt_attn_bwd(a);
   if (rc) return rc;
   for (int s2 : t->used_slots) dirty[s2] = 1;
+  if (rope && dKs)   // dK_self back through the rotation (in place)
+    return rope_table_rotate(dKs, dKs, rope->cs, t->T, p->desc.Hkv, rope->layout, 1, (cudaStream_t)stream);
   return CAS_OK;
+}
+
+int cas_prefix_attn_bwd_layer(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                              const void* Ks, const void* Vs, const void* O, const float* LSE, const void* dO,
+                              float scale, void* dQ, void* dKs, void* dVs, void* workspace, size_t workspace_bytes,
+                              void* stream) {
+  return attn_bwd_impl(p, t, layer, Hq, Q, Ks, Vs, O, LSE, dO, scale, dQ, dKs, dVs, workspace, workspace_bytes, stream,
+                       nullptr);
+}
+
+int cas_prefix_attn_bwd_rope(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q_rot,
+                             const void* Ks_rot, const void* Vs, const void* O, const float* LSE, const void* dO,
+                             const cas_rope* rope, float scale, void* dQ, void* dKs, void* dVs, void* workspace,
+                             size_t workspace_bytes, void* stream) {
+  if (!rope) { set_error("null rope"); return CAS_ERR_INVALID_ARG; }
+  return attn_bwd_impl(p, t, layer, Hq, Q_rot, Ks_rot, Vs, O, LSE, dO, scale, dQ, dKs, dVs, workspace, workspace_bytes,
+                       stream, rope);
 }
 
 int cas_prefix_attn_bwd(cas_pool* p, const cas_slot_table* t, int32_t Hq, const void* Q, const void* Ks,
@@ -1306,13 +1367,13 @@ int cas_train_step_layers(cas_pool* p, const cas_slot_table* const* tables, int3
     // forward through the layer stack, then backward in reverse order: the order a model visits its layers in
     for (int l = 0; l < L; ++l) {
       const cas_layer_io& x = io[(size_t)m * L + l];
-      rc = cas_prefix_attn_fwd_layer(p, t, l, Hq, x.Q, x.K_self, x.V_self, scale, x.O, x.LSE, stream);
+      rc = attn_fwd_impl(p, t, l, Hq, x.Q, x.K_self, x.V_self, scale, x.O, x.LSE, stream, x.rope, x.Q_rot, x.K_self_rot);
       if (rc) return rc;
     }
     for (int l = L - 1; l >= 0; --l) {
       const cas_layer_io& x = io[(size_t)m * L + l];
-      rc = cas_prefix_attn_bwd_layer(p, t, l, Hq, x.Q, x.K_self, x.V_self, x.O, x.LSE, x.dO, scale, x.dQ, x.dK_self,
-                                     x.dV_self, workspace, workspace_bytes, stream);
+      rc = attn_bwd_impl(p, t, l, Hq, x.rope ? x.Q_rot : x.Q, x.rope && x.K_self ? x.K_self_rot : x.K_self, x.V_self, x.O,
+                         x.LSE, x.dO, scale, x.dQ, x.dK_self, x.dV_self, workspace, workspace_bytes, stream, x.rope);
       if (rc) return rc;
     }
   }

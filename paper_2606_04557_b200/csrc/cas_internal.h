@@ -244,8 +244,15 @@ struct AttnArgs {
   void* workspace;
   size_t workspace_bytes;
   cudaStream_t stream;
+  // RoPE fused into the tensor-core kernels (cas_prefix_attn_*_rope): cos/sin table [T, 64] of cas_rope_table;
+  // forward: Q is rotated as its tile is loaded and written to Q_rot; backward: dQ leaves through the transpose
+  const float* rope_cs = nullptr;
+  int rope_layout = 0;
+  void* Q_rot = nullptr;
 };
 
+int rope_table_rotate(const void* src, void* dst, const float* cs, int64_t T, int H, int layout, int inverse,
+                      cudaStream_t st);
 int simt_attn_fwd(const AttnArgs& a);
 int simt_attn_bwd(const AttnArgs& a);
 size_t simt_bwd_workspace(const cas_slot_table* t, int Hq);

@@ -150,7 +150,107 @@ static int rope_launch(const RopeSeqs& sq, void* X, int H, int D, int layout, in
   return err == cudaSuccess ? CAS_OK : cuda_fail(err, "rope_kernel launch");
 }
 
+// ---- fused path: a cos/sin table per packed batch, shared by every head and every layer -----------------------
+// cs[t][k] = (cos, sin)(m_t * base^(-2k/D)), angles formed and reduced in double as above.  The forward kernel
+// rotates a Q tile in shared memory with it, dq_convert_kernel applies the transpose to dQ; K_self / dK_self (1/G of
+// the bytes) go through rope_table_rotate_kernel.
+__global__ void __launch_bounds__(256)
+rope_table_kernel(const __grid_constant__ RopeSeqs sq, float2* __restrict__ cs, int half) {
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int k = (int)(gid % half);
+  const int64_t tl = gid / half;
+  const int t_first = sq.seq_off[0], n_tok = sq.seq_off[sq.n] - t_first;
+  if (tl >= n_tok) return;
+  const int t = t_first + (int)tl;
+  int lo = 0, hi = sq.n - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (sq.seq_off[mid] <= t) lo = mid; else hi = mid - 1;
+  }
+  const double m = (double)(sq.pos_off[lo] + (int64_t)(t - sq.seq_off[lo]));
+  const double a = m * sq.theta[k];
+  const double r = fma(-rint(a * 0.15915494309189535), 6.283185307179586, a);
+  float s, co;
+  sincosf((float)r, &s, &co);
+  cs[(int64_t)t * half + k] = make_float2(co, s);
+}
+
+// dst[t, h, :] = R(t) src[t, h, :] (or its transpose), bf16, D = 128; one thread = one 16-byte chunk position of a
+// row (8 chunks per half): layout 0 rotates the four pairs inside each of its two chunks, layout 1 pairs chunk c of
+// the first half with chunk c of the second.
+__global__ void __launch_bounds__(256)
+rope_table_rotate_kernel(const __nv_bfloat16* __restrict__ src, __nv_bfloat16* __restrict__ dst,
+                         const float2* __restrict__ cs, int64_t n_rows, int H, int layout, int inverse) {
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int c = (int)(gid & 7);
+  const int64_t row = gid >> 3;                      // (t, h)
+  if (row >= n_rows) return;
+  const int64_t t = row / H;
+  const float2* tab = cs + t * 64;
+  float fa[8], fb[8];
+  load16(src + row * 128 + c * 8, fa);
+  load16(src + row * 128 + 64 + c * 8, fb);
+  const float sg = inverse ? -1.f : 1.f;
+  if (layout == 0) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float2 w0 = tab[4 * c + i], w1 = tab[32 + 4 * c + i];
+      const float a0 = fa[2 * i], b0 = fa[2 * i + 1], a1 = fb[2 * i], b1 = fb[2 * i + 1];
+      fa[2 * i] = a0 * w0.x - b0 * sg * w0.y;
+      fa[2 * i + 1] = a0 * sg * w0.y + b0 * w0.x;
+      fb[2 * i] = a1 * w1.x - b1 * sg * w1.y;
+      fb[2 * i + 1] = a1 * sg * w1.y + b1 * w1.x;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const float2 w = tab[8 * c + i];
+      const float a = fa[i], b = fb[i];
+      fa[i] = a * w.x - b * sg * w.y;
+      fb[i] = a * sg * w.y + b * w.x;
+    }
+  }
+  store16(dst + row * 128 + c * 8, fa);
+  store16(dst + row * 128 + 64 + c * 8, fb);
+}
+
+int rope_table_rotate(const void* src, void* dst, const float* cs, int64_t T, int H, int layout, int inverse,
+                      cudaStream_t st) {
+  const int64_t n_rows = T * H;
+  if (n_rows <= 0) return CAS_OK;
+  rope_table_rotate_kernel<<<(unsigned)((n_rows * 8 + 255) / 256), 256, 0, st>>>(
+      (const __nv_bfloat16*)src, (__nv_bfloat16*)dst, (const float2*)cs, n_rows, H, layout, inverse);
+  cudaError_t err = cudaGetLastError();
+  return err == cudaSuccess ? CAS_OK : cuda_fail(err, "rope_table_rotate_kernel launch");
+}
+
 }  // namespace cas
+
+extern "C" int cas_rope_table(int32_t B, const int32_t* seq_off, const int64_t* pos_off, int32_t D, double base,
+                              float* cs, void* stream) {
+  using namespace cas;
+  if (!seq_off || !pos_off || !cs || B < 1) { set_error("null / empty args"); return CAS_ERR_INVALID_ARG; }
+  if (!(base > 1.0)) { set_error("RoPE base must be > 1"); return CAS_ERR_INVALID_ARG; }
+  if (D < 2 || D > 256 || D % 2) { set_error("D = %d", D); return CAS_ERR_SHAPE; }
+  if (seq_off[0] != 0) { set_error("offsets must start at 0"); return CAS_ERR_INVALID_ARG; }
+  for (int b = 0; b < B; ++b) {
+    if (seq_off[b + 1] < seq_off[b]) { set_error("seq_off not monotone"); return CAS_ERR_INVALID_ARG; }
+    if (pos_off[b] < 0) { set_error("negative position offset"); return CAS_ERR_INVALID_ARG; }
+  }
+  for (int b0 = 0; b0 < B; b0 += kRopeSeqs) {
+    RopeSeqs sq;
+    for (int k = 0; k < D / 2; ++k) sq.theta[k] = pow(base, -2.0 * (double)k / (double)D);
+    sq.n = std::min(kRopeSeqs, B - b0);
+    for (int i = 0; i <= sq.n; ++i) sq.seq_off[i] = seq_off[b0 + i];
+    for (int i = 0; i < sq.n; ++i) sq.pos_off[i] = pos_off[b0 + i];
+    const int64_t n_thr = (int64_t)(sq.seq_off[sq.n] - sq.seq_off[0]) * (D / 2);
+    if (n_thr <= 0) continue;
+    rope_table_kernel<<<(unsigned)((n_thr + 255) / 256), 256, 0, (cudaStream_t)stream>>>(sq, (float2*)cs, D / 2);
+    cudaError_t err = cudaGetLastError();
+    if (err != cudaSuccess) return cuda_fail(err, "rope_table_kernel launch");
+  }
+  return CAS_OK;
+}
 
 extern "C" int cas_rope_apply(int32_t dtype, int32_t B, const int32_t* seq_off, const int64_t* pos_off, int32_t H,
                               int32_t D, double base, int32_t layout, int32_t inverse, void* X, void* stream) {

@@ -73,7 +73,8 @@ bwd_prep_kernel(const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __rest
 // dQ[t,h,:] = bf16(scale * scratch);  one warp per (t, h) row, lane = 4 columns.
 __global__ void __launch_bounds__(256)
 dq_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dQ, const int32_t* __restrict__ seq_off,
-                  const int32_t* __restrict__ qtile_off, int B, int Hq, int64_t nqt, float scale, int64_t n_rows) {
+                  const int32_t* __restrict__ qtile_off, int B, int Hq, int64_t nqt, float scale, int64_t n_rows,
+                  const float2* __restrict__ rope_cs, int rope_layout) {
   const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (w >= n_rows) return;
@@ -88,9 +89,31 @@ dq_convert_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dQ,
   const int r = row & 127, c = lane >> 3, j = lane & 7;
   const float4 v = *reinterpret_cast<const float4*>(acc + (((int64_t)h * nqt + u) * 4 + c) * 4096 + r * 32 +
                                                     ((j ^ (r & 7)) << 2));
+  float x0 = v.x * scale, x1 = v.y * scale, x2 = v.z * scale, x3 = v.w * scale;     // columns 4*lane .. 4*lane+3
+  if (rope_cs) {
+    // fused RoPE backward: dQ w.r.t. the un-rotated queries = R(t)^T dQ_rot, in fp32 before the one
+    // rounding to bf16.  The whole warp is here (a warp = one row), so the shuffles are safe.
+    const float2* tab = rope_cs + (int64_t)t * 64;
+    if (rope_layout == 0) {                       // pairs (2k, 2k+1): k = 2*lane, 2*lane+1
+      const float2 w0 = __ldg(tab + 2 * lane), w1 = __ldg(tab + 2 * lane + 1);
+      const float a0 = x0, b0 = x1, a1 = x2, b1 = x3;
+      x0 = a0 * w0.x + b0 * w0.y;  x1 = -a0 * w0.y + b0 * w0.x;
+      x2 = a1 * w1.x + b1 * w1.y;  x3 = -a1 * w1.y + b1 * w1.x;
+    } else {                                      // pairs (k, k + 64): lanes l and l + 16 hold the two halves
+      const float y0 = __shfl_xor_sync(0xffffffffu, x0, 16), y1 = __shfl_xor_sync(0xffffffffu, x1, 16);
+      const float y2 = __shfl_xor_sync(0xffffffffu, x2, 16), y3 = __shfl_xor_sync(0xffffffffu, x3, 16);
+      const int k = 4 * (lane & 15);
+      const float2 w0 = __ldg(tab + k), w1 = __ldg(tab + k + 1), w2 = __ldg(tab + k + 2), w3 = __ldg(tab + k + 3);
+      if (lane < 16) {                            // own = a, partner = b:  a' = a cos + b sin
+        x0 = x0 * w0.x + y0 * w0.y;  x1 = x1 * w1.x + y1 * w1.y;  x2 = x2 * w2.x + y2 * w2.y;  x3 = x3 * w3.x + y3 * w3.y;
+      } else {                                    // own = b, partner = a:  b' = -a sin + b cos
+        x0 = -y0 * w0.y + x0 * w0.x;  x1 = -y1 * w1.y + x1 * w1.x;  x2 = -y2 * w2.y + x2 * w2.x;  x3 = -y3 * w3.y + x3 * w3.x;
+      }
+    }
+  }
   uint2 o;
-  o.x = pack_bf16(v.x * scale, v.y * scale);
-  o.y = pack_bf16(v.z * scale, v.w * scale);
+  o.x = pack_bf16(x0, x1);
+  o.y = pack_bf16(x2, x3);
   *reinterpret_cast<uint2*>(dQ + w * 128 + lane * 4) = o;
 }
 
@@ -562,7 +585,8 @@ int tc_attn_bwd(const AttnArgs& a) {
   tc_bwd_kernel<<<grid, kBwdThreads, kBwdSmem, a.stream>>>(tmQ, tmdO, a.L->tm_K, a.L->tm_V, tmKs, tmVs, a.L->tm_K16,
                                                            a.L->tm_V16, prm, dirty);
   dq_convert_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
-      dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows);
+      dQacc, (__nv_bfloat16*)a.dQ, t->d_seq_off, t->d_qtile_off, t->B, a.Hq, (int64_t)nqt, a.scale, n_rows,
+      (const float2*)a.rope_cs, a.rope_layout);
   cudaError_t e = cudaGetLastError();
   return e == cudaSuccess ? CAS_OK : cuda_fail(e, "tc bwd launch");
 }

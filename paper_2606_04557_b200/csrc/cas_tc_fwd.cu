@@ -74,7 +74,7 @@ constexpr int kFwdThreads = 384;   // 3 warpgroups: two softmax groups + (TMA, M
 constexpr uint32_t kTile = 32768, kHalf = 16384;
 constexpr uint32_t kOffQ = 0, kOffK = 2 * kTile, kOffV = 4 * kTile, kOffBar = 6 * kTile;
 constexpr uint32_t kFwdSmem = 6 * kTile + 256 + 1024;   // + barriers + alignment slack
-enum { B_QF = 0, B_KF = 2, B_KE = 4, B_VF = 6, B_VE = 8, B_SF = 10, B_PF = 12, B_OD = 14, B_N = 15 };
+enum { B_QF = 0, B_KF = 2, B_KE = 4, B_VF = 6, B_VE = 8, B_SF = 10, B_PF = 12, B_OD = 14, B_QR = 15, B_N = 17 };
 
 struct FwdParams {
   const int32_t* seq_off;
@@ -85,6 +85,9 @@ struct FwdParams {
   __nv_bfloat16* O;
   float* LSE;
   float* part;                   // split-KV partials of the tail blocks: [tail block][part][256 rows][kFwdPartStride]
+  const float2* rope_cs;         // fused RoPE: (cos, sin) per [token][pair] or null
+  __nv_bfloat16* Q_rot;          // the rotated Q rows (the backward pass reads them)
+  int rope_layout;
   int Hq, Hkv, has_self;
   int n_blocks;                  // (item, head) blocks = items x Hq, in KV-group-major order
   int n_whole;                   // blocks [0, n_whole) run whole; each later one is cut into n_parts CTAs
@@ -138,7 +141,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
   const int n_max = nq == 2 ? nkv1 : nkv0;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < B_N; ++i) mbar_init(bar(i), (i == B_PF || i == B_PF + 1) ? 128 : 1);
+    for (int i = 0; i < B_N; ++i) mbar_init(bar(i), (i == B_PF || i == B_PF + 1 || i == B_QR || i == B_QR + 1) ? 128 : 1);
     fence_mbar_init();
   }
   if (warp == 8) {
@@ -215,8 +218,9 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
           mma_ts(tbase + 256 + t * 128, tbase + t * 128 + kk * 8, desc_mnmajor(va + kk * 2048, kHalf), idesc_pv,
                  (j > 0 || kk > 0) ? 1u : 0u);
       };
-      mbar_wait(bar(B_QF), 0);
-      if (nq == 2) mbar_wait(bar(B_QF + 1), 0);
+      // with fused RoPE the softmax warpgroups rotate the Q tiles in shared memory first
+      mbar_wait(bar(prm.rope_cs ? B_QR : B_QF), 0);
+      if (nq == 2) mbar_wait(bar((prm.rope_cs ? B_QR : B_QF) + 1), 0);
       mbar_wait(bar(B_KF), 0);
       tc_fence_after();
       issue_qk(0, 0);
@@ -269,6 +273,74 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
       const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
       const uint32_t tS = tbase + t * 128 + lane_base, tO = tbase + 256 + t * 128 + lane_base;
       const int nkv = t == 0 ? nkv0 : nkv1;
+      if (prm.rope_cs) {
+        // FUSED RoPE: thread = query row.  The row's 16-byte chunk c of half hh sits at chunk position
+        // c ^ (r & 7) of its 128-byte line (TMA 128B swizzle); rotate in place for the MMAs and write the rotated row
+        // to Q_rot for the backward pass (each (row, head) belongs to one block; of a split block, part 0 writes).
+        // the cos/sin of chunk c+1 are fetched (four 16-byte loads, L2) while chunk c is rotated, those of chunk 0
+        // before the Q tile has even arrived: the rotation sits in front of the block's first MMA
+        const bool live = row < lq;
+        const float4* tab4 = reinterpret_cast<const float4*>(prm.rope_cs + (int64_t)(t0 + (live ? row : 0)) * 64);
+        const int lay = prm.rope_layout;
+        auto fetch = [&](int c, float4 (&w)[4]) {       // layout 0: pairs 4c..4c+3 and 32+4c..; layout 1: pairs 8c..8c+7
+          const int i0 = lay == 0 ? 2 * c : 4 * c, i1 = lay == 0 ? 16 + 2 * c : 4 * c + 2;
+          w[0] = __ldg(tab4 + i0); w[1] = __ldg(tab4 + i0 + 1); w[2] = __ldg(tab4 + i1); w[3] = __ldg(tab4 + i1 + 1);
+        };
+        float4 wn[4];
+        fetch(0, wn);
+        mbar_wait(bar(B_QF + t), 0);
+        if (live) {
+          __nv_bfloat16* qrow = prm.Q_rot + ((int64_t)(t0 + row) * prm.Hq + h) * 128;
+          const uint32_t qb = sbase + kOffQ + t * kTile + r * 128;
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            const float4 w4[4] = {wn[0], wn[1], wn[2], wn[3]};
+            if (c < 7) fetch(c + 1, wn);
+            const float2 w[8] = {{w4[0].x, w4[0].y}, {w4[0].z, w4[0].w}, {w4[1].x, w4[1].y}, {w4[1].z, w4[1].w},
+                                 {w4[2].x, w4[2].y}, {w4[2].z, w4[2].w}, {w4[3].x, w4[3].y}, {w4[3].z, w4[3].w}};
+            const uint32_t pos = (uint32_t)((c ^ (r & 7)) << 4);
+            uint32_t ua[4], ub[4];
+            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(ua[0]), "=r"(ua[1]), "=r"(ua[2]), "=r"(ua[3]) : "r"(qb + pos));
+            asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(ub[0]), "=r"(ub[1]), "=r"(ub[2]), "=r"(ub[3]) : "r"(qb + kHalf + pos));
+            float fa[8], fb[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ua[i]));
+              const float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&ub[i]));
+              fa[2 * i] = x.x; fa[2 * i + 1] = x.y; fb[2 * i] = y.x; fb[2 * i + 1] = y.y;
+            }
+            if (lay == 0) {                        // pairs (2k, 2k+1): four inside each chunk (w[0..3]: first half)
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float2 w0 = w[i], w1 = w[4 + i];
+                const float a0 = fa[2 * i], b0 = fa[2 * i + 1], a1 = fb[2 * i], b1 = fb[2 * i + 1];
+                fa[2 * i] = a0 * w0.x - b0 * w0.y;  fa[2 * i + 1] = a0 * w0.y + b0 * w0.x;
+                fb[2 * i] = a1 * w1.x - b1 * w1.y;  fb[2 * i + 1] = a1 * w1.y + b1 * w1.x;
+              }
+            } else {                               // pairs (k, k + 64): chunk c of both halves
+#pragma unroll
+              for (int i = 0; i < 8; ++i) {
+                const float a = fa[i], b = fb[i];
+                fa[i] = a * w[i].x - b * w[i].y;
+                fb[i] = a * w[i].y + b * w[i].x;
+              }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              ua[i] = pack_bf16(fa[2 * i], fa[2 * i + 1]);
+              ub[i] = pack_bf16(fb[2 * i], fb[2 * i + 1]);
+            }
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(qb + pos), "r"(ua[0]), "r"(ua[1]), "r"(ua[2]), "r"(ua[3]) : "memory");
+            asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(qb + kHalf + pos), "r"(ub[0]), "r"(ub[1]), "r"(ub[2]), "r"(ub[3]) : "memory");
+            if (part == 0) {
+              *reinterpret_cast<uint4*>(qrow + 8 * c) = make_uint4(ua[0], ua[1], ua[2], ua[3]);
+              *reinterpret_cast<uint4*>(qrow + 64 + 8 * c) = make_uint4(ub[0], ub[1], ub[2], ub[3]);
+            }
+          }
+        }
+        fence_proxy_async();
+        mbar_arrive(bar(B_QR + t));
+      }
       float m = -INFINITY, l = 0.f;
       for (int j = 0; j < nkv; ++j) {
         int limit;
@@ -526,7 +598,8 @@ int tc_attn_fwd(const AttnArgs& a) {
     part = (float*)pm->fwd_part;
   }
   FwdParams prm{t->d_seq_off, t->d_kv_tile_off, t->d_kv_tiles, t->d_ptiles, items, (__nv_bfloat16*)a.O_out, a.LSE_out,
-                part, a.Hq, a.Hkv, has_self, n_blocks, n_blocks - n_tail, n_parts, a.scale * 1.4426950408889634f};
+                part, (const float2*)a.rope_cs, (__nv_bfloat16*)a.Q_rot, a.rope_layout,
+                a.Hq, a.Hkv, has_self, n_blocks, n_blocks - n_tail, n_parts, a.scale * 1.4426950408889634f};
   const unsigned grid = (unsigned)(n_blocks - n_tail + n_tail * n_parts);
   tc_fwd_kernel<<<grid, kFwdThreads, kFwdSmem, a.stream>>>(tmQ, a.L->tm_K, a.L->tm_V, tmKs, tmVs, a.L->tm_K16, a.L->tm_V16, prm);
   cudaError_t e = cudaGetLastError();
