@@ -4,14 +4,22 @@
 One "step" = one pass of the whole hot path over one batch of BASELINE.json configs[1]
 (c2, bf16 3B-like layer): slot-table build (host) -> prefix-attention forward -> backward (dK/dV
 scatter-accumulated into the cartridge gradient slots) -> fused Adam over the resident cartridges.
-(c2 has no rotation; `--config c3` adds the plan + swap-out/in overlapped on the side stream.)
+(c2 has no rotation; c3 adds the plan + swap-out/in overlapped on the side streams.)
 
 metric  = prefix-attn fwd+bwd TFLOP/s: algorithmic FLOPs 14*D*Hq*pairs (visible pairs only,
           DESIGN.md "Algorithmic work") divided by the time of the WHOLE step (Adam included).
-roofline= the dominant kernel (attention backward) against the measured bf16 peak.
-e2e     = the same metric through cas_train_step_host(): pinned HOST buffers, H2D of Q/K_self/V_self/dO
-          and D2H of O/LSE/dQ inside the timed region.
+roofline= the dominant kernel (attention backward) against the measured bf16 peak: the BURST figure when the
+          timed region is shorter than a second, the sustained one otherwise (decode configs: HBM).
+e2e     = the same metric through cas_train_step_host_async(): pinned HOST buffers, H2D of Q/K_self/V_self/dO
+          and D2H of O/LSE/dQ/dK_self/dV_self of every step inside the timed region, steps pipelined over two
+          device buffer sets, cas_train_step_host_wait before the clock stops; the per-call-complete variant
+          (cas_train_step_host) is reported beside it.
 cpu_baseline = the oracle (numpy fp64, as it stands) timed on a bounded sample of the same workload.
+
+The default run (`python bench.py`, about two minutes) prints ONE JSON line: c2 is the headline; `sustained` is a
+>= 3 s loop of the same steps with its own clock samples; `extra` carries one compact record each for c3 (with and
+without rotation, swap alone against the host-link peak measured in the same run), c4, c5 "all loaded", c5 top-8
+and c_pages.  `--no-extra` gives the headline config only; `--config X` benches another config as the headline.
 
 `--impl reference` times the oracle alone (this tier has no reference implementation to install).
 Multi-GPU: replicas only -- every rank runs its own batch on its own pool,
