@@ -33,6 +33,7 @@
 #include <algorithm>
 #include <cstring>
 #include <map>
+#include <type_traits>
 
 #include "cas_sm100.cuh"
 #include "cas_tc_common.cuh"
@@ -657,26 +658,33 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
           if (c > 0) tc_wait_st();
           if (c < 3) tmem_ld32(tS + 32 * (c + 1), buf[(c + 1) & 1]);
           uint32_t* s = buf[c & 1];
+          // the masked form is a separate copy of the loop: selects inside the common one cost the full tiles (all of
+          // c5) a third of their exp phase
+          auto exp_chunk = [&](auto masked_tag) {
+            constexpr bool kMasked = decltype(masked_tag)::value;
 #pragma unroll
-          for (int i = 0; i < 16; i += 2) {
-            float a0, a1, b0, b1;
-            unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
-            unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
-            a0 = ex2_approx(a0); a1 = ex2_approx(a1);
-            if ((i & 6) != 6) exp2_poly2(b0, b1, b0, b1);    // 3 of every 8 scores on the FMA pipe
-            else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
-            if (ragged) {
-              // a masked key weighs EXACTLY 0 (its raw score may be anything; its V row may be a stale cache row)
-              a0 = (mw[c] >> (2 * i)) & 1u ? a0 : 0.f;
-              a1 = (mw[c] >> (2 * i + 1)) & 1u ? a1 : 0.f;
-              b0 = (mw[c] >> (2 * i + 2)) & 1u ? b0 : 0.f;
-              b1 = (mw[c] >> (2 * i + 3)) & 1u ? b1 : 0.f;
+            for (int i = 0; i < 16; i += 2) {
+              float a0, a1, b0, b1;
+              unpack2(fma2(pack2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), sc2, nm2), a0, a1);
+              unpack2(fma2(pack2(__uint_as_float(s[2 * i + 2]), __uint_as_float(s[2 * i + 3])), sc2, nm2), b0, b1);
+              a0 = ex2_approx(a0); a1 = ex2_approx(a1);
+              if ((i & 6) != 6) exp2_poly2(b0, b1, b0, b1);    // 3 of every 8 scores on the FMA pipe
+              else { b0 = ex2_approx(b0); b1 = ex2_approx(b1); }
+              if (kMasked) {
+                // a masked key weighs EXACTLY 0 (its raw score may be anything; its V row may be a stale cache row)
+                a0 = (mw[c] >> (2 * i)) & 1u ? a0 : 0.f;
+                a1 = (mw[c] >> (2 * i + 1)) & 1u ? a1 : 0.f;
+                b0 = (mw[c] >> (2 * i + 2)) & 1u ? b0 : 0.f;
+                b1 = (mw[c] >> (2 * i + 3)) & 1u ? b1 : 0.f;
+              }
+              sum2a = add2(sum2a, pack2(a0, a1));
+              sum2b = add2(sum2b, pack2(b0, b1));
+              s[i] = pack_bf16(a0, a1);
+              s[i + 1] = pack_bf16(b0, b1);
             }
-            sum2a = add2(sum2a, pack2(a0, a1));
-            sum2b = add2(sum2b, pack2(b0, b1));
-            s[i] = pack_bf16(a0, a1);
-            s[i + 1] = pack_bf16(b0, b1);
-          }
+          };
+          if (ragged) exp_chunk(std::true_type{});
+          else exp_chunk(std::false_type{});
           tmem_st16(tS + 16 * c, s);                         // P of keys [32c, 32c+32) -> columns [16c, 16c+16)
         }
         {
