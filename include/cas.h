@@ -352,6 +352,24 @@ int cas_prefix_attn_bwd_layer(cas_pool* pool, const cas_slot_table* table, int32
 int cas_decode_attn_layer(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq, const void* Q,
                           const void* K_cache, const void* V_cache, int32_t cache_cap, const int32_t* self_len,
                           float scale, void* O, float* LSE, void* stream);
+/* ---- a forward call that allocates nothing ---------------------------------------------------------------
+ * cas_prefix_attn_fwd_layer for callers that may not call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  cas_prefix_attn_fwd keeps the split-KV partials of its tail blocks
+ * (cas_slot_table_fwd_split) in a pool-owned buffer that it allocates, and may grow, inside a call; this variant keeps
+ * them in a file-scope device array of the library instead -- 148 split CTAs x 256 rows x 132 floats = 20,004,864
+ * bytes, held by every GPU that loads the library until the process exits -- and calls no cudaMalloc / cudaFree or
+ * allocating library routine (the first forward call on a table plans the split with a few small host-heap vectors;
+ * later calls reuse the plan).  Same arguments, same kernels, same result bits as cas_prefix_attn_fwd_layer.
+ * Errors: CAS_ERR_SHAPE unless the tensor-core training kernel serves the call (bf16, D = 128, some sequence with
+ * more than one query token); CAS_ERR_CAPACITY when the table's split needs more than 148 split CTAs (it never does
+ * on a GPU with <= 148 SMs).  ALL calls on a device share the one array, which keeps the last call's contents
+ * (nothing in it has to start at zero: a call reads only the partial rows its own CTAs wrote): calls of this entry
+ * point that overlap on the GPU -- two streams, two pools, two host threads -- race; order them on one stream or
+ * with events.  Asynchronous on `stream`. */
+int cas_prefix_attn_fwd_noalloc(cas_pool* pool, const cas_slot_table* table, int32_t layer, int32_t Hq,
+                                const void* Q, const void* K_self, const void* V_self, float scale, void* O,
+                                float* LSE, void* stream);
+
 /* ---- RoPE fused into the attention calls (PAPER.md:77 the offset is "recomputed at each
  * step") -----------------------------------------------------------------------------------------------------
  * cas_rope_table writes, once per packed batch (it serves every head and every layer), cs[t][k] = (cos, sin) of

@@ -339,6 +339,13 @@ def cas_prefix_attn_bwd_rope(pool: Pool, tab: SlotTable, Hq: int, Q_rot, Ks_rot,
                                           C.c_size_t(workspace.numel() * workspace.element_size()), _stream(stream)))
 
 
+def cas_prefix_attn_fwd_noalloc(pool: Pool, tab: SlotTable, Hq: int, Q, Ks, Vs, scale: float, O, LSE, stream=None,
+                                layer: int = 0):
+    _check(lib().cas_prefix_attn_fwd_noalloc(pool.handle, tab.handle, C.c_int32(layer), C.c_int32(Hq), _dptr(Q),
+                                             _dptr(Ks), _dptr(Vs), C.c_float(scale), _dptr(O), _dptr(LSE),
+                                             _stream(stream)))
+
+
 class LayerIO(C.Structure):
     _fields_ = [("Q", C.c_void_p), ("K_self", C.c_void_p), ("V_self", C.c_void_p), ("dO", C.c_void_p),
                 ("O", C.c_void_p), ("LSE", C.c_void_p), ("dQ", C.c_void_p), ("dK_self", C.c_void_p),

@@ -764,6 +764,30 @@ int cas_prefix_attn_fwd_layer(cas_pool* p, const cas_slot_table* t, int32_t laye
   return attn_fwd_impl(p, t, layer, Hq, Q, Ks, Vs, scale, O, LSE, stream, nullptr, nullptr, nullptr);
 }
 
+int cas_prefix_attn_fwd_noalloc(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
+                                const void* Ks, const void* Vs, float scale, void* O, float* LSE, void* stream) {
+  int rc = check_attn(p, t, Hq, Ks, Vs, scale);
+  if (rc) return rc;
+  if (layer < 0 || layer >= p->n_layers) { set_error("layer %d out of range", layer); return CAS_ERR_INVALID_ARG; }
+  if (!Q || !O || !LSE) { set_error("null Q/O/LSE"); return CAS_ERR_INVALID_ARG; }
+  // only the tensor-core training kernel: the decode kernel allocates its work list and scratch at a table's first
+  // call, and the CUDA-core path has no scratch to place
+  if (!use_tc(p, t, Hq, &rc) || rc || tc_decode_supported(p, t, Hq)) {
+    if (rc) return rc;
+    set_error("cas_prefix_attn_fwd_noalloc runs the tensor-core forward kernel (bf16, D = 128, not decode-shaped)");
+    return CAS_ERR_SHAPE;
+  }
+  rc = table_on_stream(t, stream);
+  if (rc) return rc;
+  AttnArgs a{};
+  a.pool = p; a.tab = t; a.Hq = Hq; a.Hkv = p->desc.Hkv; a.D = p->desc.D; a.dtype = p->desc.dtype;
+  a.Q = Q; a.Ks = Ks; a.Vs = Vs; a.O_out = O; a.LSE_out = LSE; a.scale = scale;
+  a.stream = (cudaStream_t)stream;
+  a.layer = layer; a.L = &p->layers[layer];
+  a.static_scratch = true;
+  return tc_attn_fwd(a);
+}
+
 int cas_prefix_attn_fwd_rope(cas_pool* p, const cas_slot_table* t, int32_t layer, int32_t Hq, const void* Q,
                              const void* Ks, const void* Vs, const cas_rope* rope, void* Q_rot, void* Ks_rot,
                              float scale, void* O, float* LSE, void* stream) {

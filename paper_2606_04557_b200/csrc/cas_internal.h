@@ -249,6 +249,7 @@ struct AttnArgs {
   const float* rope_cs = nullptr;
   int rope_layout = 0;
   void* Q_rot = nullptr;
+  bool static_scratch = false;   // cas_prefix_attn_fwd_noalloc: split-KV partials in the library's static device array
 };
 
 int rope_table_rotate(const void* src, void* dst, const float* cs, int64_t T, int H, int layout, int inverse,

@@ -18,6 +18,7 @@
 #include "cas_tc_common.cuh"
 #include <algorithm>
 #include <cstdlib>
+#include <mutex>
 #include <vector>
 
 namespace cas {
@@ -551,6 +552,34 @@ static void plan_tail_split(const cas_slot_table* t, int Hq, int Hkv, bool has_s
   *n_parts = parts;
 }
 
+// ---- cas_prefix_attn_fwd_noalloc: the tail blocks' split-KV partials in a file-scope device array --------------
+// For callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  Every GPU
+// that loads the library holds these 20,004,864 bytes until exit.  In host code the array's NAME is a host-side
+// stand-in, not a device address: the kernels get the address cudaGetSymbolAddress returns, looked up once per device
+// with that device current.  All calls share the array (calls that overlap on the GPU race); nothing in it has to
+// start at zero: a call reads only the partial rows its own CTAs have written.
+constexpr int kNoAllocPartBlocks = 148;      // split CTAs (tail blocks x parts) one call may use
+static __device__ __align__(256) float g_fwd_part_static[(size_t)kNoAllocPartBlocks * 256 * kFwdPartStride];
+
+static int fwd_static_scratch(float** out) {
+  constexpr int kMaxDev = 64;
+  static float* addr[kMaxDev] = {};
+  static std::mutex mu;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  if (dev < 0 || dev >= kMaxDev) { set_error("device ordinal %d not supported by the static scratch", dev); return CAS_ERR_INVALID_ARG; }
+  std::lock_guard<std::mutex> lk(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_fwd_part_static);      // the address on the CURRENT device
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_fwd_part_static)");
+    addr[dev] = (float*)p;
+  }
+  *out = addr[dev];
+  return CAS_OK;
+}
+
 int tc_attn_fwd(const AttnArgs& a) {
   const cas_slot_table* t = a.tab;
   const FwdItem* items = t->d_fwd_items;
@@ -579,7 +608,16 @@ int tc_attn_fwd(const AttnArgs& a) {
   }
   const int n_blocks = (int)(n_items * a.Hq), n_tail = t->fwd_n_tail, n_parts = t->fwd_n_parts;
   float* part = nullptr;
-  if (n_tail) {
+  if (n_tail && a.static_scratch) {
+    if (n_tail * n_parts > kNoAllocPartBlocks) {
+      set_error("cas_prefix_attn_fwd_noalloc: this table splits %d tail blocks into %d parts = %d split CTAs; the static "
+                "scratch holds %d (%zu bytes): use cas_prefix_attn_fwd", n_tail, n_parts, n_tail * n_parts,
+                kNoAllocPartBlocks, sizeof(float) * kNoAllocPartBlocks * 256 * kFwdPartStride);
+      return CAS_ERR_CAPACITY;
+    }
+    rc = fwd_static_scratch(&part);
+    if (rc) return rc;
+  } else if (n_tail) {
     // pool-owned, grow-only: forward calls on one pool are ordered by the caller's stream (cas.h)
     const size_t need = (size_t)n_tail * n_parts * 256 * kFwdPartStride * sizeof(float);
     cas_pool* pm = const_cast<cas_pool*>(a.pool);
