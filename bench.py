@@ -463,6 +463,7 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
         # fwd (+ fwd_combine when the tail is split), bwd_prep, bwd, dq_convert, adam  /  decode (+ decode_combine)
         fwd_split = tc and cas.cas_slot_table_fwd_split(sess.tab)[0] > 0
         n_launch = (5 + int(fwd_split)) if cfg.backward else (1 if sess.tab.B * cfg.Hq <= 256 else 2)
+        adam_dram = load_traffic().get(cfg_name, {}).get("adam") if cfg.backward else None
         line = {
             "metric": METRIC, "value": total_flops / (ms_step_max * 1e-3) / 1e12, "unit": UNIT,
             "n_gpus": world, "steps": steps, "warmup": max(warmup, 3), "ms_per_step": ms_step_max,
@@ -485,9 +486,14 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
                           "fwd_bwd_frac_of_bf16_burst_peak": (fwd_fl + bwd_fl) / ((t_fwd + t_bwd) * 1e-3) / 1e12 / peaks["bf16"],
                           "adam_gbs": (adam_bytes / (t_adam * 1e-3) / 1e9) if cfg.backward else None,
                           "adam_frac_of_hbm_peak": (adam_bytes / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if cfg.backward else None,
+                          # the same launch against its REAL DRAM traffic (ncu dram__bytes_read + write of the committed
+                          # capture): the fraction that is a bound -- the algorithmic one above can exceed 1
+                          "adam_dram_bytes": adam_dram,
+                          "adam_dram_gbs": (adam_dram / (t_adam * 1e-3) / 1e9) if adam_dram else None,
+                          "adam_frac_of_hbm_peak_dram": (adam_dram / (t_adam * 1e-3) / 1e9 / peaks["hbm"]) if adam_dram else None,
                           "adam_note": ("algorithmic 30/26 B per element; a fraction above 1 means part of it is served by "
-                                        "L2 (gradient rows the backward pass has just written): see roofline traffic in "
-                                        "profiles/") if cfg.backward else None},
+                                        "L2 (gradient rows the backward pass has just written): adam_dram_* use the DRAM "
+                                        "bytes of the ncu capture in profiles/") if cfg.backward else None},
             "roofline": roof,
             "gpu_launches": steps * (n_launch + (cfg.rotate_in if rotate else 0)),
             "clocks": clocks,

@@ -37,33 +37,61 @@ constexpr float kLog2e = 1.4426950408889634f;
 
 // delta[t,h] = sum_d dO*O (B1), stored head-major and padded per sequence to whole 128-row tiles
 // (so each (head, Q tile) is one aligned 512-byte run): auxD[h][tile*128 + r] = -delta; auxL = -LSE*log2(e).
+// The same pass ZEROES the fp32 dQ scratch row of every (t, h) (no separate 100 MB memset launch) and the padding
+// entries of auxL / auxD behind the last token of every sequence (they are multiplied by masked zeros in the main
+// kernel and must be finite).  Eight lanes per (t, h) row, 16 columns = two 16-byte loads per tensor and lane: a
+// warp covers four consecutive rows = 1 KB contiguous of O and of dO.
 __global__ void __launch_bounds__(256)
 bwd_prep_kernel(const __nv_bfloat16* __restrict__ O, const __nv_bfloat16* __restrict__ dO,
                 const float* __restrict__ LSE, const int32_t* __restrict__ seq_off,
                 const int32_t* __restrict__ qtile_off, int B, int Hq, int64_t aux_stride,
-                float* __restrict__ auxL, float* __restrict__ auxD, int64_t n_rows) {
-  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;   // (t, h) row
-  const int lane = threadIdx.x & 31;
-  if (w >= n_rows) return;
-  const int t = (int)(w / Hq), h = (int)(w % Hq);
-  const uint2 a = *reinterpret_cast<const uint2*>(O + w * 128 + lane * 4);
-  const uint2 b = *reinterpret_cast<const uint2*>(dO + w * 128 + lane * 4);
-  const float2 a0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&a.x));
-  const float2 a1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&a.y));
-  const float2 b0 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&b.x));
-  const float2 b1 = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&b.y));
-  float s = a0.x * b0.x + a0.y * b0.y + a1.x * b1.x + a1.y * b1.y;
+                float* __restrict__ auxL, float* __restrict__ auxD, float* __restrict__ dQacc, int64_t n_rows) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 3;   // (t, h) row
+  const int sub = threadIdx.x & 7;
+  const bool live = w < n_rows;
+  const int64_t wr = live ? w : 0;
+  const int t = (int)(wr / Hq), h = (int)(wr % Hq);
+  const uint4* po = reinterpret_cast<const uint4*>(O + wr * 128 + sub * 16);
+  const uint4* pd = reinterpret_cast<const uint4*>(dO + wr * 128 + sub * 16);
+  const uint4 a0 = po[0], a1 = po[1], b0 = pd[0], b1 = pd[1];
+  const uint32_t av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+  const uint32_t bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+  float s = 0.f;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  if (lane == 0) {
-    int lo = 0, hi = B - 1;                      // sequence of token t
-    while (lo < hi) {
-      const int mid = (lo + hi + 1) >> 1;
-      if (seq_off[mid] <= t) lo = mid; else hi = mid - 1;
-    }
-    const int64_t pos = (int64_t)h * aux_stride + (int64_t)qtile_off[lo] * 128 + (t - seq_off[lo]);
+  for (int i = 0; i < 8; ++i) {
+    const float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&av[i]));
+    const float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&bv[i]));
+    s += x.x * y.x + x.y * y.y;
+  }
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (!live) return;
+  int lo = 0, hi = B - 1;                        // sequence of token t
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (seq_off[mid] <= t) lo = mid; else hi = mid - 1;
+  }
+  const int row = t - seq_off[lo];
+  const int64_t u = qtile_off[lo] + (row >> 7);
+  const int r = row & 127;
+  // this row's 512 bytes of the dQ scratch: quarter c = sub >> 1 holds 128 bytes of it, this lane zeroes one half
+  {
+    float4* z = reinterpret_cast<float4*>(dQacc + (((int64_t)h * (aux_stride >> 7) + u) * 4 + (sub >> 1)) * 4096 + r * 32 +
+                                          (sub & 1) * 16);
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    z[0] = zero; z[1] = zero; z[2] = zero; z[3] = zero;
+  }
+  const int64_t pos = (int64_t)h * aux_stride + u * 128 + r;
+  if (sub == 0) {
     auxD[pos] = -s;                    // negated: the main kernel adds them with packed FADD2 / FFMA2
-    auxL[pos] = -LSE[w] * kLog2e;
+    auxL[pos] = -LSE[wr] * kLog2e;
+  }
+  // the last token of a sequence also clears the padding of its last tile (<= 127 entries per head)
+  if (t + 1 == seq_off[lo + 1]) {
+    for (int x = r + 1 + sub; x < 128; x += 8) {
+      auxD[pos - r + x] = 0.f;
+      auxL[pos - r + x] = 0.f;
+    }
   }
 }
 
@@ -553,11 +581,12 @@ int tc_attn_bwd(const AttnArgs& a) {
   float* dQacc = (float*)ws;
   float* auxL = (float*)(ws + b_acc);
   float* auxD = (float*)(ws + b_acc + b_aux);
-  CAS_CUDA(cudaMemsetAsync(ws, 0, b_acc + 2 * b_aux, a.stream));
+  // no memset: bwd_prep_kernel zeroes the dQ scratch rows of every real (t, h) and the aux padding; the scratch rows of
+  // padding tokens are only ever added to (masked zeros) and never read
   const int64_t n_rows = (int64_t)t->T * a.Hq;
-  bwd_prep_kernel<<<(unsigned)((n_rows * 32 + 255) / 256), 256, 0, a.stream>>>(
+  bwd_prep_kernel<<<(unsigned)((n_rows * 8 + 255) / 256), 256, 0, a.stream>>>(
       (const __nv_bfloat16*)a.O, (const __nv_bfloat16*)a.dO, a.LSE_in, t->d_seq_off, t->d_qtile_off, t->B, a.Hq,
-      (int64_t)nqt * 128, auxL, auxD, n_rows);
+      (int64_t)nqt * 128, auxL, auxD, dQacc, n_rows);
   CUtensorMap tmQ, tmdO, tmKs, tmVs;
   int rc = make_thd_map(&tmQ, a.Q, t->T, a.Hq, 128);
   if (rc) return rc;
