@@ -645,6 +645,7 @@ tc_decode_kernel(const __grid_constant__ CUtensorMap tmK, const __grid_constant_
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
             tmem_st32(tOw + cc * 32, o);
+            tc_wait_st();                            // the store has read o[] before the next chunk's load reuses it
           }
         }
         const uint64_t sc2 = pack2(prm.scale_log2, prm.scale_log2), nm2 = pack2(-m, -m);

@@ -398,6 +398,7 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
 #pragma unroll
             for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * f);
             tmem_st32(tO + c * 32, o);
+            tc_wait_st();                            // the store has read o[] before the next chunk's load reuses it
           }
         }
         // p = 2^(s*scale_log2 - m): one packed FFMA per two scores, one MUFU each, packed row sum
