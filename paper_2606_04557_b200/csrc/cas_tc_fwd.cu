@@ -236,14 +236,13 @@ tc_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ C
         const bool act0 = j < nkv0, act1 = nq == 2;
         const bool nxt0 = j + 1 < nkv0, nxt1 = nq == 2 && j + 1 < n_max;
         mbar_wait(bar(B_VF + s), (j >> 1) & 1);
+        // K(j+1) is waited for HERE, before P0(j): every mbarrier wait of this thread costs ~250 clk even when the
+        // phase is long complete, and this one would otherwise sit between PV0(j) and QK0(j+1) on tile 0's chain
+        if (nxt0 || nxt1) mbar_wait(bar(B_KF + ((j + 1) & 1)), ((j + 1) >> 1) & 1);
         if (act0) {
           mbar_wait(bar(B_PF), j & 1);
           tc_fence_after();
           issue_pv(0, j);
-        }
-        if (nxt0 || nxt1) {
-          mbar_wait(bar(B_KF + ((j + 1) & 1)), ((j + 1) >> 1) & 1);
-          tc_fence_after();
         }
         if (nxt0) {
           issue_qk(0, j + 1);
