@@ -256,7 +256,7 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
     rotate = cfg.rotate_in > 0 and not no_swap
     rot = {"step": 0, "rng": np.random.Generator(np.random.PCG64(BASE_SEED + 1000 + rank)), "bytes": 0}
     if cfg.rotate_in > 0:
-        from workloads.generate import draw_batch_selection
+        from workloads.generate import draw_batch_selection, draw_batch_selection_uniform
 
     def prepare():
         tau = rot["step"]
@@ -267,8 +267,13 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
             # K4 step protocol: draw among resident+stable cartridges, protect them, plan, swap on
             # the side stream while fwd/bwd/Adam run on the main stream, commit.
             c = cas.cas_pool_counters(sess.pool)
-            stable = [i for i in range(cfg.n_carts) if c["slot_of"][i] >= 0 and not c["in_transit"][i]]
-            sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable, wl.cart_len)
+            stable = np.nonzero((c["slot_of"] >= 0) & (c["in_transit"] == 0))[0]
+            if cfg.selection == "uniform" and cfg.n_dist != -2:
+                # the same recipe drawn for the whole batch at once: per-sequence Generator.choice calls cost more
+                # host time than a c_pages step costs on the GPU
+                sel_off, sel_cart = draw_batch_selection_uniform(cfg, rot["rng"], stable)
+            else:
+                sel_off, sel_cart = draw_batch_selection(cfg, rot["rng"], stable.tolist(), wl.cart_len)
         rot["sel"] = (sel_off, sel_cart)
         if cfg.backward or tau == 0:
             # training: a new batch and a new slot table every step.  Decode (c5): the selection is fixed while
@@ -276,7 +281,7 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
             sess.tab.close()
             sess.tab = cas.cas_slot_table_build(sess.pool, wl.seq_off, sel_off, sel_cart, tau)
         if rotate:
-            prot = sorted(set(int(x) for x in sel_cart))
+            prot = np.unique(sel_cart).tolist()
             man, n = cas.cas_plan_rotation(sess.pool, tau, cfg.rotate_in, cfg.rotate_out, prot, 260604)
             cas.cas_swap_out(sess.pool, man, n, tau, after_stream=stream)
             cas.cas_swap_in(sess.pool, man, n, tau)
@@ -287,10 +292,11 @@ def run_config(args, cfg_name, steps, warmup, rank, world, local_rank, do_e2e, d
         if cfg.backward:
             # Adam updates every resident cartridge that is not in transit this step (K4); algorithmic bytes: 30 B per
             # element of a slot that holds gradients, 26 B per element of a clean one
-            used = set(int(x) for x in sel_cart)
-            el = lambda c: 2 * int(wl.cart_len[c]) * cfg.Hkv * cfg.D
-            upd = [c for c in (stable if cfg.rotate_in > 0 else range(cfg.n_slots)) if c not in leaving]
-            adam_acc["bytes"] += sum((30 if c in used else 26) * el(c) for c in upd)
+            upd = np.asarray(stable if cfg.rotate_in > 0 else np.arange(cfg.n_slots), dtype=np.int64)
+            if leaving:
+                upd = upd[~np.isin(upd, np.fromiter(leaving, dtype=np.int64))]
+            per_el = np.where(np.isin(upd, sel_cart), 30, 26)
+            adam_acc["bytes"] += int((per_el * 2 * wl.cart_len[upd].astype(np.int64) * cfg.Hkv * cfg.D).sum())
             adam_acc["steps"] += 1
 
     def finish():

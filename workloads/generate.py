@@ -131,6 +131,32 @@ def draw_batch_selection(cfg: CasConfig, rng: np.random.Generator, candidates: S
     return np.asarray(sel_off, dtype=np.int32), np.asarray(sel, dtype=np.int32)
 
 
+def draw_batch_selection_uniform(cfg: CasConfig, rng: np.random.Generator, candidates: np.ndarray):
+    """The "uniform" recipe of draw_batch_selection for a whole batch in a few array operations (same
+    distribution: per sequence a target and n_dist distinct distractors, uniform without replacement, in draw
+    order; another random stream).  For drivers that draw a fresh batch every step among the currently resident
+    cartridges (bench.py's rotation configs), where 32 calls of Generator.choice cost more host time than the step
+    costs on the GPU.  Holds no method arithmetic."""
+    assert cfg.selection == "uniform" and cfg.n_dist != -2
+    cand = np.asarray(candidates, dtype=np.int32)
+    n = len(cand)
+    if cfg.n_dist == -1:
+        nd = rng.integers(0, cfg.n_dist_max + 1, size=cfg.B)
+    else:
+        nd = np.full(cfg.B, cfg.n_dist, dtype=np.int64)
+    k = np.minimum(1 + nd, n).astype(np.int64)
+    kmax = int(k.max())
+    # the first kmax entries of a uniform random permutation of the candidates, per sequence: smallest random keys
+    keys = rng.random((cfg.B, n))
+    first = np.argpartition(keys, kmax - 1, axis=1)[:, :kmax] if kmax < n else np.argsort(keys, axis=1)
+    order = np.take_along_axis(keys, first, axis=1).argsort(axis=1)
+    first = np.take_along_axis(first, order, axis=1)                  # draw order = ascending key
+    sel_off = np.zeros(cfg.B + 1, dtype=np.int32)
+    np.cumsum(k, out=sel_off[1:])
+    mask = np.arange(kmax)[None, :] < k[:, None]
+    return sel_off, cand[first[mask]].astype(np.int32)
+
+
 def draw_query_block(cfg: CasConfig, rng: np.random.Generator, seq_off: np.ndarray,
                      with_dO: bool = True):
     """Q ~ N(0,1); self K/V ~ N(0, kv_std); dO ~ N(0,1)."""
