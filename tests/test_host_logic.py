@@ -247,3 +247,36 @@ def test_select_retrieved_bit_exact_against_oracle():
     with pytest.raises(cas.CasError) as e:
         cas.cas_select_retrieved([3], [0, 1], 2)
     assert e.value.name == "CAS_ERR_INVALID_ARG"
+
+
+def test_batch_sampler_for_the_bench_keeps_the_uniform_recipe():
+    """workloads.generate.draw_batch_selection_uniform (bench.py's rotation configs draw a fresh batch every step):
+    same recipe as draw_batch_selection("uniform") -- per sequence a target and n_dist DISTINCT distractors among the
+    candidates, every candidate equally likely at every position, n_dist ~ U{0..n_dist_max} -- checked as properties
+    and by frequencies over many draws."""
+    from workloads import CONFIGS
+    from workloads.generate import draw_batch_selection_uniform
+    cfg = CONFIGS["c_pages"]
+    rng = np.random.Generator(np.random.PCG64(7))
+    cand = np.arange(40, 240, dtype=np.int32)[::2]                  # 100 candidates, not 0..n-1
+    counts = np.zeros(cfg.n_dist_max + 2, np.int64)
+    first = np.zeros(400, np.int64)
+    for _ in range(300):
+        sel_off, sel_cart = draw_batch_selection_uniform(cfg, rng, cand)
+        assert sel_off[0] == 0 and len(sel_off) == cfg.B + 1 and sel_off[-1] == len(sel_cart)
+        assert np.isin(sel_cart, cand).all()
+        for b in range(cfg.B):
+            s = sel_cart[sel_off[b]:sel_off[b + 1]]
+            assert 1 <= len(s) <= cfg.n_dist_max + 1 and len(set(s.tolist())) == len(s)
+            counts[len(s)] += 1
+            first[s[0]] += 1
+    n = 300 * cfg.B
+    # list lengths 1..11 equally likely (binomial 5-sigma band), targets uniform over the candidates
+    exp = n / (cfg.n_dist_max + 1)
+    assert counts[0] == 0 and np.all(np.abs(counts[1:] - exp) < 5 * np.sqrt(exp))
+    f = first[cand]
+    assert first.sum() == f.sum() and np.all(np.abs(f - n / len(cand)) < 5 * np.sqrt(n / len(cand)))
+    # a fixed n_dist (config 3: target + 15 distractors of 64)
+    c3 = CONFIGS["c3"]
+    sel_off, sel_cart = draw_batch_selection_uniform(c3, rng, np.arange(64))
+    assert np.diff(sel_off).tolist() == [1 + c3.n_dist] * c3.B
